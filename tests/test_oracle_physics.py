@@ -1,0 +1,245 @@
+"""Pins for the oracle from closed forms and independent formulations (CPU only).
+
+ * Plane-wave dispersion on the vacuum (Higgs mode, transverse gauge mode): exact
+   solution of the linearised discrete equations, m^2 = lambda0 sigma^2 resp.
+   2 e0^2 sigma^2 (beta = 1) — fixes every dx and dt factor of Eqs. 7-10, 12-15.
+ * Leapfrog is O(dt^2): time-centred Minkowski energy, written
+   independently in numpy (tests/indep.py), oscillates ∝ dt^2 without drift.
+ * Vortex-antivortex pair: relaxes to a static solution with windings {+1,-1},
+   energy -> 2 mu L_z with mu = 2 pi sigma^2 at O(dx^2), <v^2> = 0.
+ * Winding (Eq. 16): brute-force integer formulation, flux
+   conservation, zero net flux through periodic planes, 1/3 density for random phases.
+ * Lagrangian-weighted sums (Eqs. 17-18): naive numpy evaluation.
+"""
+import numpy as np
+import pytest
+
+from tests import indep
+from paper_2005_14454_b200 import inputs
+
+
+# ------------------------------------------------------------------ dispersion
+
+def _omega_hat(kvec, dx, dt, m2):
+    lap = sum(4.0 / dx**2 * np.sin(0.5 * k * dx) ** 2 for k in kvec)
+    return 2.0 / dt * np.arcsin(0.5 * dt * np.sqrt(lap + m2))
+
+
+def test_dispersion_closed_form_value():
+    """The helper itself: k = (1,2,0)·2π/8, dx=.5, dt=.1, m²=2 gives 2.229951 (continuum 2.254828)."""
+    k = 2 * np.pi / 8.0 * np.array([1, 2, 0])
+    assert np.sqrt((k**2).sum() + 2.0) == pytest.approx(2.254828, abs=1e-6)
+    assert _omega_hat(k, 0.5, 0.1, 2.0) == pytest.approx(2.229951, abs=1e-6)
+
+
+@pytest.mark.parametrize("mode", ["higgs", "gauge"])
+def test_plane_wave_dispersion(oracle, mode):
+    o = oracle
+    nx, ny, nz, dx, dt, nsteps, amp = 8, 8, 4, 0.5, 0.1, 200, 1e-7
+    lam, e0, sig = 2.0, 1.0, 1.0
+    P = o.make_params(nx, ny, nz, dx=dx, lambda0=lam, e0=e0, sigma=sig, p=0.0, s=0.0)
+    kvec = 2 * np.pi / (np.array([nx, ny, nz]) * dx) * np.array([1, 2, 0])
+    z, y, x = np.meshgrid(np.arange(nz), np.arange(ny), np.arange(nx), indexing="ij")
+    kx = (kvec[0] * x + kvec[1] * y + kvec[2] * z) * dx
+    m2 = lam * sig**2 if mode == "higgs" else 2 * e0**2 * sig**2
+    w = _omega_hat(kvec, dx, dt, m2)
+
+    def wave(t):
+        return amp * np.cos(kx - w * t)
+
+    f = o.empty_fields(P)
+    f[0] = sig
+    comp, mom = (0, 2) if mode == "higgs" else (6, 9)     # gauge: polarisation z ⟂ k
+    f[comp] += wave(0.0)
+    f[mom] = (wave(0.0) - wave(-dt)) / dt                  # exact half-step momentum
+    o.step(P, f, nsteps, 1.0, dt)
+    got = f[comp] - (sig if mode == "higgs" else 0.0)
+    err = np.abs(got - wave(nsteps * dt)).max() / amp
+    assert err < (5e-6 if mode == "higgs" else 1e-9)       # Higgs: O(amp) nonlinearity
+    # a wrong mass (factor 2 in the current or the potential) dephases by O(1)
+    w_bad = _omega_hat(kvec, dx, dt, 2 * m2)
+    assert np.abs(got - amp * np.cos(kx - w_bad * nsteps * dt)).max() / amp > 0.1
+
+
+# ---------------------------------------------------------------------- energy
+
+def _centred_energy_track(o, P, f, nsteps, dt):
+    E = []
+    for _ in range(nsteps):
+        pi_old, ep_old = f[2:4].copy(), f[7:10].copy()
+        g = f.copy()
+        o.step(P, g, 1, 1.0, dt)
+        Pi_c = 0.5 * ((pi_old[0] + g[2]) + 1j * (pi_old[1] + g[3]))
+        ep_c = [0.5 * (ep_old[i] + g[7 + i]) for i in range(3)]
+        E.append(indep.energy(f, P.dx, P.lambda0, P.e0, P.sigma, 1.0, Pi=Pi_c, ep=ep_c))
+        f[...] = g
+    return np.array(E)
+
+
+def test_minkowski_energy_second_order(oracle):
+    o = oracle
+    n = 12
+    P = o.make_params(n, dx=0.5, p=0.0, s=0.0)
+    dev = []
+    for dt in (0.1, 0.05, 0.025):
+        f = inputs.smooth_state(n, n, n, seed=4)
+        E = _centred_energy_track(o, P, f, int(round(8.0 / dt)), dt)
+        dev.append(np.abs(E / E[0] - 1).max())
+        # no secular drift: last quarter's mean equals first quarter's mean to within the oscillation
+        q4 = len(E) // 4
+        assert abs(E[-q4:].mean() - E[:q4].mean()) / E[0] < dev[-1]
+    assert dev[0] < 2e-2
+    assert 3.0 < dev[0] / dev[1] < 5.0
+    assert 3.0 < dev[1] / dev[2] < 5.0
+
+
+# ----------------------------------------------------------------- vortex pair
+
+def _vortex_pair(o, nxy, dx, relax_steps):
+    P_relax = o.make_params(nxy, nxy, 1, dx=dx, p=1.0, s=0.0)   # delta = omega = dt/tau, q = 1
+    f = o.empty_fields(P_relax)
+    y, x = np.meshgrid(np.arange(nxy), np.arange(nxy), indexing="ij")
+    c1 = (nxy / 4 + 0.5, nxy / 2 + 0.5)
+    c2 = (3 * nxy / 4 + 0.5, nxy / 2 + 0.5)
+    r1 = np.hypot(x - c1[0], y - c1[1]) * dx
+    r2 = np.hypot(x - c2[0], y - c2[1]) * dx
+    a1 = np.arctan2(y - c1[1], x - c1[0])
+    a2 = np.arctan2(y - c2[1], x - c2[0])
+    phi = np.tanh(r1 / 1.2) * np.tanh(r2 / 1.2) * np.exp(1j * (a1 - a2))
+    f[0, 0], f[1, 0] = phi.real, phi.imag
+    dt = 0.2 * dx
+    delta = 0.15
+    for _ in range(relax_steps):
+        o.step(P_relax, f, 1, dt / delta, dt)                    # constant damping
+    return f, dt
+
+
+def _pair_energy(o, nxy, dx, relax_steps):
+    f, dt = _vortex_pair(o, nxy, dx, relax_steps)
+    P = o.make_params(nxy, nxy, 1, dx=dx, p=0.0, s=0.0)
+    d = o.diagnostics(P, f, 1.0, dt)
+    return P, f, dt, d
+
+
+def test_vortex_pair_static_and_tension(oracle):
+    o = oracle
+    P, f, dt, d = _pair_energy(o, 48, 0.5, 3000)
+    w, near = o.winding(P, f)
+    assert sorted(w[0].ravel()[w[0].ravel() != 0].tolist()) == [-1, 1]
+    assert not w[1].any() and not w[2].any()
+    assert d["n_wind"] == 2 and d["n_wind_xy"] == 2 and d["n_near_branch"] == 0 and d["n_big_plaq"] == 0
+    assert d["string_length"] == pytest.approx(2 * 0.5)
+    assert d["xi_w"] == pytest.approx(np.sqrt(48 * 48 * 0.5**3 / 1.0))
+    # relaxed: momenta tiny, Gauss holds, v^2 = 0
+    eps_relax = max(np.abs(f[2:4]).max(), np.abs(f[7:10]).max())
+    assert eps_relax < 1e-5
+    assert d["gauss_max"] < 1e-12
+    assert d["v2_phi"] < 1e-8
+    # energy = -sum L dx^3 = 2 mu Lz (1 - O(dx^2)), mu = 2 pi sigma^2
+    mu, Lz = 2 * np.pi, 0.5
+    deficit_coarse = 1 - (-d["sum_L"] * 0.5**3) / (2 * mu * Lz)
+    assert 0.005 < deficit_coarse < 0.02
+    # energy from the independent numpy expression agrees
+    assert indep.energy(f, 0.5, 2.0, 1.0, 1.0) == pytest.approx(-d["sum_L"] * 0.5**3, rel=1e-6)
+    # stays static under undamped Minkowski evolution
+    g = f.copy()
+    o.step(P, g, 100, 1.0, dt)
+    assert np.abs(g[0:2] - f[0:2]).max() < 1e-3
+    w2, _ = o.winding(P, g)
+    assert np.array_equal(w, w2)
+
+
+def test_vortex_pair_tension_converges_second_order(oracle):
+    o = oracle
+    mu = 2 * np.pi
+    _, _, _, d1 = _pair_energy(o, 32, 0.5, 2500)
+    _, _, _, d2 = _pair_energy(o, 64, 0.25, 5000)
+    def1 = 1 - (-d1["sum_L"] * 0.5**3) / (2 * mu * 0.5)
+    def2 = 1 - (-d2["sum_L"] * 0.25**3) / (2 * mu * 0.25)
+    assert 0 < def2 < def1
+    assert 3.0 < def1 / def2 < 5.5
+
+
+# --------------------------------------------------------------------- winding
+
+@pytest.mark.parametrize("shape", [(4, 4, 4), (6, 5, 4), (8, 8, 8), (7, 3, 5)])
+def test_winding_bruteforce(oracle, shape):
+    o = oracle
+    nx, ny, nz = shape
+    P = o.make_params(nx, ny, nz)
+    for seed in range(3):
+        f = inputs.random_state(nx, ny, nz, seed=100 + seed, th_amp=0.4, round_to_f32=False)
+        w, near = o.winding(P, f)
+        wb = indep.winding_bruteforce(f)
+        assert near.sum() == 0
+        assert np.array_equal(w.astype(np.int64), wb)
+        assert np.abs(w).sum() > 0
+        d = o.diagnostics(P, f, 1.0, 0.1)
+        assert d["n_wind"] == np.abs(wb).sum()
+        assert (d["n_wind_xy"], d["n_wind_xz"], d["n_wind_yz"]) == tuple(np.abs(wb[k]).sum() for k in range(3))
+
+
+def test_winding_flux_conservation_and_planes(oracle):
+    o = oracle
+    n = 16
+    P = o.make_params(n, dx=0.5, p=1.0, s=0.0)
+    f = o.init_fields(P, seed=7)
+    o.step(P, f, 25, 1.0, 0.1)
+    w, _ = o.winding(P, f)
+    w = w.astype(np.int64)
+    wxy, wxz, wyz = w
+    up = indep.up
+    div = (up(wxy, 2) - wxy) + (up(wyz, 0) - wyz) - (up(wxz, 1) - wxz)
+    assert not div.any()
+    assert np.abs(w).sum() > 50
+    assert not wxy.sum(axis=(1, 2)).any()     # each z-plane
+    assert not wxz.sum(axis=(0, 2)).any()     # each y-plane
+    assert not wyz.sum(axis=(0, 1)).any()     # each x-plane
+
+
+def test_winding_random_phase_density(oracle):
+    o = oracle
+    n = 32
+    P = o.make_params(n)
+    f = o.init_fields(P, seed=1)
+    d = o.diagnostics(P, f, 1.0, 0.1)
+    frac = d["n_wind"] / (3 * n**3)
+    assert abs(frac - 1 / 3) < 4 * np.sqrt((1 / 3) * (2 / 3) / (3 * n**3)) * 2
+
+
+def test_winding_near_branch_flag(oracle):
+    o = oracle
+    P = o.make_params(4)
+    f = o.empty_fields(P)
+    f[0] = 1.0
+    f[0, 1, 2, 3] = -1.0                      # phase difference exactly pi on its 6 links
+    d = o.diagnostics(P, f, 1.0, 0.1)
+    assert d["n_near_branch"] == 12           # the 12 plaquettes that have this site as a corner
+    f[4] = 3.2                                # |Phi| stays 0 for uniform theta
+    assert o.diagnostics(P, f, 1.0, 0.1)["n_big_plaq"] == 0
+    f[4, 0, 0, 0] = 0.0
+    assert o.diagnostics(P, f, 1.0, 0.1)["n_big_plaq"] > 0
+
+
+# -------------------------------------------------------------------- <v^2>_phi
+
+@pytest.mark.parametrize("case", [dict(p=0.0, s=0.0), dict(p=1.0, s=1.0, tau_ref=3.0), dict(p=2.0, s=0.5, tau_ref=2.0)])
+def test_lagrangian_sums_naive(oracle, case):
+    o = oracle
+    P = o.make_params(6, 5, 4, dx=0.5, lambda0=1.7, e0=0.8, sigma=1.1, **case)
+    f = inputs.random_state(6, 5, 4, seed=21, round_to_f32=False)
+    tau, dt = 1.7, 0.1
+    a, q, dl, om = o.coeffs(P, tau, dt)
+    d = o.diagnostics(P, f, tau, dt)
+    s_pi, s_gr, s_L = indep.lagrangian_sums(f, P.dx, P.lambda0, P.e0, P.sigma, q)
+    assert d["sum_pi2_L"] == pytest.approx(s_pi, rel=1e-11)
+    assert d["sum_grad2_L"] == pytest.approx(s_gr, rel=1e-11)
+    assert d["sum_L"] == pytest.approx(s_L, rel=1e-11)
+    R = s_pi / s_gr
+    assert d["v2_phi"] == pytest.approx(2 * R / (1 + R), rel=1e-11)
+    # Gauss residual of a generic (non-constraint-satisfying) state vs the numpy form
+    G, div, ch = indep.gauss_residual(f, P.dx, P.e0, q * (1 - dl) / (1 - om))
+    assert d["gauss_max"] == pytest.approx(np.abs(G).max(), rel=1e-12)
+    assert d["gauss_l2"] == pytest.approx(np.sqrt((G**2).sum()), rel=1e-12)
+    assert d["gauss_rel"] == pytest.approx(
+        np.sqrt((G**2).sum()) / (np.sqrt((div**2).sum()) + np.sqrt((ch**2).sum())), rel=1e-12)
