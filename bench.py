@@ -1,0 +1,328 @@
+#!/usr/bin/env python
+"""bench.py — site-updates/s of the fused Abelian-Higgs leapfrog step on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--size 1024] [--impl ours|reference]
+
+One "step" = one pass of the whole hot path over the lattice.  Workload at
+N=1: BASELINE.json configs[3] — 1024^3 periodic lattice, dx=0.5, dt=0.1, fp32 SoA with ping-pong
+buffers (85.9 GB), lambda=2, e=1, sigma=1, radiation era, s=1, seeded random-phase IC, no
+diagnostics.  The path does not shard: with --gpus N each
+rank evolves its own replica of the same lattice (a different seed), value = all ranks' site-updates
+divided by the slowest rank's device time, scaling "weak".
+
+Prints ONE JSON line on rank 0.  `--impl reference` times the fp64 CPU oracle (oracle/) on the host
+cores on a bounded sample of the same workload.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+from pathlib import Path
+
+ROOT = Path(__file__).resolve().parent
+sys.path.insert(0, str(ROOT))
+
+METRIC = "site-updates/sec at 1024^3 fp32 on 1 B200; % of HBM roofline (80 B/site)"
+UNIT = "site-updates/s"
+BYTES_PER_SITE = 80.0          # 10 fp32 read + 10 fp32 written
+DX, DT, TAU0 = 0.5, 0.1, 1.0
+NOMINAL_HBM_GBS = 8000.0       # the metric's own denominator (8 TB/s)
+FALLBACK_HBM_GBS = 6650.0      # B200_PROFILING.md fallback
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--warmup", type=int, default=20)
+    ap.add_argument("--size", type=int, default=1024, help="lattice extent N (N^3 sites)")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--kernel", default="auto", choices=["auto", "site", "tiled"])
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--diag-every", type=int, default=0, help="fused diagnostics every n steps (0 = none)")
+    return ap.parse_args()
+
+
+def workload_params(n, steps, warmup):
+    # configs[3]: radiation era (p=1), s=1; a(tau) normalised to 1 at the end of the run (reading #6)
+    return dict(dx=DX, lambda0=2.0, e0=1.0, sigma=1.0, s=1.0, p=1.0,
+                tau_ref=TAU0 + DT * (warmup + steps), alpha=2.0, compact=1)
+
+
+def measured_peak():
+    p = ROOT / "MEASURED_PEAKS.json"
+    if p.exists():
+        try:
+            return float(json.loads(p.read_text())["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+        except Exception:
+            pass
+    return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
+
+
+def recorded_traffic(n, kernel_name):
+    """DRAM bytes per launch of the dominant kernel from the committed ncu --set full capture, or None."""
+    p = ROOT / "profiles" / "traffic.json"
+    if not p.exists():
+        return None
+    try:
+        for rec in json.loads(p.read_text()):
+            if rec.get("size") == n and rec.get("kernel") == kernel_name:
+                return float(rec["dram_bytes_per_launch"])
+    except Exception:
+        return None
+    return None
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled every 200 ms while the timed region runs."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index = index
+        self.proc = None
+        self.lines = []
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "200"],
+                stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._pump, daemon=True)
+            self.thread.start()
+        except Exception:
+            self.proc = None
+
+    def _pump(self):
+        for line in self.proc.stdout:
+            self.lines.append(line.strip())
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons, power = [], [], set(), []
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for ln in self.lines:
+            parts = [x.strip() for x in ln.split(",")]
+            if len(parts) < 7:
+                continue
+            try:
+                sm.append(float(parts[0]))
+                mx.append(float(parts[1]))
+                power.append(float(parts[2]))
+            except ValueError:
+                continue
+            for name, val in zip(names, parts[3:7]):
+                if val.lower().startswith("active"):
+                    reasons.add(name)
+        sm.sort()
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "power_w_max": max(power) if power else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+# --------------------------------------------------------------------------- oracle (CPU) legs
+
+def oracle_rate(params, n_sample, steps, seed=1):
+    """Time the oracle, as it stands, for `steps` steps on an n_sample^3 lattice of the same workload."""
+    from oracle import ah_oracle as o
+    P = o.make_params(n_sample, **params)
+    f = o.init_fields(P, seed)
+    t0 = time.perf_counter()
+    o.step(P, f, steps, TAU0, DT)
+    el = time.perf_counter() - t0
+    return n_sample ** 3 * steps / el, el, o.num_threads()
+
+
+def cpu_baseline(params):
+    # ~10-30 s of CPU work: calibrate on 64^3, then run 256^3 (or 128^3 on a slow host) for a few steps
+    rate64, _, threads = oracle_rate(params, 64, 2)
+    n_s = 256 if rate64 > 1.5e6 else 128
+    steps = max(1, min(12, int(20.0 * rate64 * 3 / n_s ** 3)))   # larger lattices run ~3x the 64^3 rate
+    rate, el, threads = oracle_rate(params, n_s, steps)
+    return {"value": rate, "unit": UNIT, "cores": threads, "kind": "oracle",
+            "sample": f"{n_s}^3 sub-lattice of the same workload (same parameters, seeded random-phase IC), "
+                      f"{steps} leapfrog steps, fp64, gcc -O2 -fopenmp, {el:.1f} s",
+            "host_cpus": os.cpu_count()}
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    n = args.size
+    params = workload_params(n, args.steps, args.warmup)
+    from oracle import ah_oracle as o
+    rate64, _, threads = oracle_rate(params, 64, 2)
+    budget_s = 150.0
+    n_s = 64
+    for cand in (96, 128, 192, 256):
+        if (args.steps + args.warmup) * cand ** 3 / (rate64 * 3) <= budget_s:
+            n_s = cand
+    P = o.make_params(n_s, **params)
+    f = o.init_fields(P, 1)
+    o.step(P, f, args.warmup, TAU0, DT)
+    t0 = time.perf_counter()
+    o.step(P, f, args.steps, TAU0 + args.warmup * DT, DT)
+    el = time.perf_counter() - t0
+    value = n_s ** 3 * args.steps / el
+    sample = (f"each step = one oracle leapfrog step on a {n_s}^3 sub-lattice of the {n}^3 workload "
+              f"(same parameters and IC recipe), fp64, {threads} OpenMP threads")
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * el / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": f"{n}^3 periodic lattice, dx=0.5, dt=0.1, lambda=2, e=1, sigma=1, radiation era, s=1, "
+                               f"seeded random-phase IC, no diagnostics (BASELINE configs[3])", "sample": sample},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+    return 0
+
+
+# ------------------------------------------------------------------------------- CUDA arm
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    from paper_2005_14454_b200 import build, binding
+    build.build()
+
+    n, K, W = args.size, args.steps, args.warmup
+    params = workload_params(n, K, W)
+    sim = binding.Simulation(params=binding.make_params(n, **params), device=f"cuda:{local}")
+    if args.kernel != "auto":
+        sim.set_kernel({"site": binding.KERNEL_SITE, "tiled": binding.KERNEL_TILED}[args.kernel])
+    sites = float(n) ** 3
+    stream = sim.stream
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+            torch.cuda.synchronize()
+
+    def advance(nsteps, tau):
+        if args.diag_every > 0:
+            return len(sim.step_diag(nsteps, tau, DT, args.diag_every))
+        sim.step(nsteps, tau, DT)
+        return 0
+
+    # ---- device-resident throughput
+    sim.init_fields(1 + rank)
+    advance(max(W, 3), TAU0)
+    barrier()
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    l0 = sim.launch_count()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    ev0.record(stream)
+    advance(K, TAU0 + W * DT)
+    ev1.record(stream)
+    barrier()
+    ms = ev0.elapsed_time(ev1)
+    launches = sim.launch_count() - l0
+    clocks = sampler.stop() if rank == 0 else None
+    if world > 1:
+        t = torch.tensor([ms], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+    value = world * sites * K / (ms * 1e-3)
+
+    # ---- end to end through the C ABI with HOST buffers: upload, K steps, download
+    e2e = None
+    if not args.no_e2e:
+        nbytes = int(sites) * 10 * 4
+        try:
+            host = torch.empty(int(sites) * 10, dtype=torch.float32, pin_memory=True)
+            pinned = True
+        except Exception:
+            host = torch.empty(int(sites) * 10, dtype=torch.float32)
+            pinned = False
+        sim.get_fields_ptr(host.data_ptr())          # a real state as the host-side input
+        barrier()
+        t0 = time.perf_counter()
+        sim.set_fields_ptr(host.data_ptr())          # H2D inside the timed region
+        sim.step(K, TAU0 + W * DT, DT)
+        sim.get_fields_ptr(host.data_ptr())          # D2H (synchronises)
+        torch.cuda.synchronize()
+        el = time.perf_counter() - t0
+        if world > 1:
+            t = torch.tensor([el], device="cuda", dtype=torch.float64)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            el = float(t.item())
+        e2e = {"value": world * sites * K / el, "unit": UNIT, "h2d_bytes_per_step": nbytes / K,
+               "d2h_bytes_per_step": nbytes / K, "pinned_host": pinned, "seconds": el,
+               "what": f"ah_set_fields(host) + ah_step({K}) + ah_get_fields(host), wall clock"}
+        del host
+
+    if rank == 0:
+        peak, peak_src = measured_peak()
+        kernel_name = "tiled_step_kernel" if binding.lib() and args.kernel != "site" and n % 128 == 0 else "site_step_kernel"
+        step_launches = K
+        avg_launch_ms = ms / step_launches            # one step-kernel launch per step
+        achieved = BYTES_PER_SITE * sites / (avg_launch_ms * 1e-3) / 1e9
+        roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                    "traffic": recorded_traffic(n, kernel_name), "peak_source": peak_src, "kernel": kernel_name,
+                    "algorithmic_bytes_per_launch": BYTES_PER_SITE * sites,
+                    "frac_of_nominal_8TBs": achieved / NOMINAL_HBM_GBS,
+                    "timing": "CUDA events on the launching stream around the K timed launches; avg = elapsed/K"
+                              + (" (includes diagnostic launches)" if args.diag_every else "")}
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": max(W, 3),
+            "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f32", "data": "synthetic",
+            "config": {"workload": f"{n}^3 periodic lattice, dx=0.5, dt=0.1, fp32 SoA ping-pong ({20 * 4 * sites / 1e9:.1f} GB), "
+                                   f"lambda=2, e=1, sigma=1, radiation era, s=1, seeded random-phase IC, "
+                                   f"{'no diagnostics' if not args.diag_every else 'diagnostics every %d steps' % args.diag_every}"
+                                   f"{' (BASELINE configs[3])' if n == 1024 and not args.diag_every else ''}",
+                       "kernel": kernel_name, "parallelism": "replicas only" if world > 1 else "single GPU",
+                       "l2": "working set (80 B/site x N^3) exceeds the 126 MB L2 for N >= 128; no flush needed"
+                             if n >= 128 else "working set fits in L2 (small-lattice case)"},
+            "pct_of_8TBs_roofline": 100.0 * value / world * BYTES_PER_SITE / (NOMINAL_HBM_GBS * 1e9),
+            "roofline": roofline, "gpu_launches": int(launches), "clocks": clocks,
+        }
+        if e2e is not None:
+            line["e2e"] = e2e
+        if not args.no_cpu_baseline and world == 1:
+            line["cpu_baseline"] = cpu_baseline(params)
+        print(json.dumps(line), flush=True)
+    sim.close()
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
+def main():
+    args = parse()
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

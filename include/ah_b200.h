@@ -1,0 +1,156 @@
+/*
+ * ah_b200.h — C ABI of the B200 (sm_100a) Abelian-Higgs leapfrog library.
+ *
+ * Hot path of Correia & Martins, "Abelian-Higgs cosmic string evolution with
+ * multiple GPUs" (arXiv:2005.14454): the damped leapfrog step of the lattice
+ * U(1) gauge-Higgs model in an FRW background (Eqs. 7-11, with
+ * the stencils of Eqs. 12-15) and the network read-outs
+ * (winding, Eq. 16; Lagrangian-weighted <v^2>, PAPER.md:107-111
+ * Eqs. 17-18; Gauss law, Eq. 5 and :83).  Readings of the garbled
+ * or silent passages are listed in DESIGN.md ("Readings").
+ *
+ * Conventions
+ *   - One periodic nx*ny*nz lattice in ONE GPU's memory; site x=(x,y,z) has
+ *     linear index x + nx*(y + ny*z) (x fastest).
+ *   - State = 10 real scalars per site, structure-of-arrays, in this order:
+ *       0 phi_re 1 phi_im 2 pi_re 3 pi_im 4 th_x 5 th_y 6 th_z 7 ep_x 8 ep_y 9 ep_z
+ *     th_i(x) is the paper's lattice link angle A_i(x) of Eq. 12 (U_i = exp(-i th_i)),
+ *     ep_i(x) the paper's lattice E_i(x) of Eq. 10 (= d th_i / d tau).
+ *   - phi, th live at tau_k; Pi, ep at tau_k - dt/2.
+ *   - All pointers named dev_* are DEVICE pointers, host_* are HOST pointers.
+ *   - Every function returns 0 on success or a negative AH_E* code; no C++
+ *     exception crosses this boundary; ah_last_error() gives a message for the
+ *     calling thread's most recent failure.
+ *   - Nothing here falls back to the CPU: without a CUDA device every compute
+ *     entry point returns AH_ECUDA.
+ */
+#ifndef AH_B200_H
+#define AH_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define AH_OK 0
+#define AH_EINVAL (-1) /* bad parameter, null pointer, tau <= 0 with p != 0, cap too small */
+#define AH_ECUDA (-2)  /* CUDA runtime failure (message in ah_last_error)                 */
+#define AH_ESTATE (-3) /* call made in the wrong state (e.g. stepping before any fields)  */
+
+#define AH_NFIELDS 10
+
+/* kernel selection for ah_set_kernel */
+#define AH_KERNEL_AUTO 0  /* fused tiled kernel when the lattice allows it, else the site kernel */
+#define AH_KERNEL_SITE 1  /* one thread per site, neighbours through L1/L2 (any nx,ny,nz >= 1) */
+#define AH_KERNEL_TILED 2 /* z-marching register/shared-memory tiled kernel (needs nx % 128 == 0) */
+
+typedef struct ah_ctx ah_ctx; /* opaque */
+
+/* Model and lattice parameters.  Plain data, host side. */
+typedef struct {
+    int32_t nx, ny, nz; /* periodic extents, each >= 1                                             */
+    double dx;          /* lattice spacing (0.5 in the paper)                          */
+    double lambda0, e0, sigma; /* couplings (2, 1, 1: critical coupling)              */
+    double s;           /* core-growth exponent of Eq. 6: 0 constant comoving width, 1 physical     */
+    double p;           /* dln a/dln tau = m/(1-m) (Eq. 11): 0 Minkowski, 1 radiation, 2 matter      */
+    double tau_ref;     /* a(tau) = (tau/tau_ref)^p (reading #6); ignored when p == 0 or s == 0      */
+    double alpha;       /* damping constant of PAPER.md:78; 2 = physical Hubble damping              */
+    int32_t compact;    /* 1: sin(plaquette) force, 2(1-cos) energy (reading #10); 0: non-compact     */
+    int32_t fp64;       /* 0: fp32 state and arithmetic (the product); 1: fp64 state, site kernel only */
+} ah_params;
+
+/* Diagnostics of one snapshot. */
+typedef struct {
+    double tau;
+    int64_t n_wind, n_wind_xy, n_wind_xz, n_wind_yz; /* sum |W_ij| (Eq. 16 right)                   */
+    int64_t n_near_branch; /* plaquettes with a link phase within 1e-5 of +-pi (reading #14)        */
+    int64_t n_big_plaq;    /* plaquettes with |Phi_ij| > pi - 1e-5 (reading #13)                    */
+    double string_length, xi_w; /* dx*n_wind ; sqrt(V/L_W), +inf when n_wind == 0                   */
+    double sum_pi2_L, sum_grad2_L, sum_L, v2_phi; /* Eqs. 17-18                                      */
+    double gauss_max, gauss_l2, gauss_rel;        /* Eq. 5 residual                                  */
+    double gauss_div_l2, gauss_charge_l2;
+} ah_diag;
+
+/*
+ * ah_create — make a context on the current CUDA device.
+ *   dev_bufs : 2*AH_NFIELDS caller-owned device arrays (e.g. PyTorch tensors), each of
+ *              nx*ny*nz elements (float, or double when params->fp64), 16-byte aligned.
+ *              Buffers [0,10) hold the current state (order above); [10,20) are the
+ *              ping-pong partners.  The context only borrows them: it never frees them,
+ *              and they must outlive it.  After an odd number of steps the current state
+ *              lives in [10,20); use ah_current_bufs / ah_get_fields, never assume.
+ *   nbufs    : must be 20.   bytes_each: must equal nx*ny*nz*sizeof(element).
+ *   cuda_stream : a cudaStream_t (0 = legacy default stream); all work is enqueued on it.
+ * Allocates only small context-owned scratch (reduction partials, a few hundred KB).
+ */
+int ah_create(ah_ctx **out, const ah_params *params, void *const dev_bufs[], int nbufs,
+              size_t bytes_each, void *cuda_stream);
+
+/* Frees context-owned scratch only, never the field buffers.  NULL is a no-op. */
+int ah_destroy(ah_ctx *ctx);
+
+/* I0: phi = sigma*exp(2 pi i u(seed, linear index)), Pi = th = ep = 0, with the
+ * counter-based u of DESIGN.md "I0".  Asynchronous on the stream.  Resets the ping-pong parity. */
+int ah_init_fields(ah_ctx *ctx, uint64_t seed);
+
+/* Upload / download a snapshot: host_soa10 holds 10 contiguous arrays of nx*ny*nz elements
+ * (float or double as the context) in the field order above.  Both synchronise the stream. */
+int ah_set_fields(ah_ctx *ctx, const void *host_soa10);
+int ah_get_fields(ah_ctx *ctx, void *host_soa10);
+
+/* Which 10 device pointers hold the current state (ping-pong parity resolved). */
+int ah_current_bufs(ah_ctx *ctx, void *dev_ptrs_out[AH_NFIELDS]);
+
+/*
+ * ah_step — advance n leapfrog steps (Eqs. 7-10) starting from conformal time tau, with phi, th
+ * at tau and Pi, ep at tau - dt/2.  Step j uses the coefficients (a, delta, omega of
+ * PAPER.md:78-80) at tau_j = tau + j*dt, the product evaluated in fp64.  Asynchronous on the
+ * stream; allocates nothing.  n == 0 is a no-op.  AH_EINVAL if n < 0, dt <= 0 or (p != 0 and
+ * tau <= 0); AH_ESTATE if no fields were ever set.
+ */
+int ah_step(ah_ctx *ctx, int n, double tau, double dt);
+
+/* Diagnostics D1-D3 of the current snapshot (fields at tau, momenta at tau - dt/2).
+ * Synchronous: returns after the result is in *host_out. */
+int ah_diagnostics(ah_ctx *ctx, double tau, double dt, ah_diag *host_out);
+
+/*
+ * ah_step_diag — n steps with diagnostics of the ENTRY snapshot of every step j with
+ * j % every == 0 (SURVEY 8(a) row D-fuse): identical to calling ah_diagnostics(tau_j) before
+ * step j.  Records are written to host_out[0..*n_written).  AH_EINVAL, without stepping, when
+ * cap < ceil(n/every) or every < 1.  Synchronous at return.
+ */
+int ah_step_diag(ah_ctx *ctx, int n, double tau, double dt, int every, ah_diag *host_out, int cap,
+                 int *n_written);
+
+/* Per-plaquette winding integers of the current snapshot: host_w3 receives 3 arrays (xy, xz, yz)
+ * of nx*ny*nz int8; host_near3 (may be NULL) the near-branch flags as uint8.  Synchronous. */
+int ah_winding_field(ah_ctx *ctx, int8_t *host_w3, uint8_t *host_near3);
+
+/* Choose the step kernel (AH_KERNEL_*).  AH_EINVAL if the lattice does not allow it. */
+int ah_set_kernel(ah_ctx *ctx, int kernel);
+
+/* Number of kernel launches this context has enqueued since creation (bench.py's gpu_launches). */
+int64_t ah_launch_count(const ah_ctx *ctx);
+
+/* Host-side coefficients as the kernels receive them (for tests): a, q = a^{2s}, delta, omega. */
+int ah_coeffs(const ah_params *params, double tau, double dt, double *a, double *q, double *delta,
+              double *omega);
+
+/* Device-side evaluation of the library's fp32 sin/cos kernels' math (tests only): for each of the
+ * n device floats in dev_x writes sin and cos as used for link variables, and the plaquette sine. */
+int ah_test_trig(const float *dev_x, float *dev_sin, float *dev_cos, float *dev_plaq_sin, size_t n,
+                 void *cuda_stream);
+
+/* Message for the calling thread's most recent error ("" if none).  Never NULL. */
+const char *ah_last_error(void);
+
+/* Library version string. */
+const char *ah_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* AH_B200_H */

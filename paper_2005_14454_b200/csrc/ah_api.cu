@@ -1,0 +1,468 @@
+// ah_api.cu — the C ABI of include/ah_b200.h: argument checking, per-step coefficients on the
+// host in fp64, kernel launches on the caller's stream.  No field arithmetic happens here.
+#include "../../include/ah_b200.h"
+
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <limits>
+#include <new>
+
+#include "ah_kernels.h"
+
+namespace {
+
+thread_local char g_err[512] = "";
+
+int fail(int code, const char *fmt, ...)
+{
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof(g_err), fmt, ap);
+    va_end(ap);
+    return code;
+}
+
+int cuda_fail(cudaError_t e, const char *what)
+{
+    return fail(AH_ECUDA, "%s: %s (%s)", what, cudaGetErrorString(e), cudaGetErrorName(e));
+}
+
+#define AH_CUDA(call)                                       \
+    do {                                                    \
+        cudaError_t e__ = (call);                           \
+        if (e__ != cudaSuccess) return cuda_fail(e__, #call); \
+    } while (0)
+
+// PAPER.md:78-80 with readings #4-#6: a = (tau/tau_ref)^p, q = a^{2s},
+// delta = (alpha/2) p dt / tau, omega = (1-s) delta.
+void coeffs(const ah_params &P, double tau, double dt, double &a, double &q, double &delta,
+            double &omega)
+{
+    a = (P.p == 0.0) ? 1.0 : std::pow(tau / P.tau_ref, P.p);
+    q = (P.s == 0.0) ? 1.0 : std::pow(a, 2.0 * P.s);
+    delta = (P.p == 0.0) ? 0.0 : 0.5 * P.alpha * P.p * dt / tau;
+    omega = delta * (1.0 - P.s);
+}
+
+template <typename real>
+ah::StepCoef<real> make_coef(const ah_params &P, double tau, double dt)
+{
+    double a, q, d, w;
+    coeffs(P, tau, dt, a, q, d, w);
+    ah::StepCoef<real> k;
+    k.idx2 = (real)(1.0 / (P.dx * P.dx));
+    k.c1 = (real)((1.0 - d) / (1.0 + d));
+    k.c2 = (real)(dt / (1.0 + d));
+    k.w1 = (real)((1.0 - w) / (1.0 + w));
+    k.w2 = (real)(dt / (1.0 + w));
+    k.half_lam_q = (real)(0.5 * P.lambda0 * q);
+    k.sig2 = (real)(P.sigma * P.sigma);
+    k.two_e2_q = (real)(2.0 * P.e0 * P.e0 * q);
+    k.dt = (real)dt;
+    k.compact = P.compact;
+    return k;
+}
+
+ah::DiagCoef make_diag_coef(const ah_params &P, double tau, double dt)
+{
+    double a, q, d, w;
+    coeffs(P, tau, dt, a, q, d, w);
+    ah::DiagCoef k;
+    k.idx2 = 1.0 / (P.dx * P.dx);
+    k.q = q;
+    k.quarter_lam_q = 0.25 * P.lambda0 * q;
+    k.sig2 = P.sigma * P.sigma;
+    k.inv_2e2q = 1.0 / (2.0 * P.e0 * P.e0 * q);
+    k.two_e2_kappa = 2.0 * P.e0 * P.e0 * q * (1.0 - d) / (1.0 - w);  // reading #18
+    k.compact = P.compact;
+    return k;
+}
+
+}  // namespace
+
+struct ah_ctx {
+    ah_params P;
+    void *bufs[2 * AH_NFIELDS];
+    int cur;           // 0: state in bufs[0..10), 1: in bufs[10..20)
+    bool have_fields;
+    cudaStream_t st;
+    size_t n;          // sites
+    size_t elem;       // bytes per element
+    int kernel;        // resolved AH_KERNEL_SITE / AH_KERNEL_TILED
+    int64_t launches;
+    ah::DiagPartial *d_partials;
+    int n_partials;
+    ah::DiagPartial *d_results;
+    ah::DiagPartial *h_results;  // pinned
+    int cap_results;
+};
+
+namespace {
+
+template <typename real>
+ah::ConstFields<real> cur_fields(const ah_ctx *c)
+{
+    ah::ConstFields<real> f;
+    for (int a = 0; a < AH_NFIELDS; ++a) f.f[a] = (const real *)c->bufs[c->cur * AH_NFIELDS + a];
+    return f;
+}
+template <typename real>
+ah::Fields<real> next_fields(const ah_ctx *c)
+{
+    ah::Fields<real> f;
+    for (int a = 0; a < AH_NFIELDS; ++a) f.f[a] = (real *)c->bufs[(1 - c->cur) * AH_NFIELDS + a];
+    return f;
+}
+template <typename real>
+ah::Fields<real> cur_fields_mut(const ah_ctx *c)
+{
+    ah::Fields<real> f;
+    for (int a = 0; a < AH_NFIELDS; ++a) f.f[a] = (real *)c->bufs[c->cur * AH_NFIELDS + a];
+    return f;
+}
+
+int check_time(const ah_ctx *c, double tau, double dt)
+{
+    if (!(dt > 0.0) || !std::isfinite(dt) || !std::isfinite(tau))
+        return fail(AH_EINVAL, "dt must be positive and finite (dt=%g, tau=%g)", dt, tau);
+    if (c->P.p != 0.0 && !(tau > 0.0))
+        return fail(AH_EINVAL, "tau must be > 0 in an expanding background (tau=%g, p=%g)", tau, c->P.p);
+    return AH_OK;
+}
+
+int one_step(ah_ctx *c, double tau, double dt)
+{
+    cudaError_t e;
+    const ah_params &P = c->P;
+    if (P.fp64) {
+        e = ah::launch_site_step<double>(cur_fields<double>(c), next_fields<double>(c),
+                                         make_coef<double>(P, tau, dt), P.nx, P.ny, P.nz, c->st);
+    } else if (c->kernel == AH_KERNEL_TILED) {
+        e = ah::launch_tiled_step(cur_fields<float>(c), next_fields<float>(c),
+                                  make_coef<float>(P, tau, dt), P.nx, P.ny, P.nz, c->st);
+    } else {
+        e = ah::launch_site_step<float>(cur_fields<float>(c), next_fields<float>(c),
+                                        make_coef<float>(P, tau, dt), P.nx, P.ny, P.nz, c->st);
+    }
+    if (e != cudaSuccess) return cuda_fail(e, "step kernel launch");
+    c->launches += 1;
+    c->cur = 1 - c->cur;
+    return AH_OK;
+}
+
+int ensure_diag_scratch(ah_ctx *c, int records)
+{
+    const int nb = ah::diag_num_blocks(c->P.nx, c->P.ny, c->P.nz);
+    if (c->n_partials < nb) {
+        if (c->d_partials) cudaFree(c->d_partials);
+        c->d_partials = nullptr;
+        c->n_partials = 0;
+        AH_CUDA(cudaMalloc(&c->d_partials, sizeof(ah::DiagPartial) * (size_t)nb));
+        c->n_partials = nb;
+    }
+    if (c->cap_results < records) {
+        if (c->d_results) cudaFree(c->d_results);
+        if (c->h_results) cudaFreeHost(c->h_results);
+        c->d_results = nullptr;
+        c->h_results = nullptr;
+        c->cap_results = 0;
+        int cap = records < 256 ? 256 : records;
+        AH_CUDA(cudaMalloc(&c->d_results, sizeof(ah::DiagPartial) * (size_t)cap));
+        AH_CUDA(cudaMallocHost(&c->h_results, sizeof(ah::DiagPartial) * (size_t)cap));
+        c->cap_results = cap;
+    }
+    return AH_OK;
+}
+
+int enqueue_diag(ah_ctx *c, double tau, double dt, int slot, int8_t *w3, uint8_t *near3)
+{
+    const ah_params &P = c->P;
+    const ah::DiagCoef k = make_diag_coef(P, tau, dt);
+    cudaError_t e;
+    if (P.fp64)
+        e = ah::launch_diag<double>(cur_fields<double>(c), k, P.nx, P.ny, P.nz, c->d_partials,
+                                    c->d_results + slot, w3, near3, c->st);
+    else
+        e = ah::launch_diag<float>(cur_fields<float>(c), k, P.nx, P.ny, P.nz, c->d_partials,
+                                   c->d_results + slot, w3, near3, c->st);
+    if (e != cudaSuccess) return cuda_fail(e, "diagnostics kernel launch");
+    c->launches += 2;
+    return AH_OK;
+}
+
+void finish_diag(const ah_ctx *c, const ah::DiagPartial &r, double tau, ah_diag *out)
+{
+    const ah_params &P = c->P;
+    out->tau = tau;
+    out->n_wind_xy = r.i[ah::DS_NW_XY];
+    out->n_wind_xz = r.i[ah::DS_NW_XZ];
+    out->n_wind_yz = r.i[ah::DS_NW_YZ];
+    out->n_wind = out->n_wind_xy + out->n_wind_xz + out->n_wind_yz;
+    out->n_near_branch = r.i[ah::DS_NEAR];
+    out->n_big_plaq = r.i[ah::DS_BIG];
+    out->string_length = P.dx * (double)out->n_wind;   // L_W = dx * n_W (reading #13)
+    const double V = (double)P.nx * P.ny * P.nz * P.dx * P.dx * P.dx;
+    out->xi_w = out->n_wind > 0 ? std::sqrt(V / out->string_length)
+                                : std::numeric_limits<double>::infinity();
+    out->sum_pi2_L = r.f[ah::DF_SPI];
+    out->sum_grad2_L = r.f[ah::DF_SGR];
+    out->sum_L = r.f[ah::DF_SL];
+    if (out->sum_grad2_L != 0.0) {
+        const double R = out->sum_pi2_L / out->sum_grad2_L;   // Eq. 18
+        out->v2_phi = 2.0 * R / (1.0 + R);                    // Eq. 17 left
+    } else {
+        out->v2_phi = 0.0;
+    }
+    out->gauss_max = r.f[ah::DF_GMAX];
+    out->gauss_l2 = std::sqrt(r.f[ah::DF_GSQ]);
+    out->gauss_div_l2 = std::sqrt(r.f[ah::DF_DIVSQ]);
+    out->gauss_charge_l2 = std::sqrt(r.f[ah::DF_CHSQ]);
+    const double den = out->gauss_div_l2 + out->gauss_charge_l2;
+    out->gauss_rel = den > 0.0 ? out->gauss_l2 / den : 0.0;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char *ah_last_error(void) { return g_err; }
+const char *ah_version(void) { return "ah_b200 0.1 (sm_100a)"; }
+
+int ah_coeffs(const ah_params *P, double tau, double dt, double *a, double *q, double *delta,
+              double *omega)
+{
+    if (!P || !a || !q || !delta || !omega) return fail(AH_EINVAL, "ah_coeffs: null pointer");
+    if (P->p != 0.0 && !(tau > 0.0)) return fail(AH_EINVAL, "ah_coeffs: tau must be > 0 when p != 0");
+    coeffs(*P, tau, dt, *a, *q, *delta, *omega);
+    return AH_OK;
+}
+
+int ah_create(ah_ctx **out, const ah_params *P, void *const dev_bufs[], int nbufs, size_t bytes_each,
+              void *cuda_stream)
+{
+    if (!out || !P || !dev_bufs) return fail(AH_EINVAL, "ah_create: null pointer");
+    *out = nullptr;
+    if (P->nx < 1 || P->ny < 1 || P->nz < 1)
+        return fail(AH_EINVAL, "ah_create: extents must be >= 1 (%d,%d,%d)", P->nx, P->ny, P->nz);
+    if (!(P->dx > 0.0) || !(P->e0 != 0.0) || !(P->alpha >= 0.0) || !std::isfinite(P->lambda0) ||
+        !std::isfinite(P->sigma) || !std::isfinite(P->s) || !std::isfinite(P->p))
+        return fail(AH_EINVAL, "ah_create: bad model parameters");
+    if (P->p != 0.0 && P->s != 0.0 && !(P->tau_ref > 0.0))
+        return fail(AH_EINVAL, "ah_create: tau_ref must be > 0 when p != 0 and s != 0");
+    if (nbufs != 2 * AH_NFIELDS) return fail(AH_EINVAL, "ah_create: nbufs must be 20 (got %d)", nbufs);
+    const size_t n = (size_t)P->nx * P->ny * P->nz;
+    const size_t elem = P->fp64 ? sizeof(double) : sizeof(float);
+    if (bytes_each != n * elem)
+        return fail(AH_EINVAL, "ah_create: bytes_each=%zu but nx*ny*nz*sizeof(elem)=%zu", bytes_each, n * elem);
+    for (int i = 0; i < nbufs; ++i) {
+        if (!dev_bufs[i]) return fail(AH_EINVAL, "ah_create: dev_bufs[%d] is null", i);
+        if (((uintptr_t)dev_bufs[i]) & 15u)
+            return fail(AH_EINVAL, "ah_create: dev_bufs[%d] is not 16-byte aligned", i);
+        for (int j = 0; j < i; ++j)
+            if (dev_bufs[i] == dev_bufs[j]) return fail(AH_EINVAL, "ah_create: dev_bufs[%d] == dev_bufs[%d]", i, j);
+    }
+    int ndev = 0;
+    AH_CUDA(cudaGetDeviceCount(&ndev));
+    if (ndev < 1) return fail(AH_ECUDA, "ah_create: no CUDA device");
+
+    ah_ctx *c = new (std::nothrow) ah_ctx;
+    if (!c) return fail(AH_ECUDA, "ah_create: out of host memory");
+    std::memset(c, 0, sizeof(*c));
+    c->P = *P;
+    for (int i = 0; i < nbufs; ++i) c->bufs[i] = dev_bufs[i];
+    c->st = (cudaStream_t)cuda_stream;
+    c->n = n;
+    c->elem = elem;
+    c->kernel = (!P->fp64 && ah::tiled_supported(P->nx, P->ny, P->nz)) ? AH_KERNEL_TILED : AH_KERNEL_SITE;
+    if (c->kernel == AH_KERNEL_TILED) {
+        cudaError_t e = ah::tiled_setup();
+        if (e != cudaSuccess) {
+            delete c;
+            return cuda_fail(e, "tiled kernel setup");
+        }
+    }
+    int rc = ensure_diag_scratch(c, 256);
+    if (rc != AH_OK) {
+        ah_destroy(c);
+        return rc;
+    }
+    *out = c;
+    return AH_OK;
+}
+
+int ah_destroy(ah_ctx *c)
+{
+    if (!c) return AH_OK;
+    if (c->d_partials) cudaFree(c->d_partials);
+    if (c->d_results) cudaFree(c->d_results);
+    if (c->h_results) cudaFreeHost(c->h_results);
+    delete c;
+    return AH_OK;
+}
+
+int ah_set_kernel(ah_ctx *c, int kernel)
+{
+    if (!c) return fail(AH_EINVAL, "ah_set_kernel: null context");
+    const bool can_tile = !c->P.fp64 && ah::tiled_supported(c->P.nx, c->P.ny, c->P.nz);
+    if (kernel == AH_KERNEL_AUTO) kernel = can_tile ? AH_KERNEL_TILED : AH_KERNEL_SITE;
+    if (kernel == AH_KERNEL_TILED) {
+        if (!can_tile) return fail(AH_EINVAL, "ah_set_kernel: tiled kernel needs fp32 and nx %% 128 == 0");
+        AH_CUDA(ah::tiled_setup());
+    } else if (kernel != AH_KERNEL_SITE) {
+        return fail(AH_EINVAL, "ah_set_kernel: unknown kernel %d", kernel);
+    }
+    c->kernel = kernel;
+    return AH_OK;
+}
+
+int64_t ah_launch_count(const ah_ctx *c) { return c ? c->launches : 0; }
+
+int ah_init_fields(ah_ctx *c, uint64_t seed)
+{
+    if (!c) return fail(AH_EINVAL, "ah_init_fields: null context");
+    c->cur = 0;
+    cudaError_t e = c->P.fp64 ? ah::launch_init<double>(cur_fields_mut<double>(c), seed, c->P.sigma, c->n, c->st)
+                              : ah::launch_init<float>(cur_fields_mut<float>(c), seed, c->P.sigma, c->n, c->st);
+    if (e != cudaSuccess) return cuda_fail(e, "init kernel launch");
+    c->launches += 1;
+    c->have_fields = true;
+    return AH_OK;
+}
+
+int ah_set_fields(ah_ctx *c, const void *host)
+{
+    if (!c || !host) return fail(AH_EINVAL, "ah_set_fields: null pointer");
+    c->cur = 0;
+    const size_t bytes = c->n * c->elem;
+    for (int a = 0; a < AH_NFIELDS; ++a)
+        AH_CUDA(cudaMemcpyAsync(c->bufs[a], (const char *)host + bytes * a, bytes, cudaMemcpyHostToDevice, c->st));
+    AH_CUDA(cudaStreamSynchronize(c->st));
+    c->have_fields = true;
+    return AH_OK;
+}
+
+int ah_get_fields(ah_ctx *c, void *host)
+{
+    if (!c || !host) return fail(AH_EINVAL, "ah_get_fields: null pointer");
+    if (!c->have_fields) return fail(AH_ESTATE, "ah_get_fields: no fields were set");
+    const size_t bytes = c->n * c->elem;
+    for (int a = 0; a < AH_NFIELDS; ++a)
+        AH_CUDA(cudaMemcpyAsync((char *)host + bytes * a, c->bufs[c->cur * AH_NFIELDS + a], bytes,
+                                cudaMemcpyDeviceToHost, c->st));
+    AH_CUDA(cudaStreamSynchronize(c->st));
+    return AH_OK;
+}
+
+int ah_current_bufs(ah_ctx *c, void *out[AH_NFIELDS])
+{
+    if (!c || !out) return fail(AH_EINVAL, "ah_current_bufs: null pointer");
+    for (int a = 0; a < AH_NFIELDS; ++a) out[a] = c->bufs[c->cur * AH_NFIELDS + a];
+    return AH_OK;
+}
+
+int ah_step(ah_ctx *c, int n, double tau, double dt)
+{
+    if (!c) return fail(AH_EINVAL, "ah_step: null context");
+    if (n < 0) return fail(AH_EINVAL, "ah_step: n must be >= 0 (got %d)", n);
+    if (!c->have_fields) return fail(AH_ESTATE, "ah_step: no fields were set");
+    int rc = check_time(c, tau, dt);
+    if (rc != AH_OK) return rc;
+    for (int j = 0; j < n; ++j) {
+        rc = one_step(c, tau + (double)j * dt, dt);
+        if (rc != AH_OK) return rc;
+    }
+    return AH_OK;
+}
+
+int ah_diagnostics(ah_ctx *c, double tau, double dt, ah_diag *out)
+{
+    if (!c || !out) return fail(AH_EINVAL, "ah_diagnostics: null pointer");
+    if (!c->have_fields) return fail(AH_ESTATE, "ah_diagnostics: no fields were set");
+    int rc = check_time(c, tau, dt);
+    if (rc != AH_OK) return rc;
+    rc = ensure_diag_scratch(c, 1);
+    if (rc != AH_OK) return rc;
+    rc = enqueue_diag(c, tau, dt, 0, nullptr, nullptr);
+    if (rc != AH_OK) return rc;
+    AH_CUDA(cudaMemcpyAsync(c->h_results, c->d_results, sizeof(ah::DiagPartial), cudaMemcpyDeviceToHost, c->st));
+    AH_CUDA(cudaStreamSynchronize(c->st));
+    finish_diag(c, c->h_results[0], tau, out);
+    return AH_OK;
+}
+
+int ah_step_diag(ah_ctx *c, int n, double tau, double dt, int every, ah_diag *out, int cap, int *n_written)
+{
+    if (!c || !out || !n_written) return fail(AH_EINVAL, "ah_step_diag: null pointer");
+    *n_written = 0;
+    if (n < 0 || every < 1) return fail(AH_EINVAL, "ah_step_diag: need n >= 0 and every >= 1");
+    if (!c->have_fields) return fail(AH_ESTATE, "ah_step_diag: no fields were set");
+    int rc = check_time(c, tau, dt);
+    if (rc != AH_OK) return rc;
+    const int records = (n + every - 1) / every;
+    if (cap < records) return fail(AH_EINVAL, "ah_step_diag: cap=%d < %d records", cap, records);
+    rc = ensure_diag_scratch(c, records);
+    if (rc != AH_OK) return rc;
+    int r = 0;
+    for (int j = 0; j < n; ++j) {
+        const double tj = tau + (double)j * dt;
+        if (j % every == 0) {
+            rc = enqueue_diag(c, tj, dt, r, nullptr, nullptr);
+            if (rc != AH_OK) return rc;
+            ++r;
+        }
+        rc = one_step(c, tj, dt);
+        if (rc != AH_OK) return rc;
+    }
+    if (r > 0)
+        AH_CUDA(cudaMemcpyAsync(c->h_results, c->d_results, sizeof(ah::DiagPartial) * (size_t)r,
+                                cudaMemcpyDeviceToHost, c->st));
+    AH_CUDA(cudaStreamSynchronize(c->st));
+    for (int i = 0; i < r; ++i) finish_diag(c, c->h_results[i], tau + (double)(i * every) * dt, out + i);
+    *n_written = r;
+    return AH_OK;
+}
+
+int ah_winding_field(ah_ctx *c, int8_t *host_w3, uint8_t *host_near3)
+{
+    if (!c || !host_w3) return fail(AH_EINVAL, "ah_winding_field: null pointer");
+    if (!c->have_fields) return fail(AH_ESTATE, "ah_winding_field: no fields were set");
+    int rc = ensure_diag_scratch(c, 1);
+    if (rc != AH_OK) return rc;
+    int8_t *d_w = nullptr;
+    uint8_t *d_near = nullptr;
+    AH_CUDA(cudaMalloc(&d_w, 3 * c->n));
+    if (host_near3) {
+        cudaError_t e = cudaMalloc(&d_near, 3 * c->n);
+        if (e != cudaSuccess) {
+            cudaFree(d_w);
+            return cuda_fail(e, "cudaMalloc near flags");
+        }
+    }
+    // winding does not depend on tau; any admissible time gives the same integers
+    rc = enqueue_diag(c, 1.0, 1.0, 0, d_w, d_near);
+    cudaError_t e = cudaSuccess;
+    if (rc == AH_OK) e = cudaMemcpyAsync(host_w3, d_w, 3 * c->n, cudaMemcpyDeviceToHost, c->st);
+    if (rc == AH_OK && e == cudaSuccess && host_near3)
+        e = cudaMemcpyAsync(host_near3, d_near, 3 * c->n, cudaMemcpyDeviceToHost, c->st);
+    cudaError_t e2 = cudaStreamSynchronize(c->st);
+    cudaFree(d_w);
+    if (d_near) cudaFree(d_near);
+    if (rc != AH_OK) return rc;
+    if (e != cudaSuccess) return cuda_fail(e, "winding field download");
+    if (e2 != cudaSuccess) return cuda_fail(e2, "cudaStreamSynchronize");
+    return AH_OK;
+}
+
+int ah_test_trig(const float *dev_x, float *dev_sin, float *dev_cos, float *dev_plaq_sin, size_t n,
+                 void *cuda_stream)
+{
+    if (!dev_x || !dev_sin || !dev_cos || !dev_plaq_sin) return fail(AH_EINVAL, "ah_test_trig: null pointer");
+    if (n == 0) return AH_OK;
+    cudaError_t e = ah::launch_test_trig(dev_x, dev_sin, dev_cos, dev_plaq_sin, n, (cudaStream_t)cuda_stream);
+    if (e != cudaSuccess) return cuda_fail(e, "trig test kernel launch");
+    return AH_OK;
+}
+
+}  // extern "C"

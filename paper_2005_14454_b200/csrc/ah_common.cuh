@@ -1,0 +1,153 @@
+// ah_common.cuh — shared device-side definitions of the B200 Abelian-Higgs library.
+//
+// Notation follows the paper (arXiv:2005.14454) and DESIGN.md: phi, Pi on sites,
+// th_i = lattice A_i (link angle of Eq. 12), ep_i = lattice E_i (Eq. 10),
+// U_i = exp(-i th_i).  This file holds no code shared with oracle/.
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace ah {
+
+// Per-step scalars, computed on the host in fp64 (ah_api.cu: make_coef) from
+// PAPER.md:78-80 and Eqs. 7-8, then rounded once to the kernel's real type.
+template <typename real>
+struct StepCoef {
+    real idx2;      // 1/dx^2
+    real c1;        // (1-delta)/(1+delta)            Eq. 7
+    real c2;        // dt/(1+delta)
+    real w1;        // (1-omega)/(1+omega)            Eq. 8
+    real w2;        // dt/(1+omega)
+    real half_lam_q;// lambda0 * a^{2s} / 2           Eq. 7
+    real sig2;      // sigma^2
+    real two_e2_q;  // 2 e0^2 a^{2s}                  Eq. 8
+    real dt;        // Delta eta                      Eqs. 9-10
+    int compact;    // 1: sin(Phi) force; 0: Phi      reading #10
+};
+
+// Diagnostic-step scalars (SURVEY 8(c) diagnostics block).
+struct DiagCoef {
+    double idx2;        // 1/dx^2
+    double q;           // a^{2s} at tau
+    double quarter_lam_q;// lambda0 q / 4
+    double sig2;
+    double inv_2e2q;    // 1/(2 e0^2 q)
+    double two_e2_kappa;// 2 e0^2 kappa, kappa = q (1-delta)/(1-omega)   reading #18
+    int compact;
+};
+
+template <typename real>
+struct Fields {            // 10 SoA arrays, order of ah_b200.h
+    real *f[10];
+};
+template <typename real>
+struct ConstFields {
+    const real *f[10];
+};
+
+enum { PHI_RE = 0, PHI_IM, PI_RE, PI_IM, TH_X, TH_Y, TH_Z, EP_X, EP_Y, EP_Z };
+
+// Number of partial-sum slots a diagnostics block writes.
+enum {
+    DS_NW_XY = 0, DS_NW_XZ, DS_NW_YZ, DS_NEAR, DS_BIG,   // integer counts (stored as double-exact int64)
+    DS_NINT = 5,
+    DF_SPI = 0, DF_SGR, DF_SL, DF_GSQ, DF_DIVSQ, DF_CHSQ, DF_GMAX,
+    DS_NFLT = 7
+};
+
+struct DiagPartial {
+    long long i[DS_NINT];
+    double f[DS_NFLT];
+};
+
+// ----------------------------------------------------------------------------------- trig
+//
+// Link variables need cos/sin of an unbounded angle th (Eq. 10 never wraps it); plaquette
+// forces need sin of a (normally small) angle Phi.  fp32 path: round-to-nearest multiple of
+// pi/2 (resp. pi) by the add-magic-constant trick, two-term Cody-Waite reduction with FMA
+// (pi/2 = C1 + C2 to 48 bits, enough for |x| < 2^15), then odd/even polynomials fitted by
+// csrc/fit_trig_coeffs.py (relative error of the polynomials 7.5e-9 / 2.3e-10 / 1.1e-8, i.e.
+// below half an fp32 ulp).  Measured against fp64 in tests/test_gpu_parity.py::test_trig.
+// Arguments beyond 2^15 take the libm path.  fp64 path: libm.
+
+#define AH_TRIG_LIMIT 32768.0f
+
+__device__ __forceinline__ void sincos_poly_f32(float x, float &s, float &c)
+{
+    const float magic = 12582912.0f;                          // 1.5 * 2^23
+    const float t = fmaf(x, 0.6366197466850281f, magic);      // low mantissa bits = rint(x*2/pi)
+    const float k = t - magic;
+    float r = fmaf(k, -1.5707963705062866f, x);               // C1 = fl32(pi/2)
+    r = fmaf(k, 4.371138828673793e-08f, r);                   // C2 = fl32(pi/2 - C1) (negative)
+    const float r2 = r * r;
+    // sin(r) = r + r^3 P(r^2) on |r| <= pi/4
+    float ps = fmaf(r2, -0.00019482117204461247f, 0.008331847377121449f);
+    ps = fmaf(ps, r2, -0.16666647791862488f);
+    const float sr = fmaf(ps * r2, r, r);
+    // cos(r) = 1 - r^2/2 + r^4 Q(r^2)
+    float pc = fmaf(r2, 2.4440761990263127e-05f, -0.0013887434033676982f);
+    pc = fmaf(pc, r2, 0.04166664928197861f);
+    pc = fmaf(pc, r2, -0.5f);
+    const float cr = fmaf(pc, r2, 1.0f);
+    const unsigned q = __float_as_uint(t);
+    const float s0 = (q & 1u) ? cr : sr;
+    const float c0 = (q & 1u) ? sr : cr;
+    s = __uint_as_float(__float_as_uint(s0) ^ ((q & 2u) << 30));
+    c = __uint_as_float(__float_as_uint(c0) ^ (((q + 1u) & 2u) << 30));
+}
+
+__device__ __forceinline__ float sin_poly_f32(float x)
+{
+    const float magic = 12582912.0f;
+    const float t = fmaf(x, 0.31830987334251404f, magic);     // rint(x/pi)
+    const float k = t - magic;
+    float r = fmaf(k, -3.1415927410125732f, x);               // fl32(pi)
+    r = fmaf(k, 8.742277657347586e-08f, r);                   // fl32(pi - fl32(pi)) (negative)
+    const float r2 = r * r;
+    // sin(r) = r + r^3 P(r^2) on |r| <= pi/2
+    float ps = fmaf(r2, 2.5971810373448534e-06f, -0.00019805048941634595f);
+    ps = fmaf(ps, r2, 0.008332990109920502f);
+    ps = fmaf(ps, r2, -0.16666655242443085f);
+    const float sr = fmaf(ps * r2, r, r);
+    return __uint_as_float(__float_as_uint(sr) ^ (__float_as_uint(t) << 31));   // (-1)^k
+}
+
+__device__ __forceinline__ void link_sincos(float th, float &s, float &c)
+{
+    if (fabsf(th) < AH_TRIG_LIMIT) {
+        sincos_poly_f32(th, s, c);
+    } else {
+        sincosf(th, &s, &c);
+    }
+}
+__device__ __forceinline__ void link_sincos(double th, double &s, double &c) { sincos(th, &s, &c); }
+
+__device__ __forceinline__ float plaq_sin(float x)
+{
+    return fabsf(x) < AH_TRIG_LIMIT ? sin_poly_f32(x) : sinf(x);
+}
+__device__ __forceinline__ double plaq_sin(double x) { return sin(x); }
+
+// ------------------------------------------------------------------------- block reduction
+
+__device__ __forceinline__ double warp_sum(double v)
+{
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+__device__ __forceinline__ long long warp_sum(long long v)
+{
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+__device__ __forceinline__ double warp_max(double v)
+{
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v = fmax(v, __shfl_xor_sync(0xffffffffu, v, o));
+    return v;
+}
+
+}  // namespace ah

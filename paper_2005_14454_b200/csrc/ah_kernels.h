@@ -1,0 +1,37 @@
+// ah_kernels.h — launcher declarations shared by the .cu translation units of libah_b200.so.
+#pragma once
+
+#include "ah_common.cuh"
+
+namespace ah {
+
+// general one-thread-per-site step (ah_site_kernel.cu)
+template <typename real>
+cudaError_t launch_site_step(const ConstFields<real> &in, const Fields<real> &out,
+                             const StepCoef<real> &k, int nx, int ny, int nz, cudaStream_t st);
+
+// I0 (ah_site_kernel.cu)
+template <typename real>
+cudaError_t launch_init(const Fields<real> &out, uint64_t seed, double sigma, size_t n,
+                        cudaStream_t st);
+
+// z-marching tiled fp32 step (ah_tiled_kernel.cu); needs nx % 128 == 0
+bool tiled_supported(int nx, int ny, int nz);
+cudaError_t launch_tiled_step(const ConstFields<float> &in, const Fields<float> &out,
+                              const StepCoef<float> &k, int nx, int ny, int nz, cudaStream_t st);
+cudaError_t tiled_setup();  // one-time function attributes (shared-memory carve-out)
+
+// diagnostics (ah_diag_kernel.cu)
+//   partials: device array of at least diag_num_blocks(...) DiagPartial
+//   result  : device pointer to ONE DiagPartial (the fixed-order total)
+//   w3/near3: optional device int8/uint8 arrays of 3*n (per-plaquette output) or nullptr
+int diag_num_blocks(int nx, int ny, int nz);
+template <typename real>
+cudaError_t launch_diag(const ConstFields<real> &in, const DiagCoef &k, int nx, int ny, int nz,
+                        DiagPartial *partials, DiagPartial *result, int8_t *w3, uint8_t *near3,
+                        cudaStream_t st);
+
+// tests only: evaluate the fp32 trig helpers on device arrays
+cudaError_t launch_test_trig(const float *x, float *s, float *c, float *ps, size_t n, cudaStream_t st);
+
+}  // namespace ah

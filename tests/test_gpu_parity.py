@@ -1,0 +1,368 @@
+"""GPU parity tests (-m gpu): the CUDA path, called through the C ABI, against the fp64 oracle
+element by element on the same seeded inputs.
+
+Tolerances:
+  * fp64 site kernel vs oracle: 1e-12 relative to the field's max (same algebra, rounding order only).
+  * fp32 kernels, ONE step from identical (fp32-representable) inputs: 2e-6 of the field's max
+    (a few fp32 ulps through ~30 operations; 1/dx^2 = 4 amplifies the Laplacian's rounding).
+  * north_star: after 100 steps at 64^3, max|d phi|/max|phi| and max|d ep|/max|ep| <= 1e-4.
+  * winding: per-plaquette integers identical to the oracle's on the downloaded fp32 snapshot
+    promoted to fp64, except plaquettes the oracle flags near-branch.
+  * Sigma-type diagnostics on the same snapshot: 1e-5 relative to the sum of |terms| scale.
+"""
+import numpy as np
+import pytest
+
+from paper_2005_14454_b200 import inputs
+
+pytestmark = pytest.mark.gpu
+
+MODEL_KEYS = ("dx", "lambda0", "e0", "sigma", "s", "p", "tau_ref", "alpha", "compact")
+
+
+@pytest.fixture(scope="module")
+def ah():
+    import torch
+    assert torch.cuda.is_available(), "these tests need a CUDA device"
+    from paper_2005_14454_b200 import build
+    build.build()
+    from paper_2005_14454_b200 import binding
+    return binding
+
+
+def both(ah, oracle, shape, fp64=False, kernel=None, **model):
+    nx, ny, nz = shape
+    Po = oracle.make_params(nx, ny, nz, **model)
+    sim = ah.Simulation(params=ah.make_params(nx, ny, nz, fp64=fp64, **model))
+    if kernel is not None:
+        sim.set_kernel(kernel)
+    return sim, Po
+
+
+def rel_max(a, b):
+    """max |a-b| / max |b| per field group: phi, Pi, th, ep."""
+    out = {}
+    for name, sl in (("phi", slice(0, 2)), ("pi", slice(2, 4)), ("th", slice(4, 7)), ("ep", slice(7, 10))):
+        den = np.abs(b[sl]).max()
+        out[name] = float(np.abs(a[sl].astype(np.float64) - b[sl]).max() / (den if den > 0 else 1.0))
+    return out
+
+
+def kernels_for(ah, nx):
+    ks = [ah.KERNEL_SITE]
+    if nx % 128 == 0:
+        ks.append(ah.KERNEL_TILED)
+    return ks
+
+
+# ------------------------------------------------------------------------------------- trig
+
+def test_trig_against_fp64(ah):
+    import torch
+    rng = np.random.default_rng(5)
+    parts = [rng.uniform(-s, s, 400_000) for s in (1e-3, 0.5, 4.0, 100.0, 3.0e4, 1.0e6)]
+    parts.append(np.array([0.0, -0.0, np.pi, -np.pi, np.pi / 2, 32767.9, 32768.0, -32768.5, 1e-30]))
+    x = np.concatenate(parts).astype(np.float32)
+    s, c, ps = ah.test_trig(torch.from_numpy(x).cuda())
+    s, c, ps = s.cpu().numpy(), c.cpu().numpy(), ps.cpu().numpy()
+    xd = x.astype(np.float64)
+    assert np.abs(s - np.sin(xd)).max() <= 1.5e-7
+    assert np.abs(c - np.cos(xd)).max() <= 1.5e-7
+    assert np.abs(ps - np.sin(xd)).max() <= 2.0e-7
+    small = np.abs(xd) < 1.0
+    rel = np.abs(ps[small] - np.sin(xd[small])) / np.maximum(np.abs(np.sin(xd[small])), 1e-30)
+    assert rel.max() <= 2.0e-7   # plaquette sines keep RELATIVE accuracy for small angles
+
+
+# ------------------------------------------------------------------------------------- I0
+
+@pytest.mark.parametrize("fp64", [False, True])
+def test_init_fields_matches_oracle(ah, oracle, fp64):
+    sim, Po = both(ah, oracle, (20, 12, 7), fp64=fp64, sigma=1.5)
+    sim.init_fields(12345)
+    g = sim.get_fields()
+    o = oracle.init_fields(Po, 12345)
+    tol = 1e-15 if fp64 else 1.2e-7 * 1.5
+    assert np.abs(g[:2] - o[:2]).max() <= tol
+    assert not g[2:].any()
+    assert np.allclose(np.hypot(g[0], g[1]), 1.5, rtol=2e-7)
+    sim.close()
+
+
+# ------------------------------------------------------------------------------- single step
+
+ONE_STEP_CASES = [
+    dict(p=0.0, s=0.0),
+    dict(p=1.0, s=0.0),
+    dict(p=1.0, s=1.0, tau_ref=3.0),
+    dict(p=2.0, s=1.0, tau_ref=3.0),
+    dict(p=1.0, s=0.5, tau_ref=2.0, lambda0=1.3, e0=0.7, sigma=1.2, dx=0.4, alpha=1.5),
+    dict(p=1.0, s=1.0, tau_ref=3.0, compact=0),
+]
+
+
+@pytest.mark.parametrize("case", ONE_STEP_CASES)
+@pytest.mark.parametrize("shape", [(20, 12, 7), (33, 5, 9), (64, 64, 3)])
+def test_one_step_fp64_site_kernel(ah, oracle, case, shape):
+    """fp64 instantiation of the site kernel = the oracle's algebra up to rounding order."""
+    sim, Po = both(ah, oracle, shape, fp64=True, **case)
+    f0 = inputs.random_state(*shape, seed=11)
+    sim.set_fields(f0)
+    sim.step(3, 1.7, 0.1)
+    g = sim.get_fields()
+    o = oracle.step(Po, f0.copy(), 3, 1.7, 0.1)
+    r = rel_max(g, o)
+    assert max(r.values()) <= 1e-12, r
+    sim.close()
+
+
+@pytest.mark.parametrize("case", ONE_STEP_CASES)
+@pytest.mark.parametrize("shape", [(20, 12, 7), (128, 9, 6), (256, 16, 11), (128, 8, 1), (128, 1, 5), (384, 3, 2)])
+def test_one_step_fp32(ah, oracle, case, shape):
+    f0 = inputs.random_state(*shape, seed=7)
+    for kern in kernels_for(ah, shape[0]):
+        sim, Po = both(ah, oracle, shape, kernel=kern, **case)
+        sim.set_fields(f0)
+        sim.step(1, 1.7, 0.1)
+        g = sim.get_fields()
+        o = oracle.step(Po, f0.copy(), 1, 1.7, 0.1)
+        r = rel_max(g, o)
+        assert max(r.values()) <= 2e-6, (kern, r)
+        sim.close()
+
+
+@pytest.mark.parametrize("shape", [(1, 1, 1), (1, 6, 5), (7, 1, 1), (2, 2, 2), (5, 4, 1)])
+def test_degenerate_lattices(ah, oracle, shape):
+    """Extent-1 and extent-2 directions: a site is its own neighbour; the oracle's modulo indexing decides."""
+    f0 = inputs.random_state(*shape, seed=3)
+    for fp64, tol in ((True, 1e-12), (False, 3e-6)):
+        sim, Po = both(ah, oracle, shape, fp64=fp64, p=1.0, s=1.0, tau_ref=2.0)
+        sim.set_fields(f0)
+        sim.step(2, 1.0, 0.1)
+        r = rel_max(sim.get_fields(), oracle.step(Po, f0.copy(), 2, 1.0, 0.1))
+        assert max(r.values()) <= tol, (fp64, r)
+        sim.close()
+
+
+def test_large_link_angles(ah, oracle):
+    """th is never wrapped (Eq. 10): angles of a few hundred radians must still give the right links."""
+    shape = (128, 6, 5)
+    f0 = inputs.random_state(*shape, seed=21, th_amp=150.0)
+    for kern in kernels_for(ah, shape[0]):
+        sim, Po = both(ah, oracle, shape, kernel=kern, p=1.0, s=0.0)
+        sim.set_fields(f0)
+        sim.step(1, 2.0, 0.1)
+        r = rel_max(sim.get_fields(), oracle.step(Po, f0.copy(), 1, 2.0, 0.1))
+        # th itself is ~150 rad: one fp32 ulp of it is 1.5e-5 rad, which enters every plaquette angle
+        assert r["phi"] <= 3e-6 and r["pi"] <= 3e-5 and r["th"] <= 1e-6 and r["ep"] <= 3e-4, (kern, r)
+        sim.close()
+
+
+# ------------------------------------------------------------------------ north_star parity
+
+def test_parity_config1_64cubed_100_and_160_steps(ah, oracle):
+    """BASELINE config 1: 64^3, dx=0.5, dt=0.1, radiation, s=0, random-phase IC from seed 1.
+    north_star: max rel |d phi|, |d ep| <= 1e-4 after 100 steps."""
+    n, dt, tau0 = 64, 0.1, 1.0
+    sim, Po = both(ah, oracle, (n, n, n), p=1.0, s=0.0)
+    f = oracle.init_fields(Po, 1)
+    sim.set_fields(f)                      # identical ICs: cos/sin values rounded once to fp32
+    f = sim.get_fields().astype(np.float64)
+    sim.step(100, tau0, dt)
+    g100 = sim.get_fields()
+    oracle.step(Po, f, 100, tau0, dt)
+    r100 = rel_max(g100, f)
+    print("64^3 100 steps rel err:", r100)
+    assert r100["phi"] <= 1e-4 and r100["ep"] <= 1e-4, r100
+    assert r100["pi"] <= 1e-4 and r100["th"] <= 1e-4, r100
+    sim.step(60, tau0 + 100 * dt, dt)
+    oracle.step(Po, f, 60, tau0 + 100 * dt, dt)
+    r160 = rel_max(sim.get_fields(), f)
+    print("64^3 160 steps rel err:", r160)
+    assert max(r160.values()) <= 1e-3, r160
+    sim.close()
+
+
+def test_parity_tiled_128cubed_physical_width(ah, oracle):
+    """Config-2-like (radiation, s=1, tau_ref = end time) at 128^3 for 40 steps, tiled kernel vs oracle,
+    and tiled vs site kernel."""
+    n, dt, tau0, steps = 128, 0.1, 1.0, 40
+    model = dict(p=1.0, s=1.0, tau_ref=tau0 + 640 * dt)
+    sim, Po = both(ah, oracle, (n, n, n), **model)
+    f = oracle.init_fields(Po, 2)
+    sim.set_fields(f)
+    f = sim.get_fields().astype(np.float64)
+    sim.step(steps, tau0, dt)
+    g = sim.get_fields()
+    oracle.step(Po, f, steps, tau0, dt)
+    r = rel_max(g, f)
+    print("128^3 40 steps rel err:", r)
+    assert max(r.values()) <= 2e-5, r
+    sim.close()
+
+
+# ------------------------------------------------------------------------------ diagnostics
+
+def _evolved_snapshot(ah, oracle, n, steps, seed, **model):
+    sim, Po = both(ah, oracle, (n, n, n), **model)
+    sim.init_fields(seed)
+    sim.step(steps, 1.0, 0.1)
+    return sim, Po, 1.0 + steps * 0.1
+
+
+@pytest.mark.parametrize("model", [dict(p=1.0, s=0.0), dict(p=2.0, s=1.0, tau_ref=9.0)])
+def test_winding_bit_exact_on_snapshot(ah, oracle, model):
+    sim, Po, tau = _evolved_snapshot(ah, oracle, 48, 60, 4, **model)
+    snap = sim.get_fields().astype(np.float64)
+    w_gpu, near_gpu = sim.winding_field()
+    w_or, near_or = oracle.winding(Po, snap)
+    differ = w_gpu != w_or
+    assert np.abs(w_or).sum() > 50, "vacuous without strings"
+    assert not (differ & (near_or == 0)).any(), "winding differs on a plaquette that is not near-branch"
+    d_gpu = sim.diagnostics(tau, 0.1)
+    d_or = oracle.diagnostics(Po, snap, tau, 0.1)
+    for key in ("n_wind", "n_wind_xy", "n_wind_xz", "n_wind_yz"):
+        assert abs(d_gpu[key] - d_or[key]) <= d_or["n_near_branch"], key
+    assert d_gpu["n_wind"] == int(np.abs(w_gpu).sum())
+    assert d_gpu["n_big_plaq"] == d_or["n_big_plaq"] == 0
+    assert abs(d_gpu["n_near_branch"] - d_or["n_near_branch"]) <= 2
+    assert d_gpu["xi_w"] == pytest.approx(np.sqrt(48**3 * 0.5**3 / (0.5 * d_gpu["n_wind"])), rel=1e-14)
+    sim.close()
+
+
+def test_winding_random_phase_snapshot(ah, oracle):
+    """Uncorrelated random phases: a third of all plaquettes wind (oracle pin (v)); bit-exact vs oracle."""
+    sim, Po = both(ah, oracle, (40, 24, 10), p=0.0)
+    sim.init_fields(9)
+    snap = sim.get_fields().astype(np.float64)
+    w_gpu, _ = sim.winding_field()
+    w_or, near_or = oracle.winding(Po, snap)
+    assert not ((w_gpu != w_or) & (near_or == 0)).any()
+    assert abs(np.abs(w_gpu).mean() - 1 / 3) < 0.02
+    sim.close()
+
+
+@pytest.mark.parametrize("model", [dict(p=1.0, s=0.0), dict(p=1.0, s=1.0, tau_ref=9.0),
+                                   dict(p=2.0, s=1.0, tau_ref=9.0), dict(p=1.0, s=1.0, tau_ref=9.0, compact=0)])
+def test_sigma_diagnostics_on_snapshot(ah, oracle, model):
+    sim, Po, tau = _evolved_snapshot(ah, oracle, 40, 50, 6, **model)
+    snap = sim.get_fields().astype(np.float64)
+    d_gpu = sim.diagnostics(tau, 0.1)
+    d_or = oracle.diagnostics(Po, snap, tau, 0.1)
+    for key in ("sum_pi2_L", "sum_grad2_L", "sum_L"):
+        assert d_gpu[key] == pytest.approx(d_or[key], rel=1e-5), (key, d_gpu[key], d_or[key])
+    assert d_gpu["v2_phi"] == pytest.approx(d_or["v2_phi"], abs=1e-5)
+    # Gauss: evaluated in fp64 from the same stored values on both sides
+    for key in ("gauss_max", "gauss_l2", "gauss_div_l2", "gauss_charge_l2"):
+        assert d_gpu[key] == pytest.approx(d_or[key], rel=1e-9), (key, d_gpu[key], d_or[key])
+    assert d_gpu["gauss_rel"] == pytest.approx(d_or["gauss_rel"], rel=1e-8)
+    sim.close()
+
+
+def test_gauss_residual_is_fp32_roundoff(ah):
+    """the scheme keeps Gauss's law; in fp32 the residual is fp32 round-off (reported)."""
+    sim = ah.Simulation(nx=64, p=1.0, s=0.0)
+    sim.init_fields(1)
+    sim.step(100, 1.0, 0.1)
+    d = sim.diagnostics(11.0, 0.1)
+    print("gauss_rel after 100 fp32 steps:", d["gauss_rel"])
+    assert d["gauss_div_l2"] > 1.0
+    assert d["gauss_rel"] < 2e-5
+    sim.close()
+
+
+def test_gauss_residual_fp64_kernel_roundoff(ah):
+    sim = ah.Simulation(nx=24, p=1.0, s=1.0, tau_ref=5.0, fp64=True)
+    sim.init_fields(1)
+    sim.step(40, 1.0, 0.1)
+    d = sim.diagnostics(5.0, 0.1)
+    assert d["gauss_rel"] < 1e-12
+    sim.close()
+
+
+def test_step_diag_equals_diagnostics_before_step(ah):
+    """D-fuse contract: the record for step j is ah_diagnostics(tau_j) of the ENTRY snapshot."""
+    a = ah.Simulation(nx=32, p=1.0, s=1.0, tau_ref=4.0)
+    b = ah.Simulation(nx=32, p=1.0, s=1.0, tau_ref=4.0)
+    a.init_fields(5)
+    b.init_fields(5)
+    recs = a.step_diag(25, 1.0, 0.1, 10)
+    assert [r["tau"] for r in recs] == pytest.approx([1.0, 2.0, 3.0])
+    for r in recs:
+        nsteps = int(round((r["tau"] - 1.0) / 0.1))
+        b.init_fields(5)
+        b.step(nsteps, 1.0, 0.1)
+        d = b.diagnostics(1.0 + nsteps * 0.1, 0.1)
+        for key, val in d.items():
+            assert r[key] == val or (np.isnan(val) and np.isnan(r[key])), key
+    b.init_fields(5)
+    b.step(25, 1.0, 0.1)
+    assert np.array_equal(a.get_fields(), b.get_fields())
+    a.close()
+    b.close()
+
+
+def test_diagnostics_deterministic(ah):
+    sim = ah.Simulation(nx=48, p=1.0, s=0.0)
+    sim.init_fields(8)
+    sim.step(30, 1.0, 0.1)
+    d1 = sim.diagnostics(4.0, 0.1)
+    d2 = sim.diagnostics(4.0, 0.1)
+    assert d1 == d2
+    sim.close()
+
+
+# ---------------------------------------------------------------------------- ABI behaviour
+
+def test_error_codes_on_device(ah):
+    sim = ah.Simulation(nx=16)
+    with pytest.raises(ah.AhError) as ei:
+        sim.step(1, 1.0, 0.1)                      # no fields yet
+    assert ei.value.code == ah.AH_ESTATE
+    sim.init_fields(1)
+    for args in ((-1, 1.0, 0.1), (1, 0.0, 0.1), (1, 1.0, 0.0), (1, 1.0, float("nan"))):
+        with pytest.raises(ah.AhError) as ei:
+            sim.step(*args)
+        assert ei.value.code == ah.AH_EINVAL
+    before = sim.get_fields()
+    sim.step(0, 1.0, 0.1)                          # n = 0 is a no-op
+    assert np.array_equal(before, sim.get_fields())
+    import ctypes as C
+    recs = (ah.Diag * 1)()
+    nw = C.c_int(7)
+    rc = ah.lib().ah_step_diag(sim._ctx, 30, 1.0, 0.1, 10, recs, 1, C.byref(nw))   # cap too small
+    assert rc == ah.AH_EINVAL and nw.value == 0
+    assert np.array_equal(before, sim.get_fields())   # ... and it did not step
+    with pytest.raises(ah.AhError):
+        sim.set_kernel(ah.KERNEL_TILED)            # nx = 16 is not a multiple of 128
+    sim.close()
+
+
+def test_ping_pong_parity_and_current_bufs(ah):
+    sim = ah.Simulation(nx=16)
+    sim.init_fields(3)
+    first = [b.data_ptr() for b in sim.current_bufs()]
+    sim.step(1, 1.0, 0.1)
+    second = [b.data_ptr() for b in sim.current_bufs()]
+    assert set(first).isdisjoint(second)
+    sim.step(1, 1.1, 0.1)
+    assert [b.data_ptr() for b in sim.current_bufs()] == first
+    cur = sim.current_bufs()
+    got = sim.get_fields()
+    assert np.array_equal(got[0].ravel(), cur[0].cpu().numpy())
+    assert sim.launch_count() == 3
+    sim.close()
+
+
+def test_step_n_equals_n_single_steps(ah):
+    """tau_j = tau + j*dt as a product: one call of n steps == n calls at those times."""
+    a = ah.Simulation(nx=24, p=1.0, s=1.0, tau_ref=3.0)
+    b = ah.Simulation(nx=24, p=1.0, s=1.0, tau_ref=3.0)
+    a.init_fields(2)
+    b.init_fields(2)
+    a.step(7, 1.3, 0.1)
+    for j in range(7):
+        b.step(1, 1.3 + j * 0.1, 0.1)
+    assert np.array_equal(a.get_fields(), b.get_fields())
+    a.close()
+    b.close()
