@@ -216,6 +216,7 @@ def run_ours(args):
     sim = binding.Simulation(params=binding.make_params(n, **params), device=f"cuda:{local}")
     if args.kernel != "auto":
         sim.set_kernel({"site": binding.KERNEL_SITE, "tiled": binding.KERNEL_TILED}[args.kernel])
+    kernel_used = {binding.KERNEL_SITE: "site_step_kernel", binding.KERNEL_TILED: "tiled_step_kernel"}[sim.get_kernel()]
     sites = float(n) ** 3
     stream = sim.stream
 
@@ -282,7 +283,7 @@ def run_ours(args):
 
     if rank == 0:
         peak, peak_src = measured_peak()
-        kernel_name = "tiled_step_kernel" if binding.lib() and args.kernel != "site" and n % 128 == 0 else "site_step_kernel"
+        kernel_name = kernel_used
         step_launches = K
         avg_launch_ms = ms / step_launches            # one step-kernel launch per step
         achieved = BYTES_PER_SITE * sites / (avg_launch_ms * 1e-3) / 1e9

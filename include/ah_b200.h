@@ -132,6 +132,10 @@ int ah_winding_field(ah_ctx *ctx, int8_t *host_w3, uint8_t *host_near3);
 /* Choose the step kernel (AH_KERNEL_*).  AH_EINVAL if the lattice does not allow it. */
 int ah_set_kernel(ah_ctx *ctx, int kernel);
 
+/* The step kernel the context currently launches: AH_KERNEL_SITE or AH_KERNEL_TILED (never AUTO);
+ * AH_EINVAL for a null context. */
+int ah_get_kernel(const ah_ctx *ctx);
+
 /* Number of kernel launches this context has enqueued since creation (bench.py's gpu_launches). */
 int64_t ah_launch_count(const ah_ctx *ctx);
 

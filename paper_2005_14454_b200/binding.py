@@ -29,7 +29,7 @@ FIELD_NAMES = ("phi_re", "phi_im", "pi_re", "pi_im", "th_x", "th_y", "th_z", "ep
 # every symbol include/ah_b200.h declares (checked by tests/test_abi.py)
 EXPORTS = (
     "ah_create", "ah_destroy", "ah_init_fields", "ah_set_fields", "ah_get_fields", "ah_current_bufs",
-    "ah_step", "ah_diagnostics", "ah_step_diag", "ah_winding_field", "ah_set_kernel",
+    "ah_step", "ah_diagnostics", "ah_step_diag", "ah_winding_field", "ah_set_kernel", "ah_get_kernel",
     "ah_launch_count", "ah_coeffs", "ah_test_trig", "ah_last_error", "ah_version",
 )
 
@@ -93,6 +93,7 @@ def lib():
     L.ah_step_diag.argtypes = [vp, ip, dp, dp, ip, C.POINTER(Diag), ip, C.POINTER(ip)]
     L.ah_winding_field.argtypes = [vp, vp, vp]
     L.ah_set_kernel.argtypes = [vp, ip]
+    L.ah_get_kernel.argtypes = [vp]
     L.ah_launch_count.argtypes = [vp]
     L.ah_launch_count.restype = C.c_int64
     L.ah_coeffs.argtypes = [C.POINTER(Params), dp, dp] + [C.POINTER(dp)] * 4
@@ -235,6 +236,12 @@ class Simulation:
 
     def set_kernel(self, kernel: int):
         _check(lib().ah_set_kernel(self._ctx, int(kernel)))
+
+    def get_kernel(self) -> int:
+        k = lib().ah_get_kernel(self._ctx)
+        if k < 0:
+            _check(k)
+        return int(k)
 
     def launch_count(self) -> int:
         return int(lib().ah_launch_count(self._ctx))

@@ -317,6 +317,12 @@ int ah_set_kernel(ah_ctx *c, int kernel)
     return AH_OK;
 }
 
+int ah_get_kernel(const ah_ctx *c)
+{
+    if (!c) return fail(AH_EINVAL, "ah_get_kernel: null context");
+    return c->P.fp64 ? AH_KERNEL_SITE : c->kernel;
+}
+
 int64_t ah_launch_count(const ah_ctx *c) { return c ? c->launches : 0; }
 
 int ah_init_fields(ah_ctx *c, uint64_t seed)
