@@ -113,19 +113,22 @@ __device__ __forceinline__ float sin_poly_f32(float x)
     return __uint_as_float(__float_as_uint(sr) ^ (__float_as_uint(t) << 31));   // (-1)^k
 }
 
+// libm slow paths kept out of line: the hot loops stay small enough for the 32 KB instruction cache
+static __device__ __noinline__ void sincos_slow_f32(float th, float *s, float *c) { sincosf(th, s, c); }
+static __device__ __noinline__ float sin_slow_f32(float x) { return sinf(x); }
+
 __device__ __forceinline__ void link_sincos(float th, float &s, float &c)
 {
-    if (fabsf(th) < AH_TRIG_LIMIT) {
-        sincos_poly_f32(th, s, c);
-    } else {
-        sincosf(th, &s, &c);
-    }
+    sincos_poly_f32(th, s, c);
+    if (!(fabsf(th) < AH_TRIG_LIMIT)) sincos_slow_f32(th, &s, &c);
 }
 __device__ __forceinline__ void link_sincos(double th, double &s, double &c) { sincos(th, &s, &c); }
 
 __device__ __forceinline__ float plaq_sin(float x)
 {
-    return fabsf(x) < AH_TRIG_LIMIT ? sin_poly_f32(x) : sinf(x);
+    float r = sin_poly_f32(x);
+    if (!(fabsf(x) < AH_TRIG_LIMIT)) r = sin_slow_f32(x);
+    return r;
 }
 __device__ __forceinline__ double plaq_sin(double x) { return sin(x); }
 
