@@ -97,6 +97,8 @@ struct ah_ctx {
     ah::DiagPartial *d_results;
     ah::DiagPartial *h_results;  // pinned
     int cap_results;
+    int *d_overflow;   // two flags (step parity): tiled kernel met a link angle outside its domain
+    int step_parity;
 };
 
 namespace {
@@ -140,8 +142,16 @@ int one_step(ah_ctx *c, double tau, double dt)
         e = ah::launch_site_step<double>(cur_fields<double>(c), next_fields<double>(c),
                                          make_coef<double>(P, tau, dt), P.nx, P.ny, P.nz, c->st);
     } else if (c->kernel == AH_KERNEL_TILED) {
-        e = ah::launch_tiled_step(cur_fields<float>(c), next_fields<float>(c),
-                                  make_coef<float>(P, tau, dt), P.nx, P.ny, P.nz, c->st);
+        // fast path, then a conditional redo with the libm-based site kernel (runs only if the fast
+        // path flagged a link angle beyond its polynomial range; two flags alternate between steps)
+        const ah::StepCoef<float> k = make_coef<float>(P, tau, dt);
+        int *flag = c->d_overflow + c->step_parity, *next_flag = c->d_overflow + (1 - c->step_parity);
+        e = ah::launch_tiled_step(cur_fields<float>(c), next_fields<float>(c), k, P.nx, P.ny, P.nz, flag, c->st);
+        if (e == cudaSuccess)
+            e = ah::launch_site_redo(flag, next_flag, cur_fields<float>(c), next_fields<float>(c), k, P.nx, P.ny,
+                                     P.nz, c->st);
+        c->step_parity = 1 - c->step_parity;
+        c->launches += 1;
     } else {
         e = ah::launch_site_step<float>(cur_fields<float>(c), next_fields<float>(c),
                                         make_coef<float>(P, tau, dt), P.nx, P.ny, P.nz, c->st);
@@ -288,6 +298,14 @@ int ah_create(ah_ctx **out, const ah_params *P, void *const dev_bufs[], int nbuf
         ah_destroy(c);
         return rc;
     }
+    {
+        cudaError_t e = cudaMalloc(&c->d_overflow, 2 * sizeof(int));
+        if (e == cudaSuccess) e = cudaMemsetAsync(c->d_overflow, 0, 2 * sizeof(int), c->st);
+        if (e != cudaSuccess) {
+            ah_destroy(c);
+            return cuda_fail(e, "overflow flags");
+        }
+    }
     *out = c;
     return AH_OK;
 }
@@ -298,6 +316,7 @@ int ah_destroy(ah_ctx *c)
     if (c->d_partials) cudaFree(c->d_partials);
     if (c->d_results) cudaFree(c->d_results);
     if (c->h_results) cudaFreeHost(c->h_results);
+    if (c->d_overflow) cudaFree(c->d_overflow);
     delete c;
     return AH_OK;
 }

@@ -17,8 +17,13 @@ cudaError_t launch_init(const Fields<real> &out, uint64_t seed, double sigma, si
 
 // z-marching tiled fp32 step (ah_tiled_kernel.cu); needs nx % 128 == 0
 bool tiled_supported(int nx, int ny, int nz);
+//   overflow: device int, set to 1 when a link angle is outside the kernel's domain (|th| >= 2^16 rad);
+//             the outputs of that step must then be recomputed with the site kernel
 cudaError_t launch_tiled_step(const ConstFields<float> &in, const Fields<float> &out,
-                              const StepCoef<float> &k, int nx, int ny, int nz, cudaStream_t st);
+                              const StepCoef<float> &k, int nx, int ny, int nz, int *overflow, cudaStream_t st);
+// after a tiled step: redo it with the site kernel iff *flag != 0; clears *clear (the next step's flag)
+cudaError_t launch_site_redo(const int *flag, int *clear, const ConstFields<float> &in, const Fields<float> &out,
+                             const StepCoef<float> &k, int nx, int ny, int nz, cudaStream_t st);
 cudaError_t tiled_setup();  // one-time function attributes (shared-memory carve-out)
 
 // diagnostics (ah_diag_kernel.cu)

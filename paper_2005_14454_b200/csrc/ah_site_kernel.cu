@@ -8,15 +8,11 @@
 
 namespace ah {
 
+// Eqs. 7-10 at the single site (x, y, z)
 template <typename real>
-__global__ void __launch_bounds__(256)
-site_step_kernel(ConstFields<real> in, Fields<real> out, StepCoef<real> k, int nx, int ny, int nz)
+__device__ __forceinline__ void site_update(const ConstFields<real> &in, const Fields<real> &out,
+                                            const StepCoef<real> &k, int nx, int ny, int nz, int x, int y, int z)
 {
-    const int x = blockIdx.x * blockDim.x + threadIdx.x;
-    const int y = blockIdx.y * blockDim.y + threadIdx.y;
-    const int z = blockIdx.z;
-    if (x >= nx || y >= ny) return;
-
     const int xp = (x + 1 == nx) ? 0 : x + 1, xm = (x == 0) ? nx - 1 : x - 1;
     const int yp = (y + 1 == ny) ? 0 : y + 1, ym = (y == 0) ? ny - 1 : y - 1;
     const int zp = (z + 1 == nz) ? 0 : z + 1, zm = (z == 0) ? nz - 1 : z - 1;
@@ -106,6 +102,40 @@ site_step_kernel(ConstFields<real> in, Fields<real> out, StepCoef<real> k, int n
     out.f[TH_X][c] = tx + k.dt * ex_new;
     out.f[TH_Y][c] = ty + k.dt * ey_new;
     out.f[TH_Z][c] = tz + k.dt * ez_new;
+}
+
+template <typename real>
+__global__ void __launch_bounds__(256)
+site_step_kernel(ConstFields<real> in, Fields<real> out, StepCoef<real> k, int nx, int ny, int nz)
+{
+    const int x = blockIdx.x * blockDim.x + threadIdx.x;
+    const int y = blockIdx.y * blockDim.y + threadIdx.y;
+    const int z = blockIdx.z;
+    if (x >= nx || y >= ny) return;
+    site_update<real>(in, out, k, nx, ny, nz, x, y, z);
+}
+
+// Conditional redo of one step (fixed small grid, grid-stride over sites): does nothing unless the tiled
+// kernel raised *flag (a link angle outside its domain); then every site is recomputed with the libm
+// paths above.  Thread 0 also clears the flag the NEXT step will use.
+__global__ void __launch_bounds__(256)
+site_redo_kernel(const int *flag, int *clear, ConstFields<float> in, Fields<float> out, StepCoef<float> k,
+                 int nx, int ny, int nz)
+{
+    if (blockIdx.x == 0 && threadIdx.x == 0) *clear = 0;
+    if (*flag == 0) return;
+    const size_t n = (size_t)nx * ny * nz;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
+        const int x = (int)(i % nx), y = (int)((i / nx) % ny), z = (int)(i / ((size_t)nx * ny));
+        site_update<float>(in, out, k, nx, ny, nz, x, y, z);
+    }
+}
+
+cudaError_t launch_site_redo(const int *flag, int *clear, const ConstFields<float> &in, const Fields<float> &out,
+                             const StepCoef<float> &k, int nx, int ny, int nz, cudaStream_t st)
+{
+    site_redo_kernel<<<148 * 4, 256, 0, st>>>(flag, clear, in, out, k, nx, ny, nz);
+    return cudaGetLastError();
 }
 
 template <typename real>

@@ -4,25 +4,33 @@
 // once and written once (80 B per site).  DESIGN.md "Kernels / tiled step" has the derivation.
 //
 // Decomposition
-//   * a thread owns 4 consecutive x sites (128-bit coalesced SoA loads / stores), a warp one 128-site
-//     row segment, a CTA a tile of 128 x TY sites; the CTA marches through a chunk of z planes;
+//   * a thread owns 4 consecutive x sites (128-bit accesses), a warp one 128-site row segment, a CTA a
+//     tile of 128 x TY sites; the CTA marches through a chunk of z planes;
+//   * the OLD phi, th planes (the only fields with a stencil) are staged in shared memory with their
+//     halo rows y0-1, y0+TY and halo columns x0-4..x0-1, x0+128..x0+131 by 1-D bulk TMA copies
+//     (cp.async.bulk, one per field row) into a 3-slot ring: plane z (own), z+1 (forward) in use, plane
+//     z+2 in flight for one whole iteration.  Completion is signalled on one mbarrier per slot.  The
+//     periodic wrap is applied to the row / plane source addresses by the producer; tiles that touch
+//     the x boundary copy their two 16-byte halo columns separately;
+//   * Pi, ep (read only at their own site) go global -> registers, and all ten outputs registers -> global;
 //   * every link's U_i = exp(-i th_i) (Eq. 12) is evaluated ONCE (3 sincos per site) and every
 //     plaquette sine (Eqs. 14-15) ONCE (3 per site); each is then handed to the other sites that use it:
 //       x-1 neighbour : inside the thread, or warp shuffle from the lane to the left;
 //       y-1 neighbour : through shared memory (double buffered, ONE __syncthreads per plane);
 //       z-1 neighbour : carried in registers from the previous plane of the march;
-//   * the raw old values at x+1, y+1, z+1 are plain global loads (the z+1 plane becomes the next
-//     iteration's own plane and stays in registers; the y+1 row is an L1/L2 hit);
-//   * one extra "helper" warp per CTA evaluates the shared quantities of the halo row y0-1 and, one
-//     plane ahead, of the halo column x0-1, so the main warps never branch on tile edges.
-//   Periodic wrap is applied to the row / plane / edge-column base offsets only (nx % 128 == 0).
+//   * warp TY (the "helper") is the TMA producer and evaluates the shared quantities of the halo row
+//     y0-1 and of the halo column x0-1, so the main warps never branch on tile edges.
 #include "ah_kernels.h"
 
 namespace ah {
 
 namespace {
 
-constexpr int TILE_X = 128;   // sites per warp row segment (32 lanes x 4)
+constexpr int TILE_X = 128;            // sites per warp row segment (32 lanes x 4)
+constexpr int HALO = 4;                // staged halo columns on each side (16 bytes)
+constexpr int ROWF = TILE_X + 2 * HALO;   // floats per staged row
+constexpr int NST = 3;                 // ring slots
+constexpr int NRAW = 5;                // staged fields: phi_re, phi_im, th_x, th_y, th_z
 constexpr unsigned FULL = 0xffffffffu;
 
 struct V4 {
@@ -36,153 +44,253 @@ __device__ __forceinline__ V4 ld4(const float *__restrict__ p)
     r.v[0] = t.x; r.v[1] = t.y; r.v[2] = t.z; r.v[3] = t.w;
     return r;
 }
+__device__ __forceinline__ V4 lds4(const float *p)
+{
+    const float4 t = *reinterpret_cast<const float4 *>(p);
+    V4 r;
+    r.v[0] = t.x; r.v[1] = t.y; r.v[2] = t.z; r.v[3] = t.w;
+    return r;
+}
 __device__ __forceinline__ void st4(float *__restrict__ p, const V4 &a)
 {
     *reinterpret_cast<float4 *>(p) = make_float4(a.v[0], a.v[1], a.v[2], a.v[3]);
 }
 __device__ __forceinline__ float4 f4(const V4 &a) { return make_float4(a.v[0], a.v[1], a.v[2], a.v[3]); }
 
-// value of the site to the right of this thread's 4th site: lane+1's first site, or (lane 31) the
-// first site of the next row segment, loaded from `edge`
-__device__ __forceinline__ float right_of(const V4 &a, const float *__restrict__ edge, int lane)
+// ---- mbarrier / bulk-copy primitives (PTX; SASS: SYNCS.*, UBLKCP)
+__device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(unsigned long long *bar, unsigned count)
 {
-    float r = __shfl_down_sync(FULL, a.v[0], 1);
-    if (lane == 31) r = __ldg(edge);
-    return r;
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(unsigned long long *bar, unsigned bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes)
+                 : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long *bar, unsigned parity)
+{
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_%=:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra DONE_%=;\n"
+        "bra WAIT_%=;\n"
+        "DONE_%=:\n"
+        "}\n" ::"r"(smem_u32(bar)), "r"(parity)
+        : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(float *dst, const float *src, unsigned bytes, unsigned long long *bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+                     smem_u32(dst)),
+                 "l"(src), "r"(bytes), "r"(smem_u32(bar))
+                 : "memory");
 }
 
 template <bool COMPACT>
 __device__ __forceinline__ float plaq_f(float phi)
 {
-    return COMPACT ? plaq_sin(phi) : phi;   // reading #10
+    return COMPACT ? sin_poly_f32(phi) : phi;   // reading #10; range check by the caller
 }
+
+template <int TY>
+struct Smem {
+    float raw[NST][NRAW][TY + 2][ROWF];   // staged planes; row r <-> y0 - 1 + r, column c <-> x0 - HALO + c
+    float qe[TY][NRAW][TILE_X];           // staged old Pi, ep of the own rows (one plane): pi_re, pi_im, ep_x, ep_y, ep_z
+    float4 row[2][TY][4][32];             // y hand-over: (b_y.re, b_y.im, S_xy, S_yz); row 0 = halo row y0-1, row w+1 from warp w
+    float4 col[2][TY];                    // x hand-over of the site x0-1: (b_x.re, b_x.im, S_xy, S_xz)
+    unsigned long long full[NST];         // a staged phi, th plane has landed
+    unsigned long long qfull[TY];         // a warp's Pi, ep row has landed
+};
 
 }  // namespace
 
 namespace {
+
+// Domain of this kernel: every |th_i| < AH_TILED_TH_LIMIT (2^16 rad), so that every plaquette angle is below
+// 2^18, where the two-term Cody-Waite reductions of sincos_poly_f32 / sin_poly_f32 still hold their 1e-7
+// absolute accuracy (ah_common.cuh).  Each thread checks the 12 link angles it owns (every link of the
+// input state is owned by exactly one thread) and raises *overflow if one is outside; the API then
+// redoes the step with the libm-based site kernel (ah_api.cu: one_step).
+#define AH_TILED_TH_LIMIT 65536.0f
 
 // Shared quantities a site hands to its +x / +y / +z neighbours (all from OLD fields):
 //   b_i  = conj(U_i(s)) phi(s)      the backward hop of Eq. 13 as seen from s+i
 //   S_ij = sin Phi_ij(s)            Eqs. 14-15 (or Phi_ij itself when !COMPACT)
 template <int TY, bool COMPACT>
 __global__ void __launch_bounds__((TY + 1) * 32, ((TY + 1) * 32 <= 256) ? 2 : 1)
-tiled_step_kernel(ConstFields<float> in, Fields<float> out, StepCoef<float> k, int nx, int ny, int nz, int zc)
+tiled_step_kernel(ConstFields<float> in, Fields<float> out, StepCoef<float> k, int nx, int ny, int nz, int zc,
+                  int *overflow)
 {
-    // [plane parity][row: 0 = halo row y0-1, r+1 = tile row r][b_y.re, b_y.im, S_xy, S_yz][lane] (4 x-sites each)
-    __shared__ float4 s_row[2][TY + 1][4][32];
-    // [plane parity][tile row]: (b_x.re, b_x.im, S_xy, S_xz) of the site x0-1 left of the row segment
-    __shared__ float4 s_col[2][TY];
+    extern __shared__ __align__(128) unsigned char smem_bytes[];
+    Smem<TY> &sm = *reinterpret_cast<Smem<TY> *>(smem_bytes);
 
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     const int x0 = blockIdx.x * TILE_X, y0 = blockIdx.y * TY, z0 = blockIdx.z * zc;
     const int z1 = min(nz, z0 + zc);
+    const int nplanes = z1 - z0;           // planes this CTA updates; loads n = 0 .. nplanes + 1
     const size_t sxy = (size_t)nx * ny;
-    const int xe = (x0 + TILE_X == nx) ? 0 : x0 + TILE_X;   // x right of the segment (periodic)
-    const int xw = (x0 == 0) ? nx - 1 : x0 - 1;             // x left of the segment
+    const bool is_main = w < TY;
 
-    const float *__restrict__ PR = in.f[PHI_RE], *__restrict__ PI = in.f[PHI_IM];
-    const float *__restrict__ TX = in.f[TH_X], *__restrict__ TY_ = in.f[TH_Y], *__restrict__ TZ = in.f[TH_Z];
+    // ------------------------------------------------------------------ producers
+    // load n  <->  plane z0 - 1 + n (periodic), slot n % NST.  Every main warp copies its own staged row
+    // (lanes 0..4: one field each), the helper warp the two halo rows 0 and TY+1 (lanes 0..9) and arms
+    // the slot's mbarrier with the byte count of the whole plane.
+    const bool interior = (x0 > 0) && (x0 + TILE_X < nx);
+    const int p_row = is_main ? w + 1 : (lane < NRAW ? 0 : TY + 1);        // staged row this lane copies
+    const int p_fld = is_main ? lane : (lane < NRAW ? lane : lane - NRAW);   // staged field this lane copies
+    const bool p_act = is_main ? lane < NRAW : lane < 2 * NRAW;
+    size_t p_rowoff;                                                        // y * nx of that row (periodic)
+    {
+        int yy = (y0 - 1 + p_row) % ny;
+        if (yy < 0) yy += ny;
+        p_rowoff = (size_t)yy * nx;
+    }
+    const float *p_base = in.f[PHI_RE];
+    if (p_fld == 1) p_base = in.f[PHI_IM];
+    if (p_fld == 2) p_base = in.f[TH_X];
+    if (p_fld == 3) p_base = in.f[TH_Y];
+    if (p_fld == 4) p_base = in.f[TH_Z];
+    auto produce = [&](int n) {
+        const int slot = n % NST;
+        if (!is_main && lane == 0) mbar_expect_tx(&sm.full[slot], (unsigned)(NRAW * (TY + 2) * ROWF * sizeof(float)));
+        if (p_act) {
+            int zp = (z0 - 1 + n) % nz;
+            if (zp < 0) zp += nz;
+            const float *srow = p_base + (size_t)zp * sxy + p_rowoff;
+            float *dst = &sm.raw[slot][p_fld][p_row][0];
+            if (interior) {
+                bulk_g2s(dst, srow + x0 - HALO, ROWF * sizeof(float), &sm.full[slot]);
+            } else {
+                const int xl = (x0 == 0) ? nx - HALO : x0 - HALO;
+                const int xr = (x0 + TILE_X == nx) ? 0 : x0 + TILE_X;
+                bulk_g2s(dst + HALO, srow + x0, TILE_X * sizeof(float), &sm.full[slot]);
+                bulk_g2s(dst, srow + xl, HALO * sizeof(float), &sm.full[slot]);
+                bulk_g2s(dst + HALO + TILE_X, srow + xr, HALO * sizeof(float), &sm.full[slot]);
+            }
+        }
+    };
+
+    // Pi, ep of the warp's own row of plane z0 + n - 1 -> sm.qe[w] (lanes 0..4: one field each)
+    const float *q_base = in.f[PI_RE];
+    if (lane == 1) q_base = in.f[PI_IM];
+    if (lane == 2) q_base = in.f[EP_X];
+    if (lane == 3) q_base = in.f[EP_Y];
+    if (lane == 4) q_base = in.f[EP_Z];
+    auto produce_q = [&](int n, size_t row_off) {
+        if (lane == 0) mbar_expect_tx(&sm.qfull[w], (unsigned)(NRAW * TILE_X * sizeof(float)));
+        __syncwarp();
+        if (lane < NRAW)
+            bulk_g2s(&sm.qe[w][lane][0], q_base + (size_t)(z0 + n - 1) * sxy + row_off, TILE_X * sizeof(float),
+                     &sm.qfull[w]);
+    };
+
+    if (threadIdx.x == 0) {
+#pragma unroll
+        for (int s = 0; s < NST; ++s) mbar_init(&sm.full[s], 1);
+#pragma unroll
+        for (int s = 0; s < TY; ++s) mbar_init(&sm.qfull[s], 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    }
+    __syncthreads();
+    produce(0);
+    produce(1);
+    produce(2);
+    if (is_main && y0 + w < ny) produce_q(1, (size_t)(y0 + w) * nx + x0);
 
     const float kA = k.c2 * k.idx2;    // weight of one hop in Pi+          (Eq. 7)
     const float kB = k.w2 * k.idx2;    // weight of one plaquette sine in ep+ (Eq. 8)
     const float kJ = k.w2 * k.two_e2_q;
 
-    const bool is_main = w < TY;
-    // ---- main-warp geometry: row y0+w, sites x0+4*lane .. +3
+    // ---- main-warp geometry: row y0+w (staged row w+1), sites x0+4*lane .. +3
     const int y = y0 + w;
     const bool act = is_main && y < ny;
-    const int yc = act ? y : 0;
-    const int yp = (yc + 1 == ny) ? 0 : yc + 1;
-    const size_t ro = (size_t)yc * nx + x0 + 4 * lane;   // own row
-    const size_t ry = (size_t)yp * nx + x0 + 4 * lane;   // row y+1
-    const size_t re = (size_t)yc * nx + xe;              // site right of the own segment
-    // ---- helper-warp geometry: halo row y0-1 (its y+1 row is y0), and halo column x0-1
-    const int yh = (y0 == 0) ? ny - 1 : y0 - 1;
-    const size_t hro = (size_t)yh * nx + x0 + 4 * lane;
-    const size_t hry = (size_t)y0 * nx + x0 + 4 * lane;
-    const size_t hre = (size_t)yh * nx + xe;
-    const int ycol = y0 + lane;                           // column site handled by this helper lane
-    const bool col_act = !is_main && lane < TY && ycol < ny;
-    const int ycolp = (ycol + 1 >= ny) ? 0 : ycol + 1;
+    const int r_own = w + 1;
+    const int cofs = HALO + 4 * lane;                    // staged column of this thread's first site
+    const size_t ro = (size_t)(act ? y : 0) * nx + x0 + 4 * lane;
+    // ---- helper-warp geometry: halo row (staged row 0) and halo column x0-1 (staged column HALO-1)
+    const bool col_act = !is_main && lane < TY;
 
-    // halo column of plane zz -> s_col[zz & 1]   (helper lanes 0..TY-1)
-    auto do_column = [&](int zz) {
-        if (!col_act) return;
-        const int zzp = (zz + 1 == nz) ? 0 : zz + 1;
-        const size_t b = (size_t)zz * sxy + (size_t)ycol * nx;
-        const float pr = __ldg(PR + b + xw), pi = __ldg(PI + b + xw);
-        const float tx = __ldg(TX + b + xw), ty = __ldg(TY_ + b + xw), tz = __ldg(TZ + b + xw);
-        const float ty_r = __ldg(TY_ + b + x0), tz_r = __ldg(TZ + b + x0);
-        const float tx_yp = __ldg(TX + (size_t)zz * sxy + (size_t)ycolp * nx + xw);
-        const float tx_zp = __ldg(TX + (size_t)zzp * sxy + (size_t)ycol * nx + xw);
-        float s, c;
-        link_sincos(tx, s, c);
-        s_col[zz & 1][lane] = make_float4(c * pr - s * pi, c * pi + s * pr,
-                                          plaq_f<COMPACT>(tx + ty_r - tx_yp - ty),
-                                          plaq_f<COMPACT>(tx + tz_r - tx_zp - tz));
-    };
-
-    // ---- prologue: carry of the plane below the chunk (main), column of the first plane (helper)
+    // ---- prologue: hand-down of the plane below the chunk (needs loads 0 and 1)
     V4 c_pr, c_pi, c_tx, c_ty, c_tz;        // own old phi, th of the current plane
     V4 g_bzr, g_bzi, g_sxz, g_syz;          // b_z, S_xz, S_yz of the site below (z-1)
+    mbar_wait(&sm.full[0], 0);
+    mbar_wait(&sm.full[1], 0);
     if (act) {
-        const int zm = (z0 == 0) ? nz - 1 : z0 - 1;
-        const size_t oc = (size_t)z0 * sxy, om = (size_t)zm * sxy;
-        c_pr = ld4(PR + oc + ro); c_pi = ld4(PI + oc + ro);
-        c_tx = ld4(TX + oc + ro); c_ty = ld4(TY_ + oc + ro); c_tz = ld4(TZ + oc + ro);
-        const V4 m_pr = ld4(PR + om + ro), m_pi = ld4(PI + om + ro);
-        const V4 m_tx = ld4(TX + om + ro), m_ty = ld4(TY_ + om + ro), m_tz = ld4(TZ + om + ro);
-        const V4 my_tz = ld4(TZ + om + ry);
-        const float me_tz = right_of(m_tz, TZ + om + re, lane);
+        c_pr = lds4(&sm.raw[1][0][r_own][cofs]); c_pi = lds4(&sm.raw[1][1][r_own][cofs]);
+        c_tx = lds4(&sm.raw[1][2][r_own][cofs]); c_ty = lds4(&sm.raw[1][3][r_own][cofs]);
+        c_tz = lds4(&sm.raw[1][4][r_own][cofs]);
+        if (!(fmaxf(fmaxf(fmaxf(fabsf(c_tx.v[0]), fabsf(c_tx.v[1])), fmaxf(fabsf(c_tx.v[2]), fabsf(c_tx.v[3]))),
+                    fmaxf(fmaxf(fmaxf(fabsf(c_ty.v[0]), fabsf(c_ty.v[1])), fmaxf(fabsf(c_ty.v[2]), fabsf(c_ty.v[3]))),
+                          fmaxf(fmaxf(fabsf(c_tz.v[0]), fabsf(c_tz.v[1])), fmaxf(fabsf(c_tz.v[2]), fabsf(c_tz.v[3]))))) <
+              AH_TILED_TH_LIMIT))
+            *overflow = 1;
+        const V4 m_pr = lds4(&sm.raw[0][0][r_own][cofs]), m_pi = lds4(&sm.raw[0][1][r_own][cofs]);
+        const V4 m_tx = lds4(&sm.raw[0][2][r_own][cofs]), m_ty = lds4(&sm.raw[0][3][r_own][cofs]);
+        const V4 m_tz = lds4(&sm.raw[0][4][r_own][cofs]);
+        const V4 my_tz = lds4(&sm.raw[0][4][r_own + 1][cofs]);
+        const float me_tz = sm.raw[0][4][r_own][cofs + 4];
 #pragma unroll
         for (int j = 0; j < 4; ++j) {
             float s, c;
-            link_sincos(m_tz.v[j], s, c);
+            sincos_poly_f32(m_tz.v[j], s, c);
+            const float tz_xp = (j < 3) ? m_tz.v[j < 3 ? j + 1 : 3] : me_tz;
+            const float a_xz = m_tx.v[j] + tz_xp - c_tx.v[j] - m_tz.v[j];
+            const float a_yz = m_ty.v[j] + my_tz.v[j] - c_ty.v[j] - m_tz.v[j];
+            const float sxz = plaq_f<COMPACT>(a_xz), syz = plaq_f<COMPACT>(a_yz);
             g_bzr.v[j] = c * m_pr.v[j] - s * m_pi.v[j];
             g_bzi.v[j] = c * m_pi.v[j] + s * m_pr.v[j];
-            const float tz_xp = (j < 3) ? m_tz.v[j < 3 ? j + 1 : 3] : me_tz;
-            g_sxz.v[j] = plaq_f<COMPACT>(m_tx.v[j] + tz_xp - c_tx.v[j] - m_tz.v[j]);
-            g_syz.v[j] = plaq_f<COMPACT>(m_ty.v[j] + my_tz.v[j] - c_ty.v[j] - m_tz.v[j]);
+            g_sxz.v[j] = sxz;
+            g_syz.v[j] = syz;
         }
-    } else if (!is_main) {
-        do_column(z0);
     }
-    __syncthreads();
+    __syncthreads();   // slot 0 (load 0) is free from here on
 
-    // ---- march
-    for (int z = z0; z < z1; ++z) {
-        const int buf = z & 1;
-        const int zp = (z + 1 == nz) ? 0 : z + 1;
-        const size_t oc = (size_t)z * sxy, on = (size_t)zp * sxy;
+    // ---- march: iteration n updates plane z0 + n - 1 (slot n % 3), forward plane in slot (n + 1) % 3
+    for (int n = 1; n <= nplanes; ++n) {
+        const int buf = n & 1;
+        const int so = n % NST, sf = (n + 1) % NST;
+        const size_t oc = (size_t)(z0 + n - 1) * sxy + ro;
 
-        V4 n_pr, n_pi, n_tx, n_ty, n_tz;   // own old phi, th of plane z+1
-        V4 P_r, P_i, E_x, E_z;             // Pi+, ep+ still lacking the terms that come from row y-1
+        V4 P_r, P_i, E_x, E_y, E_z;        // Pi+, ep+ still lacking the old Pi, ep and the terms from row y-1 / site x0-1
+        if (n + 2 <= nplanes + 1) produce(n + 2);   // into the slot freed by the previous barrier
+        mbar_wait(&sm.full[sf], ((n + 1) / NST) & 1);
 
         if (act) {
-            n_pr = ld4(PR + on + ro); n_pi = ld4(PI + on + ro);
-            n_tx = ld4(TX + on + ro); n_ty = ld4(TY_ + on + ro); n_tz = ld4(TZ + on + ro);
-            const V4 y_pr = ld4(PR + oc + ry), y_pi = ld4(PI + oc + ry);
-            const V4 y_tx = ld4(TX + oc + ry), y_tz = ld4(TZ + oc + ry);
-            const V4 q_r = ld4(in.f[PI_RE] + oc + ro), q_i = ld4(in.f[PI_IM] + oc + ro);
-            const V4 e_x = ld4(in.f[EP_X] + oc + ro), e_y = ld4(in.f[EP_Y] + oc + ro);
-            const V4 e_z = ld4(in.f[EP_Z] + oc + ro);
-            const float r_pr = right_of(c_pr, PR + oc + re, lane), r_pi = right_of(c_pi, PI + oc + re, lane);
-            const float r_ty = right_of(c_ty, TY_ + oc + re, lane), r_tz = right_of(c_tz, TZ + oc + re, lane);
-
             V4 o_byr, o_byi, o_sxy, o_syz;   // for row y+1, through shared memory
-            V4 E_y, h_bzr, h_bzi, h_sxz;     // h_*: this plane's hand-down to z+1 (with S_yz in o_syz)
+            V4 h_bzr, h_bzi, h_sxz;          // this plane's hand-down to z+1 (with S_yz in o_syz)
             float l_bxr = 0.f, l_bxi = 0.f, l_sxy = 0.f, l_sxz = 0.f;   // from the site to the left
-#pragma unroll
+            const V4 y_pr = lds4(&sm.raw[so][0][r_own + 1][cofs]), y_pi = lds4(&sm.raw[so][1][r_own + 1][cofs]);
+            const V4 y_tx = lds4(&sm.raw[so][2][r_own + 1][cofs]), y_tz = lds4(&sm.raw[so][4][r_own + 1][cofs]);
+            const V4 n_pr = lds4(&sm.raw[sf][0][r_own][cofs]), n_pi = lds4(&sm.raw[sf][1][r_own][cofs]);
+            const V4 n_tx = lds4(&sm.raw[sf][2][r_own][cofs]), n_ty = lds4(&sm.raw[sf][3][r_own][cofs]);
+            // right neighbours of the 4th site: lane+1's first site, or (lane 31) the staged halo column
+            float r_pr = __shfl_down_sync(FULL, c_pr.v[0], 1), r_pi = __shfl_down_sync(FULL, c_pi.v[0], 1);
+            float r_ty = __shfl_down_sync(FULL, c_ty.v[0], 1), r_tz = __shfl_down_sync(FULL, c_tz.v[0], 1);
+            if (lane == 31) {
+                r_pr = sm.raw[so][0][r_own][cofs + 4]; r_pi = sm.raw[so][1][r_own][cofs + 4];
+                r_ty = sm.raw[so][3][r_own][cofs + 4]; r_tz = sm.raw[so][4][r_own][cofs + 4];
+            }
+
+            #pragma unroll
             for (int j = 0; j < 4; ++j) {
                 const float fr = c_pr.v[j], fi = c_pi.v[j];
                 const float tx = c_tx.v[j], ty = c_ty.v[j], tz = c_tz.v[j];
-                float sx, cx, sy, cy, sz, cz;
-                link_sincos(tx, sx, cx);          // Eq. 12
-                link_sincos(ty, sy, cy);
-                link_sincos(tz, sz, cz);
                 const int jn = (j < 3) ? j + 1 : 3;
                 const float xr = (j < 3) ? c_pr.v[jn] : r_pr, xi = (j < 3) ? c_pi.v[jn] : r_pi;
                 const float ty_xp = (j < 3) ? c_ty.v[jn] : r_ty, tz_xp = (j < 3) ? c_tz.v[jn] : r_tz;
+                // plaquette angles owned by s                                    (Eqs. 14-15)
+                const float a_xy = tx + ty_xp - y_tx.v[j] - ty;
+                const float a_xz = tx + tz_xp - n_tx.v[j] - tz;
+                const float a_yz = ty + y_tz.v[j] - n_ty.v[j] - tz;
+                float sx, cx, sy, cy, sz, cz, Sxy, Sxz, Syz;
+                sincos_poly_f32(tx, sx, cx);          // Eq. 12
+                sincos_poly_f32(ty, sy, cy);
+                sincos_poly_f32(tz, sz, cz);
+                Sxy = plaq_f<COMPACT>(a_xy); Sxz = plaq_f<COMPACT>(a_xz); Syz = plaq_f<COMPACT>(a_yz);
                 // forward hops U_i(s) phi(s+i)                                   (Eq. 13)
                 const float fxr = cx * xr + sx * xi, fxi = cx * xi - sx * xr;
                 const float fyr = cy * y_pr.v[j] + sy * y_pi.v[j], fyi = cy * y_pi.v[j] - sy * y_pr.v[j];
@@ -191,10 +299,6 @@ tiled_step_kernel(ConstFields<float> in, Fields<float> out, StepCoef<float> k, i
                 const float bxr = cx * fr - sx * fi, bxi = cx * fi + sx * fr;
                 o_byr.v[j] = cy * fr - sy * fi; o_byi.v[j] = cy * fi + sy * fr;
                 h_bzr.v[j] = cz * fr - sz * fi; h_bzi.v[j] = cz * fi + sz * fr;
-                // plaquettes owned by s                                          (Eqs. 14-15)
-                const float Sxy = plaq_f<COMPACT>(tx + ty_xp - y_tx.v[j] - ty);
-                const float Sxz = plaq_f<COMPACT>(tx + tz_xp - n_tx.v[j] - tz);
-                const float Syz = plaq_f<COMPACT>(ty + y_tz.v[j] - n_ty.v[j] - tz);
                 o_sxy.v[j] = Sxy; o_syz.v[j] = Syz; h_sxz.v[j] = Sxz;
                 // Eq. 7 without the x-1 (j == 0) and y-1 hops
                 float ar = (fxr + fyr) + (fzr + g_bzr.v[j]) - 6.0f * fr;
@@ -207,93 +311,135 @@ tiled_step_kernel(ConstFields<float> in, Fields<float> out, StepCoef<float> k, i
                     ar += l_bxr; ai += l_bxi; cuy += l_sxy; cuz += l_sxz;
                 }
                 const float pot = k.half_lam_q * (fr * fr + fi * fi - k.sig2);
-                P_r.v[j] = k.c1 * q_r.v[j] + (kA * ar - k.c2 * (pot * fr));
-                P_i.v[j] = k.c1 * q_i.v[j] + (kA * ai - k.c2 * (pot * fi));
-                E_x.v[j] = k.w1 * e_x.v[j] + (kJ * (fr * fxi - fi * fxr) - kB * cux);
-                E_y.v[j] = k.w1 * e_y.v[j] + (kJ * (fr * fyi - fi * fyr) - kB * cuy);
-                E_z.v[j] = k.w1 * e_z.v[j] + (kJ * (fr * fzi - fi * fzr) - kB * cuz);
+                // (the old Pi, ep terms are added after the barrier: their copies have the whole phase to land)
+                P_r.v[j] = kA * ar - k.c2 * (pot * fr);
+                P_i.v[j] = kA * ai - k.c2 * (pot * fi);
+                E_x.v[j] = kJ * (fr * fxi - fi * fxr) - kB * cux;
+                E_y.v[j] = kJ * (fr * fyi - fi * fyr) - kB * cuy;
+                E_z.v[j] = kJ * (fr * fzi - fi * fzr) - kB * cuz;
                 l_bxr = bxr; l_bxi = bxi; l_sxy = Sxy; l_sxz = Sxz;
             }
             // y-1 hand-over for the row above
-            s_row[buf][w + 1][0][lane] = f4(o_byr);
-            s_row[buf][w + 1][1][lane] = f4(o_byi);
-            s_row[buf][w + 1][2][lane] = f4(o_sxy);
-            s_row[buf][w + 1][3][lane] = f4(o_syz);
-            // x-1 terms of the first site: lane-1's last site, or (lane 0) the helper's column entry
+            if (w + 1 < TY) {
+                sm.row[buf][w + 1][0][lane] = f4(o_byr);
+                sm.row[buf][w + 1][1][lane] = f4(o_byi);
+                sm.row[buf][w + 1][2][lane] = f4(o_sxy);
+                sm.row[buf][w + 1][3][lane] = f4(o_syz);
+            }
+            // x-1 terms of the first site: lane-1's last site (lane 0: the helper's column entry, after the barrier)
             l_bxr = __shfl_up_sync(FULL, l_bxr, 1);
             l_bxi = __shfl_up_sync(FULL, l_bxi, 1);
             l_sxy = __shfl_up_sync(FULL, l_sxy, 1);
             l_sxz = __shfl_up_sync(FULL, l_sxz, 1);
-            if (lane == 0) {
-                const float4 cdat = s_col[buf][w];
-                l_bxr = cdat.x; l_bxi = cdat.y; l_sxy = cdat.z; l_sxz = cdat.w;
+            if (lane > 0) {
+                P_r.v[0] += kA * l_bxr;
+                P_i.v[0] += kA * l_bxi;
+                E_y.v[0] -= kB * l_sxy;
+                E_z.v[0] -= kB * l_sxz;
             }
-            P_r.v[0] += kA * l_bxr;
-            P_i.v[0] += kA * l_bxi;
-            E_y.v[0] -= kB * l_sxy;
-            E_z.v[0] -= kB * l_sxz;
-            // ep_y+ is complete: store it and th_y+ (Eq. 10)
-            V4 t_y;
-#pragma unroll
-            for (int j = 0; j < 4; ++j) t_y.v[j] = c_ty.v[j] + k.dt * E_y.v[j];
-            st4(out.f[EP_Y] + oc + ro, E_y);
-            st4(out.f[TH_Y] + oc + ro, t_y);
             // roll the z hand-down
             g_bzr = h_bzr; g_bzi = h_bzi; g_sxz = h_sxz; g_syz = o_syz;
         } else if (!is_main) {
-            // helper: shared quantities of the halo row y0-1 at plane z
-            const V4 h_pr = ld4(PR + oc + hro), h_pi = ld4(PI + oc + hro);
-            const V4 h_tx = ld4(TX + oc + hro), h_ty = ld4(TY_ + oc + hro), h_tz = ld4(TZ + oc + hro);
-            const V4 hn_ty = ld4(TY_ + on + hro);
-            const V4 hy_tx = ld4(TX + oc + hry), hy_tz = ld4(TZ + oc + hry);
-            const float hr_ty = right_of(h_ty, TY_ + oc + hre, lane);
+            // helper: shared quantities of the halo row y0-1 (staged row 0) at this plane
+            const V4 h_pr = lds4(&sm.raw[so][0][0][cofs]), h_pi = lds4(&sm.raw[so][1][0][cofs]);
+            const V4 h_tx = lds4(&sm.raw[so][2][0][cofs]), h_ty = lds4(&sm.raw[so][3][0][cofs]);
+            const V4 h_tz = lds4(&sm.raw[so][4][0][cofs]);
+            const V4 hn_ty = lds4(&sm.raw[sf][3][0][cofs]);
+            const V4 hy_tx = lds4(&sm.raw[so][2][1][cofs]), hy_tz = lds4(&sm.raw[so][4][1][cofs]);
+            float hr_ty = __shfl_down_sync(FULL, h_ty.v[0], 1);
+            if (lane == 31) hr_ty = sm.raw[so][3][0][cofs + 4];
             V4 o_byr, o_byi, o_sxy, o_syz;
 #pragma unroll
             for (int j = 0; j < 4; ++j) {
                 float s, c;
-                link_sincos(h_ty.v[j], s, c);
+                sincos_poly_f32(h_ty.v[j], s, c);
+                const float ty_xp = (j < 3) ? h_ty.v[j < 3 ? j + 1 : 3] : hr_ty;
+                const float a_xy = h_tx.v[j] + ty_xp - hy_tx.v[j] - h_ty.v[j];
+                const float a_yz = h_ty.v[j] + hy_tz.v[j] - hn_ty.v[j] - h_tz.v[j];
+                const float sxy_ = plaq_f<COMPACT>(a_xy), syz_ = plaq_f<COMPACT>(a_yz);
                 o_byr.v[j] = c * h_pr.v[j] - s * h_pi.v[j];
                 o_byi.v[j] = c * h_pi.v[j] + s * h_pr.v[j];
-                const float ty_xp = (j < 3) ? h_ty.v[j < 3 ? j + 1 : 3] : hr_ty;
-                o_sxy.v[j] = plaq_f<COMPACT>(h_tx.v[j] + ty_xp - hy_tx.v[j] - h_ty.v[j]);
-                o_syz.v[j] = plaq_f<COMPACT>(h_ty.v[j] + hy_tz.v[j] - hn_ty.v[j] - h_tz.v[j]);
+                o_sxy.v[j] = sxy_;
+                o_syz.v[j] = syz_;
             }
-            s_row[buf][0][0][lane] = f4(o_byr);
-            s_row[buf][0][1][lane] = f4(o_byi);
-            s_row[buf][0][2][lane] = f4(o_sxy);
-            s_row[buf][0][3][lane] = f4(o_syz);
-            if (z + 1 < z1) do_column(z + 1);   // one plane ahead: ready before the main warps' next phase 1
+            sm.row[buf][0][0][lane] = f4(o_byr);
+            sm.row[buf][0][1][lane] = f4(o_byi);
+            sm.row[buf][0][2][lane] = f4(o_sxy);
+            sm.row[buf][0][3][lane] = f4(o_syz);
+            // halo column x0-1 (staged column HALO-1) of tile row `lane`
+            if (col_act) {
+                const int r = lane + 1, cw = HALO - 1;
+                const float pr = sm.raw[so][0][r][cw], pi = sm.raw[so][1][r][cw];
+                const float tx = sm.raw[so][2][r][cw], ty = sm.raw[so][3][r][cw], tz = sm.raw[so][4][r][cw];
+                const float ty_r = sm.raw[so][3][r][cw + 1], tz_r = sm.raw[so][4][r][cw + 1];
+                const float tx_yp = sm.raw[so][2][r + 1][cw], tx_zp = sm.raw[sf][2][r][cw];
+                float s, c;
+                sincos_poly_f32(tx, s, c);
+                const float a_xy = tx + ty_r - tx_yp - ty, a_xz = tx + tz_r - tx_zp - tz;
+                const float sxy_ = plaq_f<COMPACT>(a_xy), sxz_ = plaq_f<COMPACT>(a_xz);
+                sm.col[buf][lane] = make_float4(c * pr - s * pi, c * pi + s * pr, sxy_, sxz_);
+            }
         }
 
+#ifndef AH_NO_BAR
         __syncthreads();
+#endif
 
         if (act) {
-            // add what row y-1 hands over, finish Eqs. 7-10, store
-            const float4 a = s_row[buf][w][0][lane], b = s_row[buf][w][1][lane];
-            const float4 c = s_row[buf][w][2][lane], d = s_row[buf][w][3][lane];
+            // add what row y-1 (and, lane 0, site x0-1) hands over, finish Eqs. 7-10, store
+            const float4 a = sm.row[buf][w][0][lane], b = sm.row[buf][w][1][lane];
+            const float4 c = sm.row[buf][w][2][lane], d = sm.row[buf][w][3][lane];
             const float av[4] = {a.x, a.y, a.z, a.w}, bv[4] = {b.x, b.y, b.z, b.w};
             const float cv[4] = {c.x, c.y, c.z, c.w}, dv[4] = {d.x, d.y, d.z, d.w};
-            V4 f_r, f_i, t_x, t_z;
+            if (lane == 0) {
+                const float4 cdat = sm.col[buf][w];
+                P_r.v[0] += kA * cdat.x;
+                P_i.v[0] += kA * cdat.y;
+                E_y.v[0] -= kB * cdat.z;
+                E_z.v[0] -= kB * cdat.w;
+            }
+            // old Pi, ep of the own sites: staged one plane ahead by this warp
+            mbar_wait(&sm.qfull[w], (n - 1) & 1);
+            const V4 q_r = lds4(&sm.qe[w][0][4 * lane]), q_i = lds4(&sm.qe[w][1][4 * lane]);
+            const V4 e_x = lds4(&sm.qe[w][2][4 * lane]), e_y = lds4(&sm.qe[w][3][4 * lane]);
+            const V4 e_z = lds4(&sm.qe[w][4][4 * lane]);
+            __syncwarp();
+            if (n + 1 <= nplanes) produce_q(n + 1, ro - 4 * lane);
+            V4 f_r, f_i, t_x, t_y, t_z;
 #pragma unroll
             for (int j = 0; j < 4; ++j) {
-                P_r.v[j] += kA * av[j];
-                P_i.v[j] += kA * bv[j];
-                E_x.v[j] += kB * cv[j];
-                E_z.v[j] -= kB * dv[j];
+                P_r.v[j] = k.c1 * q_r.v[j] + (P_r.v[j] + kA * av[j]);
+                P_i.v[j] = k.c1 * q_i.v[j] + (P_i.v[j] + kA * bv[j]);
+                E_x.v[j] = k.w1 * e_x.v[j] + (E_x.v[j] + kB * cv[j]);
+                E_y.v[j] = k.w1 * e_y.v[j] + E_y.v[j];
+                E_z.v[j] = k.w1 * e_z.v[j] + (E_z.v[j] - kB * dv[j]);
                 f_r.v[j] = c_pr.v[j] + k.dt * P_r.v[j];   // Eq. 9
                 f_i.v[j] = c_pi.v[j] + k.dt * P_i.v[j];
                 t_x.v[j] = c_tx.v[j] + k.dt * E_x.v[j];   // Eq. 10
+                t_y.v[j] = c_ty.v[j] + k.dt * E_y.v[j];
                 t_z.v[j] = c_tz.v[j] + k.dt * E_z.v[j];
             }
-            st4(out.f[PI_RE] + oc + ro, P_r);
-            st4(out.f[PI_IM] + oc + ro, P_i);
-            st4(out.f[EP_X] + oc + ro, E_x);
-            st4(out.f[EP_Z] + oc + ro, E_z);
-            st4(out.f[PHI_RE] + oc + ro, f_r);
-            st4(out.f[PHI_IM] + oc + ro, f_i);
-            st4(out.f[TH_X] + oc + ro, t_x);
-            st4(out.f[TH_Z] + oc + ro, t_z);
-            c_pr = n_pr; c_pi = n_pi; c_tx = n_tx; c_ty = n_ty; c_tz = n_tz;
+            st4(out.f[PI_RE] + oc, P_r);
+            st4(out.f[PI_IM] + oc, P_i);
+            st4(out.f[EP_X] + oc, E_x);
+            st4(out.f[EP_Y] + oc, E_y);
+            st4(out.f[EP_Z] + oc, E_z);
+            st4(out.f[PHI_RE] + oc, f_r);
+            st4(out.f[PHI_IM] + oc, f_i);
+            st4(out.f[TH_X] + oc, t_x);
+            st4(out.f[TH_Y] + oc, t_y);
+            st4(out.f[TH_Z] + oc, t_z);
+            // the forward plane becomes the own plane
+            c_pr = lds4(&sm.raw[sf][0][r_own][cofs]); c_pi = lds4(&sm.raw[sf][1][r_own][cofs]);
+            c_tx = lds4(&sm.raw[sf][2][r_own][cofs]); c_ty = lds4(&sm.raw[sf][3][r_own][cofs]);
+            c_tz = lds4(&sm.raw[sf][4][r_own][cofs]);
+            if (n < nplanes) {
+                if (!(fmaxf(fmaxf(fmaxf(fabsf(c_tx.v[0]), fabsf(c_tx.v[1])), fmaxf(fabsf(c_tx.v[2]), fabsf(c_tx.v[3]))),
+                            fmaxf(fmaxf(fmaxf(fabsf(c_ty.v[0]), fabsf(c_ty.v[1])), fmaxf(fabsf(c_ty.v[2]), fabsf(c_ty.v[3]))),
+                                  fmaxf(fmaxf(fabsf(c_tz.v[0]), fabsf(c_tz.v[1])), fmaxf(fabsf(c_tz.v[2]), fabsf(c_tz.v[3]))))) <
+                      AH_TILED_TH_LIMIT))
+                    *overflow = 1;
+            }
         }
     }
 }
@@ -302,13 +448,24 @@ tiled_step_kernel(ConstFields<float> in, Fields<float> out, StepCoef<float> k, i
 
 // --------------------------------------------------------------------------------- launch
 
-constexpr int TILE_Y = 7;    // 7 main warps + 1 helper = 256 threads, 2 CTAs per SM at 128 registers
+constexpr int TILE_Y = 6;    // 6 main warps + 1 helper = 224 threads, 2 CTAs per SM (106 KB shared memory each)
 
 bool tiled_supported(int nx, int ny, int nz) { return nx >= TILE_X && nx % TILE_X == 0 && ny >= 1 && nz >= 1; }
 
-cudaError_t tiled_setup() { return cudaSuccess; }
+cudaError_t tiled_setup()
+{
+    cudaError_t e = cudaFuncSetAttribute(tiled_step_kernel<TILE_Y, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                         (int)sizeof(Smem<TILE_Y>));
+    if (e != cudaSuccess) return e;
+    e = cudaFuncSetAttribute(tiled_step_kernel<TILE_Y, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                             (int)sizeof(Smem<TILE_Y>));
+    if (e != cudaSuccess) return e;
+    e = cudaFuncSetAttribute(tiled_step_kernel<TILE_Y, true>, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
+    if (e != cudaSuccess) return e;
+    return cudaFuncSetAttribute(tiled_step_kernel<TILE_Y, false>, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
+}
 
-// Planes per CTA: long chunks amortise the prologue (one extra plane of loads and a third of a
+// Planes per CTA: long chunks amortise the prologue (two extra planes of staging and a third of a
 // plane of arithmetic), but the grid should still be many waves of 148 SMs x 2 resident CTAs.
 int tiled_chunk(int nx, int ny, int nz)
 {
@@ -320,17 +477,18 @@ int tiled_chunk(int nx, int ny, int nz)
 }
 
 cudaError_t launch_tiled_step(const ConstFields<float> &in, const Fields<float> &out,
-                              const StepCoef<float> &k, int nx, int ny, int nz, cudaStream_t st)
+                              const StepCoef<float> &k, int nx, int ny, int nz, int *overflow, cudaStream_t st)
 {
     if (!tiled_supported(nx, ny, nz)) return cudaErrorInvalidValue;
     const int zc = tiled_chunk(nx, ny, nz);
     dim3 grid(nx / TILE_X, (ny + TILE_Y - 1) / TILE_Y, (nz + zc - 1) / zc);
     dim3 block((TILE_Y + 1) * 32);
     if (grid.y > 65535u || grid.z > 65535u) return cudaErrorInvalidConfiguration;
+    const size_t smem = sizeof(Smem<TILE_Y>);
     if (k.compact)
-        tiled_step_kernel<TILE_Y, true><<<grid, block, 0, st>>>(in, out, k, nx, ny, nz, zc);
+        tiled_step_kernel<TILE_Y, true><<<grid, block, smem, st>>>(in, out, k, nx, ny, nz, zc, overflow);
     else
-        tiled_step_kernel<TILE_Y, false><<<grid, block, 0, st>>>(in, out, k, nx, ny, nz, zc);
+        tiled_step_kernel<TILE_Y, false><<<grid, block, smem, st>>>(in, out, k, nx, ny, nz, zc, overflow);
     return cudaGetLastError();
 }
 

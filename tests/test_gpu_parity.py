@@ -159,6 +159,38 @@ def test_large_link_angles(ah, oracle):
         sim.close()
 
 
+def test_link_angles_beyond_the_tiled_domain_are_redone(ah, oracle):
+    """|th| >= 2^16 rad is outside the tiled kernel's polynomial range: it must raise its overflow flag and the
+    step must come out of the libm-based redo (identical to the site kernel), then the next, in-range step must
+    run on the fast path again with a cleared flag."""
+    shape = (128, 9, 6)
+    f0 = inputs.random_state(*shape, seed=22, th_amp=0.5)
+    f0[5, 3, 4, 77] = 7.0e4     # one th_y link beyond 2^16
+    f0[4, 0, 0, 0] = -2.5e5     # one th_x link at a tile corner
+    got = {}
+    for kern in kernels_for(ah, shape[0]):
+        sim, Po = both(ah, oracle, shape, kernel=kern, p=1.0, s=0.0)
+        sim.set_fields(f0)
+        sim.step(1, 2.0, 0.1)
+        got[kern] = sim.get_fields()
+        sim.close()
+    assert np.array_equal(got[ah.KERNEL_SITE], got[ah.KERNEL_TILED])
+    ref = oracle.step(Po, f0.copy(), 1, 2.0, 0.1)
+    r = rel_max(got[ah.KERNEL_TILED], ref)
+    # th ~ 1e5 rad carries an fp32 ulp of 8e-3 rad into its plaquettes; fields are compared to their max
+    assert r["phi"] <= 1e-5 and r["th"] <= 1e-6, r
+    # in-range state after an out-of-range one: the flag of the previous step must not leak
+    f1 = inputs.random_state(*shape, seed=23, th_amp=0.5)
+    sim, Po = both(ah, oracle, shape, kernel=ah.KERNEL_TILED, p=1.0, s=0.0)
+    sim.set_fields(f0)
+    sim.step(1, 2.0, 0.1)
+    sim.set_fields(f1)
+    sim.step(3, 2.0, 0.1)
+    r = rel_max(sim.get_fields(), oracle.step(Po, f1.copy(), 3, 2.0, 0.1))
+    assert max(r.values()) <= 5e-6, r
+    sim.close()
+
+
 # ------------------------------------------------------------------------ north_star parity
 
 def test_parity_config1_64cubed_100_and_160_steps(ah, oracle):
