@@ -16,7 +16,8 @@
 //   * every link's U_i = exp(-i th_i) (Eq. 12) is evaluated ONCE (3 sincos per site) and every
 //     plaquette sine (Eqs. 14-15) ONCE (3 per site); each is then handed to the other sites that use it:
 //       x-1 neighbour : inside the thread, or warp shuffle from the lane to the left;
-//       y-1 neighbour : through shared memory (double buffered, ONE __syncthreads per plane);
+//       y-1 neighbour : through shared memory (double buffered; warp-to-warp progress counters, no
+//                       CTA-wide barrier inside the march);
 //       z-1 neighbour : carried in registers from the previous plane of the march;
 //   * warp TY (the "helper") is the TMA producer and evaluates the shared quantities of the halo row
 //     y0-1 and of the halo column x0-1, so the main warps never branch on tile edges.
@@ -89,6 +90,25 @@ __device__ __forceinline__ void bulk_g2s(float *dst, const float *src, unsigned 
                  : "memory");
 }
 
+// ---- warp-to-warp progress through mbarriers (count 1: one elected lane arrives for its warp).  The barrier
+// [n & 1][w] is used by every other iteration; iteration n is its ((n - 1) >> 1)-th phase.  The protocol
+// (see the march) never lets a producer run two phases ahead of a waiter.
+#ifndef AH_CTA_BARRIER
+#define AH_CTA_BARRIER 1   // 1: one __syncthreads per plane (measured faster); 0: warp-to-warp mbarrier protocol
+#endif
+__device__ __forceinline__ void warp_arrive(unsigned long long *bar, int lane)
+{
+    if (AH_CTA_BARRIER) return;
+    __syncwarp();
+    if (lane == 0) asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+// wait until the warp owning `bars` has arrived for iteration m (m <= 0: nothing to wait for)
+template <int STRIDE>
+__device__ __forceinline__ void wait_iter(unsigned long long (*bars)[STRIDE], int idx, int m)
+{
+    if (!AH_CTA_BARRIER && m >= 1) mbar_wait(&bars[m & 1][idx], ((m - 1) >> 1) & 1);
+}
+
 template <bool COMPACT>
 __device__ __forceinline__ float plaq_f(float phi)
 {
@@ -103,6 +123,8 @@ struct Smem {
     float4 col[2][TY];                    // x hand-over of the site x0-1: (b_x.re, b_x.im, S_xy, S_xz)
     unsigned long long full[NST];         // a staged phi, th plane has landed
     unsigned long long qfull[TY];         // a warp's Pi, ep row has landed
+    unsigned long long p1[2][TY + 1];     // [n & 1][w]: warp w (TY = helper) has finished phase 1 of iteration n
+    unsigned long long p2[2][TY];         // [n & 1][w]: main warp w has consumed the hand-overs of iteration n
 };
 
 }  // namespace
@@ -116,6 +138,16 @@ namespace {
 // redoes the step with the libm-based site kernel (ah_api.cu: one_step).
 #define AH_TILED_TH_LIMIT 65536.0f
 
+// sin(x) for |x| < AH_SMALL_ANGLE = 0.5: x - x^3/6 + x^5/120 - x^7/5040, truncation x^9/9! <= 1.1e-8 |x|
+#define AH_SMALL_ANGLE 0.5f
+__device__ __forceinline__ float sin_small_f32(float x)
+{
+    const float x2 = x * x;
+    float p = fmaf(x2, -1.9841270e-4f, 8.3333333e-3f);
+    p = fmaf(p, x2, -1.6666667e-1f);
+    return fmaf(p * x2, x, x);
+}
+
 // Shared quantities a site hands to its +x / +y / +z neighbours (all from OLD fields):
 //   b_i  = conj(U_i(s)) phi(s)      the backward hop of Eq. 13 as seen from s+i
 //   S_ij = sin Phi_ij(s)            Eqs. 14-15 (or Phi_ij itself when !COMPACT)
@@ -127,7 +159,8 @@ tiled_step_kernel(ConstFields<float> in, Fields<float> out, StepCoef<float> k, i
     extern __shared__ __align__(128) unsigned char smem_bytes[];
     Smem<TY> &sm = *reinterpret_cast<Smem<TY> *>(smem_bytes);
 
-    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    const int lane = threadIdx.x & 31;
+    const int w = __shfl_sync(FULL, (int)(threadIdx.x >> 5), 0);   // warp-uniform by construction
     const int x0 = blockIdx.x * TILE_X, y0 = blockIdx.y * TY, z0 = blockIdx.z * zc;
     const int z1 = min(nz, z0 + zc);
     const int nplanes = z1 - z0;           // planes this CTA updates; loads n = 0 .. nplanes + 1
@@ -138,29 +171,20 @@ tiled_step_kernel(ConstFields<float> in, Fields<float> out, StepCoef<float> k, i
     // load n  <->  plane z0 - 1 + n (periodic), slot n % NST.  Every main warp copies its own staged row
     // (lanes 0..4: one field each), the helper warp the two halo rows 0 and TY+1 (lanes 0..9) and arms
     // the slot's mbarrier with the byte count of the whole plane.
+    // One elected lane per warp issues them, with warp-uniform operands (no per-lane serialisation).
     const bool interior = (x0 > 0) && (x0 + TILE_X < nx);
-    const int p_row = is_main ? w + 1 : (lane < NRAW ? 0 : TY + 1);        // staged row this lane copies
-    const int p_fld = is_main ? lane : (lane < NRAW ? lane : lane - NRAW);   // staged field this lane copies
-    const bool p_act = is_main ? lane < NRAW : lane < 2 * NRAW;
-    size_t p_rowoff;                                                        // y * nx of that row (periodic)
-    {
-        int yy = (y0 - 1 + p_row) % ny;
-        if (yy < 0) yy += ny;
-        p_rowoff = (size_t)yy * nx;
-    }
-    const float *p_base = in.f[PHI_RE];
-    if (p_fld == 1) p_base = in.f[PHI_IM];
-    if (p_fld == 2) p_base = in.f[TH_X];
-    if (p_fld == 3) p_base = in.f[TH_Y];
-    if (p_fld == 4) p_base = in.f[TH_Z];
-    auto produce = [&](int n) {
-        const int slot = n % NST;
-        if (!is_main && lane == 0) mbar_expect_tx(&sm.full[slot], (unsigned)(NRAW * (TY + 2) * ROWF * sizeof(float)));
-        if (p_act) {
-            int zp = (z0 - 1 + n) % nz;
-            if (zp < 0) zp += nz;
-            const float *srow = p_base + (size_t)zp * sxy + p_rowoff;
-            float *dst = &sm.raw[slot][p_fld][p_row][0];
+    auto wrap_y = [&](int yy) {
+        yy %= ny;
+        return yy < 0 ? yy + ny : yy;
+    };
+    const size_t p_row0 = (size_t)wrap_y(is_main ? y0 + w : y0 - 1) * nx;   // main: own row; helper: halo row y0-1
+    const size_t p_row1 = (size_t)wrap_y(y0 + TY) * nx;                      // helper only: halo row y0+TY
+    auto copy_row = [&](int slot, int r, size_t src_off) {
+        constexpr int FLD[NRAW] = {PHI_RE, PHI_IM, TH_X, TH_Y, TH_Z};
+#pragma unroll
+        for (int f = 0; f < NRAW; ++f) {
+            const float *srow = in.f[FLD[f]] + src_off;
+            float *dst = &sm.raw[slot][f][r][0];
             if (interior) {
                 bulk_g2s(dst, srow + x0 - HALO, ROWF * sizeof(float), &sm.full[slot]);
             } else {
@@ -172,19 +196,30 @@ tiled_step_kernel(ConstFields<float> in, Fields<float> out, StepCoef<float> k, i
             }
         }
     };
+    auto produce = [&](int n) {
+        if (lane != 0) return;
+        const int slot = n % NST;
+        int zp = (z0 - 1 + n) % nz;
+        if (zp < 0) zp += nz;
+        const size_t plane = (size_t)zp * sxy;
+        if (is_main) {
+            copy_row(slot, w + 1, plane + p_row0);
+        } else {
+            mbar_expect_tx(&sm.full[slot], (unsigned)(NRAW * (TY + 2) * ROWF * sizeof(float)));
+            copy_row(slot, 0, plane + p_row0);
+            copy_row(slot, TY + 1, plane + p_row1);
+        }
+    };
 
-    // Pi, ep of the warp's own row of plane z0 + n - 1 -> sm.qe[w] (lanes 0..4: one field each)
-    const float *q_base = in.f[PI_RE];
-    if (lane == 1) q_base = in.f[PI_IM];
-    if (lane == 2) q_base = in.f[EP_X];
-    if (lane == 3) q_base = in.f[EP_Y];
-    if (lane == 4) q_base = in.f[EP_Z];
+    // Pi, ep of the warp's own row of plane z0 + n - 1 -> sm.qe[w]
     auto produce_q = [&](int n, size_t row_off) {
-        if (lane == 0) mbar_expect_tx(&sm.qfull[w], (unsigned)(NRAW * TILE_X * sizeof(float)));
-        __syncwarp();
-        if (lane < NRAW)
-            bulk_g2s(&sm.qe[w][lane][0], q_base + (size_t)(z0 + n - 1) * sxy + row_off, TILE_X * sizeof(float),
-                     &sm.qfull[w]);
+        if (lane != 0) return;
+        constexpr int FLD[NRAW] = {PI_RE, PI_IM, EP_X, EP_Y, EP_Z};
+        mbar_expect_tx(&sm.qfull[w], (unsigned)(NRAW * TILE_X * sizeof(float)));
+        const size_t off = (size_t)(z0 + n - 1) * sxy + row_off;
+#pragma unroll
+        for (int f = 0; f < NRAW; ++f)
+            bulk_g2s(&sm.qe[w][f][0], in.f[FLD[f]] + off, TILE_X * sizeof(float), &sm.qfull[w]);
     };
 
     if (threadIdx.x == 0) {
@@ -192,6 +227,10 @@ tiled_step_kernel(ConstFields<float> in, Fields<float> out, StepCoef<float> k, i
         for (int s = 0; s < NST; ++s) mbar_init(&sm.full[s], 1);
 #pragma unroll
         for (int s = 0; s < TY; ++s) mbar_init(&sm.qfull[s], 1);
+#pragma unroll
+        for (int s = 0; s < 2 * (TY + 1); ++s) mbar_init(&sm.p1[0][0] + s, 1);
+#pragma unroll
+        for (int s = 0; s < 2 * TY; ++s) mbar_init(&sm.p2[0][0] + s, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
     }
@@ -249,17 +288,86 @@ tiled_step_kernel(ConstFields<float> in, Fields<float> out, StepCoef<float> k, i
     }
     __syncthreads();   // slot 0 (load 0) is free from here on
 
-    // ---- march: iteration n updates plane z0 + n - 1 (slot n % 3), forward plane in slot (n + 1) % 3
-    for (int n = 1; n <= nplanes; ++n) {
-        const int buf = n & 1;
-        const int so = n % NST, sf = (n + 1) % NST;
-        const size_t oc = (size_t)(z0 + n - 1) * sxy + ro;
-
-        V4 P_r, P_i, E_x, E_y, E_z;        // Pi+, ep+ still lacking the old Pi, ep and the terms from row y-1 / site x0-1
-        if (n + 2 <= nplanes + 1) produce(n + 2);   // into the slot freed by the previous barrier
-        mbar_wait(&sm.full[sf], ((n + 1) / NST) & 1);
-
-        if (act) {
+    // ---- march: iteration n updates plane z0 + n - 1 (slot n % 3), forward plane in slot (n + 1) % 3.
+    // There is no CTA-wide barrier in the march: a warp signals "phase 1 of iteration n done" (its hand-over
+    // is written, its reads of the staged planes are over) and "hand-overs of iteration n consumed" on
+    // mbarriers, and waits only for the warps it depends on.  The three roles run separate loops.
+    // Re-use of a ring slot: the slot of load n+2 held plane n-1; a warp's staged row was last read, in
+    // iteration n-1, by itself, by the warp below it (as its y+1 row) and by the helper (halo column), whose
+    // phase-1 signals it has already waited on; the helper's row TY+1 by the top main warp.
+    if (!is_main) {
+#pragma unroll 1
+        for (int n = 1; n <= nplanes; ++n) {
+            const int buf = n & 1;
+            const int so = n % NST, sf = (n + 1) % NST;
+            wait_iter(sm.p1, TY - 1, n - 1);
+            if (n + 2 <= nplanes + 1) produce(n + 2);
+            mbar_wait(&sm.full[sf], ((n + 1) / NST) & 1);
+            // helper: shared quantities of the halo row y0-1 (staged row 0) at this plane
+            const V4 h_pr = lds4(&sm.raw[so][0][0][cofs]), h_pi = lds4(&sm.raw[so][1][0][cofs]);
+            const V4 h_tx = lds4(&sm.raw[so][2][0][cofs]), h_ty = lds4(&sm.raw[so][3][0][cofs]);
+            const V4 h_tz = lds4(&sm.raw[so][4][0][cofs]);
+            const V4 hn_ty = lds4(&sm.raw[sf][3][0][cofs]);
+            const V4 hy_tx = lds4(&sm.raw[so][2][1][cofs]), hy_tz = lds4(&sm.raw[so][4][1][cofs]);
+            float hr_ty = __shfl_down_sync(FULL, h_ty.v[0], 1);
+            if (lane == 31) hr_ty = sm.raw[so][3][0][cofs + 4];
+            V4 o_byr, o_byi, o_sxy, o_syz;
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                float s, c;
+                sincos_poly_f32(h_ty.v[j], s, c);
+                const float ty_xp = (j < 3) ? h_ty.v[j < 3 ? j + 1 : 3] : hr_ty;
+                const float a_xy = h_tx.v[j] + ty_xp - hy_tx.v[j] - h_ty.v[j];
+                const float a_yz = h_ty.v[j] + hy_tz.v[j] - hn_ty.v[j] - h_tz.v[j];
+                const float sxy_ = plaq_f<COMPACT>(a_xy), syz_ = plaq_f<COMPACT>(a_yz);
+                o_byr.v[j] = c * h_pr.v[j] - s * h_pi.v[j];
+                o_byi.v[j] = c * h_pi.v[j] + s * h_pr.v[j];
+                o_sxy.v[j] = sxy_;
+                o_syz.v[j] = syz_;
+            }
+            // both hand-overs of iteration n-2 must have been consumed by every main warp
+            wait_iter(sm.p2, lane < TY ? lane : TY - 1, n - 2);
+            __syncwarp();
+            sm.row[buf][0][0][lane] = f4(o_byr);
+            sm.row[buf][0][1][lane] = f4(o_byi);
+            sm.row[buf][0][2][lane] = f4(o_sxy);
+            sm.row[buf][0][3][lane] = f4(o_syz);
+            // halo column x0-1 (staged column HALO-1) of tile row `lane`
+            if (col_act) {
+                const int r = lane + 1, cw = HALO - 1;
+                const float pr = sm.raw[so][0][r][cw], pi = sm.raw[so][1][r][cw];
+                const float tx = sm.raw[so][2][r][cw], ty = sm.raw[so][3][r][cw], tz = sm.raw[so][4][r][cw];
+                const float ty_r = sm.raw[so][3][r][cw + 1], tz_r = sm.raw[so][4][r][cw + 1];
+                const float tx_yp = sm.raw[so][2][r + 1][cw], tx_zp = sm.raw[sf][2][r][cw];
+                float s, c;
+                sincos_poly_f32(tx, s, c);
+                const float a_xy = tx + ty_r - tx_yp - ty, a_xz = tx + tz_r - tx_zp - tz;
+                const float sxy_ = plaq_f<COMPACT>(a_xy), sxz_ = plaq_f<COMPACT>(a_xz);
+                sm.col[buf][lane] = make_float4(c * pr - s * pi, c * pi + s * pr, sxy_, sxz_);
+            }
+            warp_arrive(&sm.p1[n & 1][TY], lane);
+            if (AH_CTA_BARRIER) __syncthreads();
+        }
+    } else if (!act) {
+        // a row beyond ny (ragged last tile): keeps the protocol going, computes nothing
+#pragma unroll 1
+        for (int n = 1; n <= nplanes; ++n) {
+            if (n + 2 <= nplanes + 1) produce(n + 2);
+            warp_arrive(&sm.p1[n & 1][w], lane);
+            if (AH_CTA_BARRIER) __syncthreads();
+            if (w > 0) wait_iter(sm.p1, w - 1, n);
+            wait_iter(sm.p1, TY, n);
+            warp_arrive(&sm.p2[n & 1][w], lane);
+        }
+    } else {
+#pragma unroll 1
+        for (int n = 1; n <= nplanes; ++n) {
+            const int buf = n & 1;
+            const int so = n % NST, sf = (n + 1) % NST;
+            const size_t oc = (size_t)(z0 + n - 1) * sxy + ro;
+            V4 P_r, P_i, E_x, E_y, E_z;   // Pi+, ep+ still lacking the old Pi, ep and the terms from row y-1 / site x0-1
+            if (n + 2 <= nplanes + 1) produce(n + 2);
+            mbar_wait(&sm.full[sf], ((n + 1) / NST) & 1);
             V4 o_byr, o_byi, o_sxy, o_syz;   // for row y+1, through shared memory
             V4 h_bzr, h_bzi, h_sxz;          // this plane's hand-down to z+1 (with S_yz in o_syz)
             float l_bxr = 0.f, l_bxi = 0.f, l_sxy = 0.f, l_sxz = 0.f;   // from the site to the left
@@ -275,22 +383,48 @@ tiled_step_kernel(ConstFields<float> in, Fields<float> out, StepCoef<float> k, i
                 r_ty = sm.raw[so][3][r_own][cofs + 4]; r_tz = sm.raw[so][4][r_own][cofs + 4];
             }
 
-            #pragma unroll
+            // plaquette angles owned by the 4 sites (Eqs. 14-15), then their sines: when every angle of the
+            // warp is small (the physical regime) a Taylor polynomial without range reduction is exact to fp32
+            V4 S_xy, S_xz, S_yz;
+            float amax = 0.f;
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                const int jn = (j < 3) ? j + 1 : 3;
+                const float ty_xp = (j < 3) ? c_ty.v[jn] : r_ty, tz_xp = (j < 3) ? c_tz.v[jn] : r_tz;
+                S_xy.v[j] = c_tx.v[j] + ty_xp - y_tx.v[j] - c_ty.v[j];
+                S_xz.v[j] = c_tx.v[j] + tz_xp - n_tx.v[j] - c_tz.v[j];
+                S_yz.v[j] = c_ty.v[j] + y_tz.v[j] - n_ty.v[j] - c_tz.v[j];
+                amax = fmaxf(amax, fmaxf(fmaxf(fabsf(S_xy.v[j]), fabsf(S_xz.v[j])), fabsf(S_yz.v[j])));
+            }
+            if (COMPACT) {
+                if (__all_sync(FULL, amax < AH_SMALL_ANGLE)) {
+#pragma unroll
+                    for (int j = 0; j < 4; ++j) {
+                        S_xy.v[j] = sin_small_f32(S_xy.v[j]);
+                        S_xz.v[j] = sin_small_f32(S_xz.v[j]);
+                        S_yz.v[j] = sin_small_f32(S_yz.v[j]);
+                    }
+                } else {
+#pragma unroll
+                    for (int j = 0; j < 4; ++j) {
+                        S_xy.v[j] = sin_poly_f32(S_xy.v[j]);
+                        S_xz.v[j] = sin_poly_f32(S_xz.v[j]);
+                        S_yz.v[j] = sin_poly_f32(S_yz.v[j]);
+                    }
+                }
+            }
+
+#pragma unroll
             for (int j = 0; j < 4; ++j) {
                 const float fr = c_pr.v[j], fi = c_pi.v[j];
                 const float tx = c_tx.v[j], ty = c_ty.v[j], tz = c_tz.v[j];
                 const int jn = (j < 3) ? j + 1 : 3;
                 const float xr = (j < 3) ? c_pr.v[jn] : r_pr, xi = (j < 3) ? c_pi.v[jn] : r_pi;
-                const float ty_xp = (j < 3) ? c_ty.v[jn] : r_ty, tz_xp = (j < 3) ? c_tz.v[jn] : r_tz;
-                // plaquette angles owned by s                                    (Eqs. 14-15)
-                const float a_xy = tx + ty_xp - y_tx.v[j] - ty;
-                const float a_xz = tx + tz_xp - n_tx.v[j] - tz;
-                const float a_yz = ty + y_tz.v[j] - n_ty.v[j] - tz;
-                float sx, cx, sy, cy, sz, cz, Sxy, Sxz, Syz;
+                const float Sxy = S_xy.v[j], Sxz = S_xz.v[j], Syz = S_yz.v[j];
+                float sx, cx, sy, cy, sz, cz;
                 sincos_poly_f32(tx, sx, cx);          // Eq. 12
                 sincos_poly_f32(ty, sy, cy);
                 sincos_poly_f32(tz, sz, cz);
-                Sxy = plaq_f<COMPACT>(a_xy); Sxz = plaq_f<COMPACT>(a_xz); Syz = plaq_f<COMPACT>(a_yz);
                 // forward hops U_i(s) phi(s+i)                                   (Eq. 13)
                 const float fxr = cx * xr + sx * xi, fxi = cx * xi - sx * xr;
                 const float fyr = cy * y_pr.v[j] + sy * y_pi.v[j], fyi = cy * y_pi.v[j] - sy * y_pr.v[j];
@@ -319,8 +453,9 @@ tiled_step_kernel(ConstFields<float> in, Fields<float> out, StepCoef<float> k, i
                 E_z.v[j] = kJ * (fr * fzi - fi * fzr) - kB * cuz;
                 l_bxr = bxr; l_bxi = bxi; l_sxy = Sxy; l_sxz = Sxz;
             }
-            // y-1 hand-over for the row above
+            // y-1 hand-over for the row above, once that warp has consumed the one of iteration n-2
             if (w + 1 < TY) {
+                wait_iter(sm.p2, w + 1, n - 2);
                 sm.row[buf][w + 1][0][lane] = f4(o_byr);
                 sm.row[buf][w + 1][1][lane] = f4(o_byi);
                 sm.row[buf][w + 1][2][lane] = f4(o_sxy);
@@ -339,53 +474,10 @@ tiled_step_kernel(ConstFields<float> in, Fields<float> out, StepCoef<float> k, i
             }
             // roll the z hand-down
             g_bzr = h_bzr; g_bzi = h_bzi; g_sxz = h_sxz; g_syz = o_syz;
-        } else if (!is_main) {
-            // helper: shared quantities of the halo row y0-1 (staged row 0) at this plane
-            const V4 h_pr = lds4(&sm.raw[so][0][0][cofs]), h_pi = lds4(&sm.raw[so][1][0][cofs]);
-            const V4 h_tx = lds4(&sm.raw[so][2][0][cofs]), h_ty = lds4(&sm.raw[so][3][0][cofs]);
-            const V4 h_tz = lds4(&sm.raw[so][4][0][cofs]);
-            const V4 hn_ty = lds4(&sm.raw[sf][3][0][cofs]);
-            const V4 hy_tx = lds4(&sm.raw[so][2][1][cofs]), hy_tz = lds4(&sm.raw[so][4][1][cofs]);
-            float hr_ty = __shfl_down_sync(FULL, h_ty.v[0], 1);
-            if (lane == 31) hr_ty = sm.raw[so][3][0][cofs + 4];
-            V4 o_byr, o_byi, o_sxy, o_syz;
-#pragma unroll
-            for (int j = 0; j < 4; ++j) {
-                float s, c;
-                sincos_poly_f32(h_ty.v[j], s, c);
-                const float ty_xp = (j < 3) ? h_ty.v[j < 3 ? j + 1 : 3] : hr_ty;
-                const float a_xy = h_tx.v[j] + ty_xp - hy_tx.v[j] - h_ty.v[j];
-                const float a_yz = h_ty.v[j] + hy_tz.v[j] - hn_ty.v[j] - h_tz.v[j];
-                const float sxy_ = plaq_f<COMPACT>(a_xy), syz_ = plaq_f<COMPACT>(a_yz);
-                o_byr.v[j] = c * h_pr.v[j] - s * h_pi.v[j];
-                o_byi.v[j] = c * h_pi.v[j] + s * h_pr.v[j];
-                o_sxy.v[j] = sxy_;
-                o_syz.v[j] = syz_;
-            }
-            sm.row[buf][0][0][lane] = f4(o_byr);
-            sm.row[buf][0][1][lane] = f4(o_byi);
-            sm.row[buf][0][2][lane] = f4(o_sxy);
-            sm.row[buf][0][3][lane] = f4(o_syz);
-            // halo column x0-1 (staged column HALO-1) of tile row `lane`
-            if (col_act) {
-                const int r = lane + 1, cw = HALO - 1;
-                const float pr = sm.raw[so][0][r][cw], pi = sm.raw[so][1][r][cw];
-                const float tx = sm.raw[so][2][r][cw], ty = sm.raw[so][3][r][cw], tz = sm.raw[so][4][r][cw];
-                const float ty_r = sm.raw[so][3][r][cw + 1], tz_r = sm.raw[so][4][r][cw + 1];
-                const float tx_yp = sm.raw[so][2][r + 1][cw], tx_zp = sm.raw[sf][2][r][cw];
-                float s, c;
-                sincos_poly_f32(tx, s, c);
-                const float a_xy = tx + ty_r - tx_yp - ty, a_xz = tx + tz_r - tx_zp - tz;
-                const float sxy_ = plaq_f<COMPACT>(a_xy), sxz_ = plaq_f<COMPACT>(a_xz);
-                sm.col[buf][lane] = make_float4(c * pr - s * pi, c * pi + s * pr, sxy_, sxz_);
-            }
-        }
-
-#ifndef AH_NO_BAR
-        __syncthreads();
-#endif
-
-        if (act) {
+            warp_arrive(&sm.p1[n & 1][w], lane);
+            if (AH_CTA_BARRIER) __syncthreads();
+            if (w > 0) wait_iter(sm.p1, w - 1, n);   // row y-1
+            wait_iter(sm.p1, TY, n);                 // helper: halo column (and, for warp 0, the halo row)
             // add what row y-1 (and, lane 0, site x0-1) hands over, finish Eqs. 7-10, store
             const float4 a = sm.row[buf][w][0][lane], b = sm.row[buf][w][1][lane];
             const float4 c = sm.row[buf][w][2][lane], d = sm.row[buf][w][3][lane];
@@ -398,6 +490,7 @@ tiled_step_kernel(ConstFields<float> in, Fields<float> out, StepCoef<float> k, i
                 E_y.v[0] -= kB * cdat.z;
                 E_z.v[0] -= kB * cdat.w;
             }
+            warp_arrive(&sm.p2[n & 1][w], lane);
             // old Pi, ep of the own sites: staged one plane ahead by this warp
             mbar_wait(&sm.qfull[w], (n - 1) & 1);
             const V4 q_r = lds4(&sm.qe[w][0][4 * lane]), q_i = lds4(&sm.qe[w][1][4 * lane]);
