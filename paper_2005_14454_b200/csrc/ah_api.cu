@@ -134,7 +134,9 @@ int check_time(const ah_ctx *c, double tau, double dt)
     return AH_OK;
 }
 
-int one_step(ah_ctx *c, double tau, double dt)
+// diag_slot >= 0 (tiled fp32 kernel only): the fused DIAG instantiation also leaves the read-outs of the entry
+// snapshot in d_results[diag_slot] (SURVEY 8(a) row D-fuse)
+int one_step(ah_ctx *c, double tau, double dt, int diag_slot = -1)
 {
     cudaError_t e;
     const ah_params &P = c->P;
@@ -146,7 +148,17 @@ int one_step(ah_ctx *c, double tau, double dt)
         // path flagged a link angle beyond its polynomial range; two flags alternate between steps)
         const ah::StepCoef<float> k = make_coef<float>(P, tau, dt);
         int *flag = c->d_overflow + c->step_parity, *next_flag = c->d_overflow + (1 - c->step_parity);
-        e = ah::launch_tiled_step(cur_fields<float>(c), next_fields<float>(c), k, P.nx, P.ny, P.nz, flag, c->st);
+        if (diag_slot >= 0) {
+            const ah::DiagCoef dk = make_diag_coef(P, tau, dt);
+            e = ah::launch_tiled_step(cur_fields<float>(c), next_fields<float>(c), k, P.nx, P.ny, P.nz, flag, c->st,
+                                      &dk, c->d_partials);
+            if (e == cudaSuccess)
+                e = ah::launch_diag_final(c->d_partials, ah::tiled_num_blocks(P.nx, P.ny, P.nz),
+                                          c->d_results + diag_slot, c->st);
+            c->launches += 1;
+        } else {
+            e = ah::launch_tiled_step(cur_fields<float>(c), next_fields<float>(c), k, P.nx, P.ny, P.nz, flag, c->st);
+        }
         if (e == cudaSuccess)
             e = ah::launch_site_redo(flag, next_flag, cur_fields<float>(c), next_fields<float>(c), k, P.nx, P.ny,
                                      P.nz, c->st);
@@ -164,7 +176,9 @@ int one_step(ah_ctx *c, double tau, double dt)
 
 int ensure_diag_scratch(ah_ctx *c, int records)
 {
-    const int nb = ah::diag_num_blocks(c->P.nx, c->P.ny, c->P.nz);
+    int nb = ah::diag_num_blocks(c->P.nx, c->P.ny, c->P.nz);
+    const int nbt = ah::tiled_num_blocks(c->P.nx, c->P.ny, c->P.nz);
+    if (nbt > nb) nb = nbt;
     if (c->n_partials < nb) {
         if (c->d_partials) cudaFree(c->d_partials);
         c->d_partials = nullptr;
@@ -432,13 +446,15 @@ int ah_step_diag(ah_ctx *c, int n, double tau, double dt, int every, ah_diag *ou
     int r = 0;
     for (int j = 0; j < n; ++j) {
         const double tj = tau + (double)j * dt;
-        if (j % every == 0) {
+        const bool diag = (j % every == 0);
+        const bool fused = diag && !c->P.fp64 && c->kernel == AH_KERNEL_TILED;
+        if (diag && !fused) {   // site / fp64 kernels: read-outs by the standalone kernel, then the step
             rc = enqueue_diag(c, tj, dt, r, nullptr, nullptr);
             if (rc != AH_OK) return rc;
-            ++r;
         }
-        rc = one_step(c, tj, dt);
+        rc = one_step(c, tj, dt, fused ? r : -1);
         if (rc != AH_OK) return rc;
+        if (diag) ++r;
     }
     if (r > 0)
         AH_CUDA(cudaMemcpyAsync(c->h_results, c->d_results, sizeof(ah::DiagPartial) * (size_t)r,

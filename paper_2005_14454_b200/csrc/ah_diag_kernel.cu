@@ -11,6 +11,7 @@
 // with warp shuffles, and summed over blocks in a fixed order by a second one-block kernel, so
 // results are bit-reproducible run to run.
 #include "ah_kernels.h"
+#include "ah_diag_site.cuh"
 
 namespace ah {
 
@@ -19,39 +20,33 @@ namespace {
 constexpr int DBX = 64, DBY = 4;   // block = 64 x 4 sites of a z plane ...
 constexpr int DBZ = 8;             // ... marched over 8 consecutive planes
 
-template <typename real> struct Consts;
-template <> struct Consts<float> {
-    static __device__ __forceinline__ float pi() { return 3.14159265358979323846f; }
-    static __device__ __forceinline__ float inv2pi() { return 0.15915494309189533577f; }
-    static __device__ __forceinline__ float atan2r(float y, float x) { return atan2f(y, x); }
-    static __device__ __forceinline__ float rintr(float x) { return rintf(x); }
-};
-template <> struct Consts<double> {
-    static __device__ __forceinline__ double pi() { return 3.14159265358979323846; }
-    static __device__ __forceinline__ double inv2pi() { return 0.15915494309189533577; }
-    static __device__ __forceinline__ double atan2r(double y, double x) { return atan2(y, x); }
-    static __device__ __forceinline__ double rintr(double x) { return rint(x); }
-};
-
-// forward hop U_i(a) phi(b) with U = cos th - i sin th
+// neighbours straight from global memory (periodic wrap on the indices)
 template <typename real>
-__device__ __forceinline__ void hop(real th, real br, real bi, real &hr, real &hi)
-{
-    real s, c;
-    link_sincos(th, s, c);
-    hr = c * br + s * bi;
-    hi = c * bi - s * br;
-}
-
-// d = Arg(conj(phi_a) h)
-template <typename real>
-__device__ __forceinline__ real link_phase(real ar, real ai, real hr, real hi)
-{
-    const real re = ar * hr + ai * hi;
-    const real im = ar * hi - ai * hr;
-    if (re == (real)0 && im == (real)0) return (real)0;
-    return Consts<real>::atan2r(im, re);
-}
+struct GlobalSiteAccessor {
+    const ConstFields<real> &in;
+    int nx, ny, nz, x, y, z;
+    __device__ __forceinline__ size_t at(int dx, int dy, int dz) const
+    {
+        int xx = x + dx, yy = y + dy, zz = z + dz;
+        if (xx >= nx) xx -= nx;
+        if (yy >= ny) yy -= ny;
+        if (zz >= nz) zz -= nz;
+        if (xx < 0) xx += nx;
+        if (yy < 0) yy += ny;
+        if (zz < 0) zz += nz;
+        return (size_t)xx + (size_t)nx * ((size_t)yy + (size_t)ny * (size_t)zz);
+    }
+    __device__ __forceinline__ real phi_re(int dx, int dy, int dz) const { return in.f[PHI_RE][at(dx, dy, dz)]; }
+    __device__ __forceinline__ real phi_im(int dx, int dy, int dz) const { return in.f[PHI_IM][at(dx, dy, dz)]; }
+    __device__ __forceinline__ real th(int i, int dx, int dy, int dz) const { return in.f[TH_X + i][at(dx, dy, dz)]; }
+    __device__ __forceinline__ real pi_re() const { return in.f[PI_RE][at(0, 0, 0)]; }
+    __device__ __forceinline__ real pi_im() const { return in.f[PI_IM][at(0, 0, 0)]; }
+    __device__ __forceinline__ real ep(int i) const { return in.f[EP_X + i][at(0, 0, 0)]; }
+    __device__ __forceinline__ real ep_back(int i) const
+    {
+        return in.f[EP_X + i][at(i == 0 ? -1 : 0, i == 1 ? -1 : 0, i == 2 ? -1 : 0)];
+    }
+};
 
 template <typename real>
 __global__ void __launch_bounds__(DBX * DBY)
@@ -66,105 +61,17 @@ diag_kernel(ConstFields<real> in, DiagCoef k, int nx, int ny, int nz, DiagPartia
     double acc[DS_NFLT] = {0, 0, 0, 0, 0, 0, 0};
 
     const int z_end = min(nz, ((int)blockIdx.z + 1) * DBZ);
+    const size_t n = (size_t)nx * ny * nz;
     for (int z = blockIdx.z * DBZ; active && z < z_end; ++z) {
-        const int xp = (x + 1 == nx) ? 0 : x + 1, xm = (x == 0) ? nx - 1 : x - 1;
-        const int yp = (y + 1 == ny) ? 0 : y + 1, ym = (y == 0) ? ny - 1 : y - 1;
-        const int zp = (z + 1 == nz) ? 0 : z + 1, zm = (z == 0) ? nz - 1 : z - 1;
-        const size_t sxy = (size_t)nx * ny;
-        auto at = [&](int xx, int yy, int zz) { return (size_t)xx + (size_t)nx * yy + sxy * zz; };
-        const size_t c = at(x, y, z);
-        const size_t ip[3] = {at(xp, y, z), at(x, yp, z), at(x, y, zp)};
-        const size_t im[3] = {at(xm, y, z), at(x, ym, z), at(x, y, zm)};
-        // (+,+) edge neighbours x+i+j for (xy, xz, yz)
-        const size_t ipp[3] = {at(xp, yp, z), at(xp, y, zp), at(x, yp, zp)};
-
-        const real *pr = in.f[PHI_RE], *pi = in.f[PHI_IM];
-        const real *th[3] = {in.f[TH_X], in.f[TH_Y], in.f[TH_Z]};
-        const real *ep[3] = {in.f[EP_X], in.f[EP_Y], in.f[EP_Z]};
-
-        const real fr = pr[c], fi = pi[c];
-        const real t0[3] = {th[0][c], th[1][c], th[2][c]};
-
-        // own forward hops and link phases d_i(x)
-        real hr[3], hi[3], d0[3];
-#pragma unroll
-        for (int i = 0; i < 3; ++i) {
-            hop<real>(t0[i], pr[ip[i]], pi[ip[i]], hr[i], hi[i]);
-            d0[i] = link_phase<real>(fr, fi, hr[i], hi[i]);
-        }
-
-        // ---- D1: three plaquettes (xy, xz, yz)
-        const real lim = Consts<real>::pi() - (real)1e-5;
-        real Phi[3];
+        const GlobalSiteAccessor<real> a{in, nx, ny, nz, x, y, z};
+        int wi[3], nearf[3];
+        diag_site<real>(a, k, cnt, acc, wi, nearf);
+        const size_t c = a.at(0, 0, 0);
 #pragma unroll
         for (int pq = 0; pq < 3; ++pq) {
-            const int i = (pq == 2) ? 1 : 0;
-            const int j = (pq == 0) ? 1 : 2;
-            // d_j(x+i): link j leaving x+i, ending at x+i+j
-            real ar = pr[ip[i]], ai = pi[ip[i]], gr, gi;
-            hop<real>(th[j][ip[i]], pr[ipp[pq]], pi[ipp[pq]], gr, gi);
-            const real d2 = link_phase<real>(ar, ai, gr, gi);
-            // d_i(x+j): link i leaving x+j, ending at x+i+j
-            ar = pr[ip[j]];
-            ai = pi[ip[j]];
-            hop<real>(th[i][ip[j]], pr[ipp[pq]], pi[ipp[pq]], gr, gi);
-            const real d3 = link_phase<real>(ar, ai, gr, gi);
-            const real d1 = d0[i], d4 = d0[j];
-            Phi[pq] = t0[i] + th[j][ip[i]] - th[i][ip[j]] - t0[j];   // Eqs. 14-15, un-wrapped
-            const real w = Consts<real>::rintr((d1 + d2 - d3 - d4 + Phi[pq]) * Consts<real>::inv2pi());
-            const int wi = (int)w;
-            const int nearf = (fabs(d1) >= lim) || (fabs(d2) >= lim) || (fabs(d3) >= lim) ||
-                              (fabs(d4) >= lim);
-            cnt[pq] += (wi < 0) ? -wi : wi;
-            cnt[DS_NEAR] += nearf;
-            cnt[DS_BIG] += (fabs(Phi[pq]) > lim) ? 1 : 0;
-            if (w3) w3[(size_t)pq * sxy * nz + c] = (int8_t)wi;
-            if (near3) near3[(size_t)pq * sxy * nz + c] = (uint8_t)nearf;
+            if (w3) w3[(size_t)pq * n + c] = (int8_t)wi[pq];
+            if (near3) near3[(size_t)pq * n + c] = (uint8_t)nearf[pq];
         }
-
-        // ---- D2: Lagrangian density of the site (reading #15)
-        const real idx2 = (real)k.idx2;
-        const real pir = in.f[PI_RE][c], pii = in.f[PI_IM][c];
-        const real pi2 = pir * pir + pii * pii;
-        real grad2 = 0, e2 = 0, b2 = 0;
-        real e0v[3];
-#pragma unroll
-        for (int i = 0; i < 3; ++i) {
-            const real dr = hr[i] - fr, di = hi[i] - fi;
-            grad2 += (dr * dr + di * di) * idx2;
-            e0v[i] = ep[i][c];
-            e2 += e0v[i] * e0v[i] * idx2;
-        }
-#pragma unroll
-        for (int pq = 0; pq < 3; ++pq) {
-            real pe;
-            if (k.compact) {
-                // 2(1 - cos Phi) = 4 sin^2(Phi/2): same number, no cancellation in fp32
-                const real sh = plaq_sin(Phi[pq] * (real)0.5);
-                pe = (real)4 * sh * sh;
-            } else {
-                pe = Phi[pq] * Phi[pq];
-            }
-            b2 += pe * idx2 * idx2;
-        }
-        const real m2 = fr * fr + fi * fi - (real)k.sig2;
-        const real pot = (real)k.quarter_lam_q * m2 * m2;
-        const real L = pi2 - grad2 - pot + (e2 - b2) * (real)k.inv_2e2q;
-        acc[DF_SPI] += (double)pi2 * (double)L;
-        acc[DF_SGR] += (double)grad2 * (double)L;
-        acc[DF_SL] += (double)L;
-
-        // ---- D3: Gauss residual, fp64 from the stored values
-        double div = 0.0;
-#pragma unroll
-        for (int i = 0; i < 3; ++i) div += (double)e0v[i] - (double)ep[i][im[i]];
-        div *= k.idx2;
-        const double charge = k.two_e2_kappa * ((double)fr * (double)pii - (double)fi * (double)pir);
-        const double G = div - charge;
-        acc[DF_GSQ] += G * G;
-        acc[DF_DIVSQ] += div * div;
-        acc[DF_CHSQ] += charge * charge;
-        acc[DF_GMAX] = fmax(acc[DF_GMAX], fabs(G));
     }
 
     // ---- block reduction: warp shuffles, then 8 warps through shared memory
@@ -248,6 +155,12 @@ diag_final_kernel(const DiagPartial *partials, int n, DiagPartial *result)
 int diag_num_blocks(int nx, int ny, int nz)
 {
     return ((nx + DBX - 1) / DBX) * ((ny + DBY - 1) / DBY) * ((nz + DBZ - 1) / DBZ);
+}
+
+cudaError_t launch_diag_final(const DiagPartial *partials, int n, DiagPartial *result, cudaStream_t st)
+{
+    diag_final_kernel<<<1, 1024, 0, st>>>(partials, n, result);
+    return cudaGetLastError();
 }
 
 template <typename real>

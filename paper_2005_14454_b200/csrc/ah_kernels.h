@@ -19,8 +19,13 @@ cudaError_t launch_init(const Fields<real> &out, uint64_t seed, double sigma, si
 bool tiled_supported(int nx, int ny, int nz);
 //   overflow: device int, set to 1 when a link angle is outside the kernel's domain (|th| >= 2^16 rad);
 //             the outputs of that step must then be recomputed with the site kernel
+//   dk, partials: both non-null selects the fused DIAG instantiation (SURVEY 8(a) row D-fuse): the step plus
+//             the read-outs of its ENTRY snapshot, one DiagPartial per CTA (tiled_num_blocks of them), to be
+//             totalled by launch_diag_final
 cudaError_t launch_tiled_step(const ConstFields<float> &in, const Fields<float> &out,
-                              const StepCoef<float> &k, int nx, int ny, int nz, int *overflow, cudaStream_t st);
+                              const StepCoef<float> &k, int nx, int ny, int nz, int *overflow, cudaStream_t st,
+                              const DiagCoef *dk = nullptr, DiagPartial *partials = nullptr);
+int tiled_num_blocks(int nx, int ny, int nz);
 // after a tiled step: redo it with the site kernel iff *flag != 0; clears *clear (the next step's flag)
 cudaError_t launch_site_redo(const int *flag, int *clear, const ConstFields<float> &in, const Fields<float> &out,
                              const StepCoef<float> &k, int nx, int ny, int nz, cudaStream_t st);
@@ -35,6 +40,9 @@ template <typename real>
 cudaError_t launch_diag(const ConstFields<real> &in, const DiagCoef &k, int nx, int ny, int nz,
                         DiagPartial *partials, DiagPartial *result, int8_t *w3, uint8_t *near3,
                         cudaStream_t st);
+
+// fixed-order total of n per-block partials into *result (one block)
+cudaError_t launch_diag_final(const DiagPartial *partials, int n, DiagPartial *result, cudaStream_t st);
 
 // tests only: evaluate the fp32 trig helpers on device arrays
 cudaError_t launch_test_trig(const float *x, float *s, float *c, float *ps, size_t n, cudaStream_t st);

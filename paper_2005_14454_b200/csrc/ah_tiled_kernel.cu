@@ -22,6 +22,7 @@
 //   * warp TY (the "helper") is the TMA producer and evaluates the shared quantities of the halo row
 //     y0-1 and of the halo column x0-1, so the main warps never branch on tile edges.
 #include "ah_kernels.h"
+#include "ah_diag_site.cuh"
 
 namespace ah {
 
@@ -151,10 +152,33 @@ __device__ __forceinline__ float sin_small_f32(float x)
 // Shared quantities a site hands to its +x / +y / +z neighbours (all from OLD fields):
 //   b_i  = conj(U_i(s)) phi(s)      the backward hop of Eq. 13 as seen from s+i
 //   S_ij = sin Phi_ij(s)            Eqs. 14-15 (or Phi_ij itself when !COMPACT)
-template <int TY, bool COMPACT>
+//
+// DIAG = true (SURVEY 8(a) row D-fuse): the same step, plus the read-outs D1-D3 of the ENTRY snapshot of every
+// site, evaluated by diag_site() from what is already staged for the step (phi, th planes with their (+,+)
+// corners, the warp's Pi, ep row); the only extra global reads are the backward ep neighbours.  Per-thread
+// sums are reduced per CTA into partials[linear CTA index]; diag_final_kernel adds them in a fixed order.
+// Staged neighbours from shared memory for diag_site(): the site is column `ci` of staged row `r`
+template <int TY>
+struct StagedSiteAccessor {
+    const Smem<TY> &sm;
+    int so, sf, r, ci, w, qi;          // slots of plane z / z+1, staged row, staged column, warp, column in sm.qe
+    float ebx, eby, ebz;               // ep_x(x - x^), ep_y(x - y^), ep_z(x - z^)
+    __device__ __forceinline__ float phi_re(int dx, int dy, int dz) const { return sm.raw[dz ? sf : so][0][r + dy][ci + dx]; }
+    __device__ __forceinline__ float phi_im(int dx, int dy, int dz) const { return sm.raw[dz ? sf : so][1][r + dy][ci + dx]; }
+    __device__ __forceinline__ float th(int i, int dx, int dy, int dz) const
+    {
+        return sm.raw[dz ? sf : so][2 + i][r + dy][ci + dx];
+    }
+    __device__ __forceinline__ float pi_re() const { return sm.qe[w][0][qi]; }
+    __device__ __forceinline__ float pi_im() const { return sm.qe[w][1][qi]; }
+    __device__ __forceinline__ float ep(int i) const { return sm.qe[w][2 + i][qi]; }
+    __device__ __forceinline__ float ep_back(int i) const { return i == 0 ? ebx : (i == 1 ? eby : ebz); }
+};
+
+template <int TY, bool COMPACT, bool DIAG>
 __global__ void __launch_bounds__((TY + 1) * 32, ((TY + 1) * 32 <= 256) ? 2 : 1)
 tiled_step_kernel(ConstFields<float> in, Fields<float> out, StepCoef<float> k, int nx, int ny, int nz, int zc,
-                  int *overflow)
+                  int *overflow, DiagCoef dk, DiagPartial *partials)
 {
     extern __shared__ __align__(128) unsigned char smem_bytes[];
     Smem<TY> &sm = *reinterpret_cast<Smem<TY> *>(smem_bytes);
@@ -288,6 +312,9 @@ tiled_step_kernel(ConstFields<float> in, Fields<float> out, StepCoef<float> k, i
     }
     __syncthreads();   // slot 0 (load 0) is free from here on
 
+    long long d_cnt[DS_NINT] = {0, 0, 0, 0, 0};      // DIAG only: this thread's partial read-outs
+    double d_acc[DS_NFLT] = {0, 0, 0, 0, 0, 0, 0};
+
     // ---- march: iteration n updates plane z0 + n - 1 (slot n % 3), forward plane in slot (n + 1) % 3.
     // There is no CTA-wide barrier in the march: a warp signals "phase 1 of iteration n done" (its hand-over
     // is written, its reads of the staged planes are over) and "hand-overs of iteration n consumed" on
@@ -368,6 +395,23 @@ tiled_step_kernel(ConstFields<float> in, Fields<float> out, StepCoef<float> k, i
             V4 P_r, P_i, E_x, E_y, E_z;   // Pi+, ep+ still lacking the old Pi, ep and the terms from row y-1 / site x0-1
             if (n + 2 <= nplanes + 1) produce(n + 2);
             mbar_wait(&sm.full[sf], ((n + 1) / NST) & 1);
+            if constexpr (DIAG) {
+                // read-outs of the entry snapshot of this plane (before anything of it is overwritten)
+                mbar_wait(&sm.qfull[w], (n - 1) & 1);
+                const int z = z0 + n - 1, zm = (z == 0) ? nz - 1 : z - 1, ym = (y == 0) ? ny - 1 : y - 1;
+                const int xw = (x0 == 0) ? nx - 1 : x0 - 1;
+                const V4 eby = ld4(in.f[EP_Y] + (size_t)z * sxy + (size_t)ym * nx + x0 + 4 * lane);
+                const V4 ebz = ld4(in.f[EP_Z] + (size_t)zm * sxy + ro);
+                const float ebx0 = (lane == 0) ? __ldg(in.f[EP_X] + (size_t)z * sxy + (size_t)y * nx + xw)
+                                               : sm.qe[w][2][4 * lane - 1];
+#pragma unroll
+                for (int j = 0; j < 4; ++j) {
+                    const StagedSiteAccessor<TY> a{sm, so, sf, r_own, cofs + j, w, 4 * lane + j,
+                                                   j == 0 ? ebx0 : sm.qe[w][2][4 * lane + j - 1], eby.v[j], ebz.v[j]};
+                    int wi[3], nearf[3];
+                    diag_site<float>(a, dk, d_cnt, d_acc, wi, nearf);
+                }
+            }
             V4 o_byr, o_byi, o_sxy, o_syz;   // for row y+1, through shared memory
             V4 h_bzr, h_bzi, h_sxz;          // this plane's hand-down to z+1 (with S_yz in o_syz)
             float l_bxr = 0.f, l_bxi = 0.f, l_sxy = 0.f, l_sxz = 0.f;   // from the site to the left
@@ -535,6 +579,40 @@ tiled_step_kernel(ConstFields<float> in, Fields<float> out, StepCoef<float> k, i
             }
         }
     }
+
+    if constexpr (DIAG) {
+        // CTA reduction: warp shuffles, then the warps through shared memory (the hand-over rows are free now)
+        __syncthreads();
+        double *s_f = reinterpret_cast<double *>(&sm.row[0][0][0][0]);       // [TY + 1][DS_NFLT]
+        long long *s_i = reinterpret_cast<long long *>(s_f + (TY + 1) * DS_NFLT);   // [TY + 1][DS_NINT]
+#pragma unroll
+        for (int a = 0; a < DS_NINT; ++a) d_cnt[a] = warp_sum(d_cnt[a]);
+#pragma unroll
+        for (int a = 0; a < DS_NFLT - 1; ++a) d_acc[a] = warp_sum(d_acc[a]);
+        d_acc[DF_GMAX] = warp_max(d_acc[DF_GMAX]);
+        if (lane == 0) {
+#pragma unroll
+            for (int a = 0; a < DS_NINT; ++a) s_i[w * DS_NINT + a] = d_cnt[a];
+#pragma unroll
+            for (int a = 0; a < DS_NFLT; ++a) s_f[w * DS_NFLT + a] = d_acc[a];
+        }
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            DiagPartial p;
+            for (int a = 0; a < DS_NINT; ++a) {
+                long long v = 0;
+                for (int ww = 0; ww <= TY; ++ww) v += s_i[ww * DS_NINT + a];
+                p.i[a] = v;
+            }
+            for (int a = 0; a < DS_NFLT; ++a) {
+                double v = 0;
+                for (int ww = 0; ww <= TY; ++ww)
+                    v = (a == DF_GMAX) ? fmax(v, s_f[ww * DS_NFLT + a]) : v + s_f[ww * DS_NFLT + a];
+                p.f[a] = v;
+            }
+            partials[blockIdx.x + (size_t)gridDim.x * (blockIdx.y + (size_t)gridDim.y * blockIdx.z)] = p;
+        }
+    }
 }
 
 }  // namespace
@@ -545,17 +623,23 @@ constexpr int TILE_Y = 6;    // 6 main warps + 1 helper = 224 threads, 2 CTAs pe
 
 bool tiled_supported(int nx, int ny, int nz) { return nx >= TILE_X && nx % TILE_X == 0 && ny >= 1 && nz >= 1; }
 
+template <bool COMPACT, bool DIAG>
+static cudaError_t setup_one()
+{
+    cudaError_t e = cudaFuncSetAttribute(tiled_step_kernel<TILE_Y, COMPACT, DIAG>,
+                                         cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Smem<TILE_Y>));
+    if (e != cudaSuccess) return e;
+    return cudaFuncSetAttribute(tiled_step_kernel<TILE_Y, COMPACT, DIAG>,
+                                cudaFuncAttributePreferredSharedMemoryCarveout, 100);
+}
+
 cudaError_t tiled_setup()
 {
-    cudaError_t e = cudaFuncSetAttribute(tiled_step_kernel<TILE_Y, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                         (int)sizeof(Smem<TILE_Y>));
-    if (e != cudaSuccess) return e;
-    e = cudaFuncSetAttribute(tiled_step_kernel<TILE_Y, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                             (int)sizeof(Smem<TILE_Y>));
-    if (e != cudaSuccess) return e;
-    e = cudaFuncSetAttribute(tiled_step_kernel<TILE_Y, true>, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
-    if (e != cudaSuccess) return e;
-    return cudaFuncSetAttribute(tiled_step_kernel<TILE_Y, false>, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
+    cudaError_t e = setup_one<true, false>();
+    if (e == cudaSuccess) e = setup_one<false, false>();
+    if (e == cudaSuccess) e = setup_one<true, true>();
+    if (e == cudaSuccess) e = setup_one<false, true>();
+    return e;
 }
 
 // Planes per CTA: long chunks amortise the prologue (two extra planes of staging and a third of a
@@ -569,8 +653,18 @@ int tiled_chunk(int nx, int ny, int nz)
     return zc < nz ? zc : nz;
 }
 
+int tiled_num_blocks(int nx, int ny, int nz)
+{
+    if (!tiled_supported(nx, ny, nz)) return 0;
+    const int zc = tiled_chunk(nx, ny, nz);
+    return (nx / TILE_X) * ((ny + TILE_Y - 1) / TILE_Y) * ((nz + zc - 1) / zc);
+}
+
+// partials == nullptr: plain step.  Otherwise the DIAG instantiation, which also writes one DiagPartial per
+// CTA (tiled_num_blocks of them) holding the read-outs of the entry snapshot.
 cudaError_t launch_tiled_step(const ConstFields<float> &in, const Fields<float> &out,
-                              const StepCoef<float> &k, int nx, int ny, int nz, int *overflow, cudaStream_t st)
+                              const StepCoef<float> &k, int nx, int ny, int nz, int *overflow, cudaStream_t st,
+                              const DiagCoef *dk, DiagPartial *partials)
 {
     if (!tiled_supported(nx, ny, nz)) return cudaErrorInvalidValue;
     const int zc = tiled_chunk(nx, ny, nz);
@@ -578,10 +672,19 @@ cudaError_t launch_tiled_step(const ConstFields<float> &in, const Fields<float> 
     dim3 block((TILE_Y + 1) * 32);
     if (grid.y > 65535u || grid.z > 65535u) return cudaErrorInvalidConfiguration;
     const size_t smem = sizeof(Smem<TILE_Y>);
-    if (k.compact)
-        tiled_step_kernel<TILE_Y, true><<<grid, block, smem, st>>>(in, out, k, nx, ny, nz, zc, overflow);
-    else
-        tiled_step_kernel<TILE_Y, false><<<grid, block, smem, st>>>(in, out, k, nx, ny, nz, zc, overflow);
+    const bool diag = partials != nullptr && dk != nullptr;
+    const DiagCoef d = diag ? *dk : DiagCoef{};
+    if (k.compact) {
+        if (diag)
+            tiled_step_kernel<TILE_Y, true, true><<<grid, block, smem, st>>>(in, out, k, nx, ny, nz, zc, overflow, d, partials);
+        else
+            tiled_step_kernel<TILE_Y, true, false><<<grid, block, smem, st>>>(in, out, k, nx, ny, nz, zc, overflow, d, nullptr);
+    } else {
+        if (diag)
+            tiled_step_kernel<TILE_Y, false, true><<<grid, block, smem, st>>>(in, out, k, nx, ny, nz, zc, overflow, d, partials);
+        else
+            tiled_step_kernel<TILE_Y, false, false><<<grid, block, smem, st>>>(in, out, k, nx, ny, nz, zc, overflow, d, nullptr);
+    }
     return cudaGetLastError();
 }
 

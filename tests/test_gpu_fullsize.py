@@ -1,0 +1,106 @@
+"""Full-size parity (-m gpu): BASELINE configs[3] (1024^3, the lattice bench.py times, in the launch configuration
+it times) checked on SAMPLED outputs the oracle can compute one by one, plus properties that hold at any size.
+
+One leapfrog step at a site depends only on the 3x3x3 cube around it (Eqs. 7-8: face neighbours and the
+(+i, -j) edge neighbours).  So for a sampled site the 5x5x5 block around it is copied off the device, the oracle
+advances that block as a 5^3 periodic lattice (the wrap never reaches the centre's stencil), and the centre is
+compared with what the CUDA path wrote for that site.  Samples include the lattice faces / edges / corners
+(periodic wrap), tile seams of the tiled kernel (x multiples of 128, y multiples of its row count, z chunk seams)
+and random interior sites.
+"""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+N = 1024
+MODEL = dict(dx=0.5, lambda0=2.0, e0=1.0, sigma=1.0, s=1.0, p=1.0, tau_ref=1.0 + 0.1 * 220, alpha=2.0, compact=1)
+TAU0, DT = 1.0, 0.1
+
+
+def _samples(rng):
+    edge = [0, 1, N - 2, N - 1]
+    seams_x = [127, 128, 511, 512, 895, 896]
+    seams_y = [5, 6, 7, 611, 612, 613, 1019, 1020, 1023]      # tile rows of 6 and 7, and the ragged last tile
+    seams_z = [63, 64, 65, 511, 512, 959, 960]
+    pts = []
+    for x in edge:
+        for y in (0, N - 1, 300):
+            for z in (0, N - 1, 700):
+                pts.append((x, y, z))
+    for x in seams_x:
+        pts.append((x, int(rng.integers(N)), int(rng.integers(N))))
+    for y in seams_y:
+        pts.append((int(rng.integers(N)), y, int(rng.integers(N))))
+    for z in seams_z:
+        pts.append((int(rng.integers(N)), int(rng.integers(N)), z))
+    for _ in range(40):
+        pts.append(tuple(int(v) for v in rng.integers(N, size=3)))
+    return np.array(pts, dtype=np.int64)
+
+
+def _gather_blocks(torch, bufs, pts):
+    """(npts, 10, 5, 5, 5) float64 blocks around the sample sites, periodic indexing, order [field][z][y][x]."""
+    dev = bufs[0].device
+    off = torch.arange(-2, 3, device=dev)
+    p = torch.as_tensor(pts, device=dev)
+    xs = (p[:, 0, None] + off[None, :]) % N
+    ys = (p[:, 1, None] + off[None, :]) % N
+    zs = (p[:, 2, None] + off[None, :]) % N
+    idx = (zs[:, :, None, None] * N + ys[:, None, :, None]) * N + xs[:, None, None, :]      # (npts, 5, 5, 5)
+    return torch.stack([b[idx] for b in bufs], dim=1).double().cpu().numpy()
+
+
+def _gather_sites(torch, bufs, pts):
+    dev = bufs[0].device
+    p = torch.as_tensor(pts, device=dev)
+    idx = (p[:, 2] * N + p[:, 1]) * N + p[:, 0]
+    return torch.stack([b[idx] for b in bufs], dim=1).double().cpu().numpy()
+
+
+def test_1024_cubed_sampled_step_parity_and_invariants(oracle):
+    import torch
+
+    assert torch.cuda.is_available()
+    free, _ = torch.cuda.mem_get_info()
+    if free < 90e9:
+        pytest.skip(f"needs ~86 GB of device memory, {free / 1e9:.0f} GB free")
+    from paper_2005_14454_b200 import binding as ah, build
+    build.build()
+
+    rng = np.random.default_rng(5)
+    pts = _samples(rng)
+    with ah.Simulation(params=ah.make_params(N, **MODEL)) as sim:
+        assert sim.get_kernel() == ah.KERNEL_TILED          # the kernel bench.py times
+        sim.init_fields(1)
+        nwarm = 20
+        sim.step(nwarm, TAU0, DT)                           # th, ep, Pi all non-trivial
+        tau = TAU0 + nwarm * DT
+        before = _gather_blocks(torch, sim.current_bufs(), pts)
+        d0 = sim.diagnostics(tau, DT)
+        sim.step(1, tau, DT)
+        after = _gather_sites(torch, sim.current_bufs(), pts)
+        d1 = sim.diagnostics(tau + DT, DT)
+
+    Po = oracle.make_params(5, 5, 5, **MODEL)
+    scale = {}
+    worst = {}
+    groups = (("phi", slice(0, 2)), ("pi", slice(2, 4)), ("th", slice(4, 7)), ("ep", slice(7, 10)))
+    for name, sl in groups:
+        scale[name] = max(np.abs(before[:, sl]).max(), 1e-30)
+        worst[name] = 0.0
+    for i in range(len(pts)):
+        ref = oracle.step(Po, np.ascontiguousarray(before[i]), 1, tau, DT)[:, 2, 2, 2]
+        for name, sl in groups:
+            worst[name] = max(worst[name], float(np.abs(after[i, sl] - ref[sl]).max() / scale[name]))
+    # one fp32 step from identical inputs: a few ulps of the field's scale (same bound as the small-lattice tests)
+    assert all(v <= 2e-6 for v in worst.values()), worst
+
+    # properties that hold at any size
+    assert d0["n_wind"] > 0 and d1["n_wind"] > 0
+    assert d0["n_wind"] == d0["n_wind_xy"] + d0["n_wind_xz"] + d0["n_wind_yz"]
+    # radiation era: the scheme keeps Gauss's law to round-off (of fp32 here), reading #18
+    assert d0["gauss_rel"] <= 2e-5 and d1["gauss_rel"] <= 2e-5, (d0["gauss_rel"], d1["gauss_rel"])
+    # Eqs. 17-18 from the raw sums (the L weight is not sign-definite before strings form, so no [0, 1] bound)
+    R = d1["sum_pi2_L"] / d1["sum_grad2_L"]
+    assert d1["v2_phi"] == pytest.approx(2.0 * R / (1.0 + R), rel=1e-12)

@@ -335,6 +335,47 @@ def test_step_diag_equals_diagnostics_before_step(ah):
     b.close()
 
 
+@pytest.mark.parametrize("shape,model", [((128, 20, 9), dict(p=1.0, s=1.0, tau_ref=4.0)),
+                                         ((256, 13, 70), dict(p=2.0, s=1.0, tau_ref=5.0)),
+                                         ((128, 6, 3), dict(p=0.0, s=0.0, compact=0))])
+def test_fused_step_diag_tiled_kernel(ah, oracle, shape, model):
+    """Row D-fuse on the tiled kernel: the DIAG instantiation (read-outs from the staged planes, inside the step
+    pass) must give, for the entry snapshot of step j, the integers of the standalone kernel exactly (same
+    per-site arithmetic) and its fp64 sums up to the order of summation; the fields it leaves are those of the
+    plain step; and the whole record agrees with the oracle on the downloaded snapshot."""
+    nx, ny, nz = shape
+    a = ah.Simulation(params=ah.make_params(nx, ny, nz, **model))
+    b = ah.Simulation(params=ah.make_params(nx, ny, nz, **model))
+    assert a.get_kernel() == ah.KERNEL_TILED
+    f0 = inputs.random_state(nx, ny, nz, seed=31, th_amp=0.4)
+    a.set_fields(f0)
+    b.set_fields(f0)
+    every, nsteps, tau0, dt = 4, 10, 1.5, 0.1
+    recs = a.step_diag(nsteps, tau0, dt, every)
+    assert len(recs) == 3
+    ints = ("n_wind", "n_wind_xy", "n_wind_xz", "n_wind_yz", "n_near_branch", "n_big_plaq")
+    sums = ("sum_pi2_L", "sum_grad2_L", "sum_L", "gauss_l2", "gauss_div_l2", "gauss_charge_l2", "v2_phi", "gauss_rel")
+    Po = oracle.make_params(nx, ny, nz, **model)
+    done = 0
+    for r in recs:
+        j = int(round((r["tau"] - tau0) / dt))
+        b.step(j - done, tau0 + done * dt, dt)
+        done = j
+        d = b.diagnostics(r["tau"], dt)
+        for key in ints:
+            assert r[key] == d[key], (key, r[key], d[key])
+        assert r["gauss_max"] == d["gauss_max"]
+        for key in sums:
+            assert r[key] == pytest.approx(d[key], rel=1e-11, abs=1e-300), key
+        od = oracle.diagnostics(Po, b.get_fields().astype(np.float64), r["tau"], dt)
+        assert abs(r["n_wind"] - od["n_wind"]) <= r["n_near_branch"] + od["n_near_branch"]
+        assert r["sum_L"] == pytest.approx(od["sum_L"], rel=1e-5, abs=1e-5 * abs(od["sum_pi2_L"]) + 1e-6)
+    b.step(nsteps - done, tau0 + done * dt, dt)
+    assert np.array_equal(a.get_fields(), b.get_fields())
+    a.close()
+    b.close()
+
+
 def test_diagnostics_deterministic(ah):
     sim = ah.Simulation(nx=48, p=1.0, s=0.0)
     sim.init_fields(8)
