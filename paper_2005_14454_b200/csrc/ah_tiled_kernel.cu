@@ -110,6 +110,20 @@ __device__ __forceinline__ void wait_iter(unsigned long long (*bars)[STRIDE], in
     if (!AH_CTA_BARRIER && m >= 1) mbar_wait(&bars[m & 1][idx], ((m - 1) >> 1) & 1);
 }
 
+// one lane of a converged warp (SASS: ELECT); lets the compiler issue what follows once, with uniform operands
+__device__ __forceinline__ bool elect_one()
+{
+    unsigned p;
+    asm volatile(
+        "{\n"
+        ".reg .pred P;\n"
+        "elect.sync _|P, 0xffffffff;\n"
+        "selp.u32 %0, 1, 0, P;\n"
+        "}\n"
+        : "=r"(p));
+    return p != 0;
+}
+
 template <bool COMPACT>
 __device__ __forceinline__ float plaq_f(float phi)
 {
@@ -220,30 +234,38 @@ tiled_step_kernel(ConstFields<float> in, Fields<float> out, StepCoef<float> k, i
             }
         }
     };
-    auto produce = [&](int n) {
-        if (lane != 0) return;
-        const int slot = n % NST;
-        int zp = (z0 - 1 + n) % nz;
-        if (zp < 0) zp += nz;
-        const size_t plane = (size_t)zp * sxy;
-        if (is_main) {
-            copy_row(slot, w + 1, plane + p_row0);
-        } else {
-            mbar_expect_tx(&sm.full[slot], (unsigned)(NRAW * (TY + 2) * ROWF * sizeof(float)));
-            copy_row(slot, 0, plane + p_row0);
-            copy_row(slot, TY + 1, plane + p_row1);
+    // running state of the next load (no division in the march): ring slot, plane offset of plane z0 - 1 + n
+    int ld_slot = 0, ld_z = (z0 == 0) ? nz - 1 : z0 - 1;
+    size_t ld_plane = (size_t)ld_z * sxy;
+    auto produce = [&]() {
+        if (elect_one()) {
+            if (is_main) {
+                copy_row(ld_slot, w + 1, ld_plane + p_row0);
+            } else {
+                mbar_expect_tx(&sm.full[ld_slot], (unsigned)(NRAW * (TY + 2) * ROWF * sizeof(float)));
+                copy_row(ld_slot, 0, ld_plane + p_row0);
+                copy_row(ld_slot, TY + 1, ld_plane + p_row1);
+            }
+        }
+        ld_slot = (ld_slot == NST - 1) ? 0 : ld_slot + 1;
+        ld_plane += sxy;
+        if (++ld_z == nz) {
+            ld_z = 0;
+            ld_plane = 0;
         }
     };
 
-    // Pi, ep of the warp's own row of plane z0 + n - 1 -> sm.qe[w]
-    auto produce_q = [&](int n, size_t row_off) {
-        if (lane != 0) return;
-        constexpr int FLD[NRAW] = {PI_RE, PI_IM, EP_X, EP_Y, EP_Z};
-        mbar_expect_tx(&sm.qfull[w], (unsigned)(NRAW * TILE_X * sizeof(float)));
-        const size_t off = (size_t)(z0 + n - 1) * sxy + row_off;
+    // Pi, ep of the warp's own row, plane after plane starting at z0 -> sm.qe[w]
+    size_t q_off = (size_t)z0 * sxy + (size_t)(y0 + w < ny ? y0 + w : 0) * nx + x0;
+    auto produce_q = [&]() {
+        if (elect_one()) {
+            constexpr int FLD[NRAW] = {PI_RE, PI_IM, EP_X, EP_Y, EP_Z};
+            mbar_expect_tx(&sm.qfull[w], (unsigned)(NRAW * TILE_X * sizeof(float)));
 #pragma unroll
-        for (int f = 0; f < NRAW; ++f)
-            bulk_g2s(&sm.qe[w][f][0], in.f[FLD[f]] + off, TILE_X * sizeof(float), &sm.qfull[w]);
+            for (int f = 0; f < NRAW; ++f)
+                bulk_g2s(&sm.qe[w][f][0], in.f[FLD[f]] + q_off, TILE_X * sizeof(float), &sm.qfull[w]);
+        }
+        q_off += sxy;
     };
 
     if (threadIdx.x == 0) {
@@ -259,10 +281,10 @@ tiled_step_kernel(ConstFields<float> in, Fields<float> out, StepCoef<float> k, i
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
     }
     __syncthreads();
-    produce(0);
-    produce(1);
-    produce(2);
-    if (is_main && y0 + w < ny) produce_q(1, (size_t)(y0 + w) * nx + x0);
+    produce();   // loads 0, 1, 2
+    produce();
+    produce();
+    if (is_main && y0 + w < ny) produce_q();
 
     const float kA = k.c2 * k.idx2;    // weight of one hop in Pi+          (Eq. 7)
     const float kB = k.w2 * k.idx2;    // weight of one plaquette sine in ep+ (Eq. 8)
@@ -312,6 +334,8 @@ tiled_step_kernel(ConstFields<float> in, Fields<float> out, StepCoef<float> k, i
     }
     __syncthreads();   // slot 0 (load 0) is free from here on
 
+    int sf = 1, sf_par = 0;                           // slot and mbarrier parity of the forward plane (load n + 1)
+    size_t oc = (size_t)z0 * sxy + ro - sxy;          // this thread's element offset in plane z0 + n - 1
     long long d_cnt[DS_NINT] = {0, 0, 0, 0, 0};      // DIAG only: this thread's partial read-outs
     double d_acc[DS_NFLT] = {0, 0, 0, 0, 0, 0, 0};
 
@@ -326,10 +350,11 @@ tiled_step_kernel(ConstFields<float> in, Fields<float> out, StepCoef<float> k, i
 #pragma unroll 1
         for (int n = 1; n <= nplanes; ++n) {
             const int buf = n & 1;
-            const int so = n % NST, sf = (n + 1) % NST;
+            const int so = sf;
+            if (++sf == NST) { sf = 0; sf_par ^= 1; }
             wait_iter(sm.p1, TY - 1, n - 1);
-            if (n + 2 <= nplanes + 1) produce(n + 2);
-            mbar_wait(&sm.full[sf], ((n + 1) / NST) & 1);
+            if (n + 2 <= nplanes + 1) produce();
+            mbar_wait(&sm.full[sf], sf_par);
             // helper: shared quantities of the halo row y0-1 (staged row 0) at this plane
             const V4 h_pr = lds4(&sm.raw[so][0][0][cofs]), h_pi = lds4(&sm.raw[so][1][0][cofs]);
             const V4 h_tx = lds4(&sm.raw[so][2][0][cofs]), h_ty = lds4(&sm.raw[so][3][0][cofs]);
@@ -379,7 +404,7 @@ tiled_step_kernel(ConstFields<float> in, Fields<float> out, StepCoef<float> k, i
         // a row beyond ny (ragged last tile): keeps the protocol going, computes nothing
 #pragma unroll 1
         for (int n = 1; n <= nplanes; ++n) {
-            if (n + 2 <= nplanes + 1) produce(n + 2);
+            if (n + 2 <= nplanes + 1) produce();
             warp_arrive(&sm.p1[n & 1][w], lane);
             if (AH_CTA_BARRIER) __syncthreads();
             if (w > 0) wait_iter(sm.p1, w - 1, n);
@@ -390,11 +415,12 @@ tiled_step_kernel(ConstFields<float> in, Fields<float> out, StepCoef<float> k, i
 #pragma unroll 1
         for (int n = 1; n <= nplanes; ++n) {
             const int buf = n & 1;
-            const int so = n % NST, sf = (n + 1) % NST;
-            const size_t oc = (size_t)(z0 + n - 1) * sxy + ro;
+            const int so = sf;
+            if (++sf == NST) { sf = 0; sf_par ^= 1; }
+            oc += sxy;
             V4 P_r, P_i, E_x, E_y, E_z;   // Pi+, ep+ still lacking the old Pi, ep and the terms from row y-1 / site x0-1
-            if (n + 2 <= nplanes + 1) produce(n + 2);
-            mbar_wait(&sm.full[sf], ((n + 1) / NST) & 1);
+            if (n + 2 <= nplanes + 1) produce();
+            mbar_wait(&sm.full[sf], sf_par);
             if constexpr (DIAG) {
                 // read-outs of the entry snapshot of this plane (before anything of it is overwritten)
                 mbar_wait(&sm.qfull[w], (n - 1) & 1);
@@ -541,7 +567,7 @@ tiled_step_kernel(ConstFields<float> in, Fields<float> out, StepCoef<float> k, i
             const V4 e_x = lds4(&sm.qe[w][2][4 * lane]), e_y = lds4(&sm.qe[w][3][4 * lane]);
             const V4 e_z = lds4(&sm.qe[w][4][4 * lane]);
             __syncwarp();
-            if (n + 1 <= nplanes) produce_q(n + 1, ro - 4 * lane);
+            if (n + 1 <= nplanes) produce_q();
             V4 f_r, f_i, t_x, t_y, t_z;
 #pragma unroll
             for (int j = 0; j < 4; ++j) {
