@@ -67,13 +67,15 @@ def measured_peak():
 
 def recorded_traffic(n, kernel_name):
     """DRAM bytes per launch of the dominant kernel from the committed ncu --set full capture, or None."""
-    p = ROOT / "profiles" / "traffic.json"
+    p = ROOT / "profiles" / "traffic.csv"
     if not p.exists():
         return None
     try:
-        for rec in json.loads(p.read_text()):
-            if rec.get("size") == n and rec.get("kernel") == kernel_name:
-                return float(rec["dram_bytes_per_launch"])
+        import csv
+        with open(p, newline="") as fh:
+            for rec in csv.DictReader(fh):
+                if int(rec["size"]) == n and rec["kernel"] == kernel_name:
+                    return float(rec["dram_bytes_per_launch"])
     except Exception:
         return None
     return None

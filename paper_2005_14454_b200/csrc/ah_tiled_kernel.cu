@@ -8,19 +8,23 @@
 //     tile of 128 x TY sites; the CTA marches through a chunk of z planes;
 //   * the OLD phi, th planes (the only fields with a stencil) are staged in shared memory with their
 //     halo rows y0-1, y0+TY and halo columns x0-4..x0-1, x0+128..x0+131 by 1-D bulk TMA copies
-//     (cp.async.bulk, one per field row) into a 3-slot ring: plane z (own), z+1 (forward) in use, plane
-//     z+2 in flight for one whole iteration.  Completion is signalled on one mbarrier per slot.  The
-//     periodic wrap is applied to the row / plane source addresses by the producer; tiles that touch
-//     the x boundary copy their two 16-byte halo columns separately;
-//   * Pi, ep (read only at their own site) go global -> registers, and all ten outputs registers -> global;
+//     (cp.async.bulk, one per field row, issued by one elected lane of the warp that owns the row) into
+//     a 3-slot ring: plane z (own), z+1 (forward) in use, plane z+2 in flight for one whole iteration.
+//     Completion is signalled on one mbarrier per slot.  The periodic wrap is applied to the row / plane
+//     source addresses; tiles that touch the x boundary copy their two 16-byte halo columns separately;
+//   * the OLD Pi, ep (read only at their own site) are staged per warp, one plane ahead, by the same
+//     mechanism (one mbarrier per warp); all ten outputs go registers -> global (128-bit stores);
+//     nothing the march waits on is a register-destination global load;
 //   * every link's U_i = exp(-i th_i) (Eq. 12) is evaluated ONCE (3 sincos per site) and every
 //     plaquette sine (Eqs. 14-15) ONCE (3 per site); each is then handed to the other sites that use it:
 //       x-1 neighbour : inside the thread, or warp shuffle from the lane to the left;
-//       y-1 neighbour : through shared memory (double buffered; warp-to-warp progress counters, no
-//                       CTA-wide barrier inside the march);
+//       y-1 neighbour : through shared memory (double buffered; ONE __syncthreads per plane);
 //       z-1 neighbour : carried in registers from the previous plane of the march;
-//   * warp TY (the "helper") is the TMA producer and evaluates the shared quantities of the halo row
-//     y0-1 and of the halo column x0-1, so the main warps never branch on tile edges.
+//   * warp TY (the "helper") copies the two halo rows, arms the plane barriers and evaluates the shared
+//     quantities of the halo row y0-1 and of the halo column x0-1, so the main warps never branch on
+//     tile edges;
+//   * no libm in the march: polynomial sin / cos (ah_common.cuh) valid for |th| < 2^16; a link outside
+//     raises a flag and the API redoes the step with the site kernel (ah_api.cu).
 #include "ah_kernels.h"
 #include "ah_diag_site.cuh"
 
@@ -81,6 +85,29 @@ __device__ __forceinline__ void mbar_wait(unsigned long long *bar, unsigned pari
         "bra WAIT_%=;\n"
         "DONE_%=:\n"
         "}\n" ::"r"(smem_u32(bar)), "r"(parity)
+        : "memory");
+}
+// L2 policies: the staged phi, th rows are read again by the neighbouring tiles (halo rows / columns) and by
+// the next z chunk, so they should outlive the read-once Pi, ep rows and the streamed outputs in L2
+__device__ __forceinline__ unsigned long long l2_policy_keep()
+{
+    unsigned long long p;
+    asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(p));
+    return p;
+}
+__device__ __forceinline__ unsigned long long l2_policy_stream()
+{
+    unsigned long long p;
+    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p));
+    return p;
+}
+__device__ __forceinline__ void bulk_g2s_hint(float *dst, const float *src, unsigned bytes, unsigned long long *bar,
+                                              unsigned long long policy)
+{
+    asm volatile(
+        "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;" ::"r"(
+            smem_u32(dst)),
+        "l"(src), "r"(bytes), "r"(smem_u32(bar)), "l"(policy)
         : "memory");
 }
 __device__ __forceinline__ void bulk_g2s(float *dst, const float *src, unsigned bytes, unsigned long long *bar)
@@ -217,6 +244,14 @@ tiled_step_kernel(ConstFields<float> in, Fields<float> out, StepCoef<float> k, i
     };
     const size_t p_row0 = (size_t)wrap_y(is_main ? y0 + w : y0 - 1) * nx;   // main: own row; helper: halo row y0-1
     const size_t p_row1 = (size_t)wrap_y(y0 + TY) * nx;                      // helper only: halo row y0+TY
+#ifndef AH_L2_HINTS
+#define AH_L2_HINTS 1
+#endif
+    const unsigned long long pol_keep = l2_policy_keep(), pol_stream = l2_policy_stream();
+    auto copy1 = [&](float *dst, const float *src, unsigned bytes, unsigned long long *bar) {
+        if (AH_L2_HINTS) bulk_g2s_hint(dst, src, bytes, bar, pol_keep);
+        else bulk_g2s(dst, src, bytes, bar);
+    };
     auto copy_row = [&](int slot, int r, size_t src_off) {
         constexpr int FLD[NRAW] = {PHI_RE, PHI_IM, TH_X, TH_Y, TH_Z};
 #pragma unroll
@@ -224,13 +259,13 @@ tiled_step_kernel(ConstFields<float> in, Fields<float> out, StepCoef<float> k, i
             const float *srow = in.f[FLD[f]] + src_off;
             float *dst = &sm.raw[slot][f][r][0];
             if (interior) {
-                bulk_g2s(dst, srow + x0 - HALO, ROWF * sizeof(float), &sm.full[slot]);
+                copy1(dst, srow + x0 - HALO, ROWF * sizeof(float), &sm.full[slot]);
             } else {
                 const int xl = (x0 == 0) ? nx - HALO : x0 - HALO;
                 const int xr = (x0 + TILE_X == nx) ? 0 : x0 + TILE_X;
-                bulk_g2s(dst + HALO, srow + x0, TILE_X * sizeof(float), &sm.full[slot]);
-                bulk_g2s(dst, srow + xl, HALO * sizeof(float), &sm.full[slot]);
-                bulk_g2s(dst + HALO + TILE_X, srow + xr, HALO * sizeof(float), &sm.full[slot]);
+                copy1(dst + HALO, srow + x0, TILE_X * sizeof(float), &sm.full[slot]);
+                copy1(dst, srow + xl, HALO * sizeof(float), &sm.full[slot]);
+                copy1(dst + HALO + TILE_X, srow + xr, HALO * sizeof(float), &sm.full[slot]);
             }
         }
     };
@@ -263,7 +298,8 @@ tiled_step_kernel(ConstFields<float> in, Fields<float> out, StepCoef<float> k, i
             mbar_expect_tx(&sm.qfull[w], (unsigned)(NRAW * TILE_X * sizeof(float)));
 #pragma unroll
             for (int f = 0; f < NRAW; ++f)
-                bulk_g2s(&sm.qe[w][f][0], in.f[FLD[f]] + q_off, TILE_X * sizeof(float), &sm.qfull[w]);
+                if (AH_L2_HINTS) bulk_g2s_hint(&sm.qe[w][f][0], in.f[FLD[f]] + q_off, TILE_X * sizeof(float), &sm.qfull[w], pol_stream);
+                else bulk_g2s(&sm.qe[w][f][0], in.f[FLD[f]] + q_off, TILE_X * sizeof(float), &sm.qfull[w]);
         }
         q_off += sxy;
     };
@@ -670,11 +706,18 @@ cudaError_t tiled_setup()
 
 // Planes per CTA: long chunks amortise the prologue (two extra planes of staging and a third of a
 // plane of arithmetic), but the grid should still be many waves of 148 SMs x 2 resident CTAs.
+// Measured at 1024^3: 64 and 128 planes tie, 256 loses 4 % to the partial last wave.
+#ifndef AH_ZC_MAX
+#define AH_ZC_MAX 64
+#endif
+#ifndef AH_MIN_WAVES
+#define AH_MIN_WAVES 8
+#endif
 int tiled_chunk(int nx, int ny, int nz)
 {
     const long long cols = (long long)(nx / TILE_X) * ((ny + TILE_Y - 1) / TILE_Y);
-    const long long want = 148LL * 2 * 8;            // >= 8 waves when the lattice allows it
-    int zc = 64;
+    const long long want = 148LL * 2 * AH_MIN_WAVES;   // enough waves that the last, partial one costs little
+    int zc = AH_ZC_MAX;
     while (zc > 8 && cols * ((nz + zc - 1) / zc) < want) zc >>= 1;
     return zc < nz ? zc : nz;
 }
