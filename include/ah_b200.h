@@ -148,6 +148,12 @@ int ah_coeffs(const ah_params *params, double tau, double dt, double *a, double 
 int ah_test_trig(const float *dev_x, float *dev_sin, float *dev_cos, float *dev_plaq_sin, size_t n,
                  void *cuda_stream);
 
+/* Same for the tiled step kernel's own trigonometry (tests only): sin/cos of the pi-reduced polynomial pair it
+ * uses for link variables (valid for |x| < 2^18; the kernel's domain is |th| < 2^16) and the un-reduced Taylor
+ * sine it uses for plaquette angles when a whole warp has |Phi| < 0.5 (dev_small_sin; meaningful for |x| < 0.5). */
+int ah_test_trig_fast(const float *dev_x, float *dev_sin, float *dev_cos, float *dev_small_sin, size_t n,
+                      void *cuda_stream);
+
 /* Message for the calling thread's most recent error ("" if none).  Never NULL. */
 const char *ah_last_error(void);
 

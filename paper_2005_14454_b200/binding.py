@@ -30,7 +30,7 @@ FIELD_NAMES = ("phi_re", "phi_im", "pi_re", "pi_im", "th_x", "th_y", "th_z", "ep
 EXPORTS = (
     "ah_create", "ah_destroy", "ah_init_fields", "ah_set_fields", "ah_get_fields", "ah_current_bufs",
     "ah_step", "ah_diagnostics", "ah_step_diag", "ah_winding_field", "ah_set_kernel", "ah_get_kernel",
-    "ah_launch_count", "ah_coeffs", "ah_test_trig", "ah_last_error", "ah_version",
+    "ah_launch_count", "ah_coeffs", "ah_test_trig", "ah_test_trig_fast", "ah_last_error", "ah_version",
 )
 
 
@@ -98,6 +98,7 @@ def lib():
     L.ah_launch_count.restype = C.c_int64
     L.ah_coeffs.argtypes = [C.POINTER(Params), dp, dp] + [C.POINTER(dp)] * 4
     L.ah_test_trig.argtypes = [vp, vp, vp, vp, C.c_size_t, vp]
+    L.ah_test_trig_fast.argtypes = [vp, vp, vp, vp, C.c_size_t, vp]
     for name in EXPORTS:
         if name not in ("ah_last_error", "ah_version", "ah_launch_count"):
             getattr(L, name).restype = ip
@@ -260,3 +261,15 @@ def test_trig(x):
         st = torch.cuda.current_stream(x.device).cuda_stream
         _check(lib().ah_test_trig(x.data_ptr(), s.data_ptr(), c.data_ptr(), ps.data_ptr(), x.numel(), C.c_void_p(st)))
     return s, c, ps
+
+
+def test_trig_fast(x):
+    """The tiled kernel's own link sin/cos (pi-reduced polynomials) and small-angle sine on a cuda float32 tensor."""
+    import torch
+
+    assert x.is_cuda and x.dtype == torch.float32 and x.is_contiguous()
+    s, c, ss = torch.empty_like(x), torch.empty_like(x), torch.empty_like(x)
+    with torch.cuda.device(x.device):
+        st = torch.cuda.current_stream(x.device).cuda_stream
+        _check(lib().ah_test_trig_fast(x.data_ptr(), s.data_ptr(), c.data_ptr(), ss.data_ptr(), x.numel(), C.c_void_p(st)))
+    return s, c, ss

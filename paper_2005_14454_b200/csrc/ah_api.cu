@@ -506,4 +506,14 @@ int ah_test_trig(const float *dev_x, float *dev_sin, float *dev_cos, float *dev_
     return AH_OK;
 }
 
+int ah_test_trig_fast(const float *dev_x, float *dev_sin, float *dev_cos, float *dev_small_sin, size_t n,
+                      void *cuda_stream)
+{
+    if (!dev_x || !dev_sin || !dev_cos || !dev_small_sin) return fail(AH_EINVAL, "ah_test_trig_fast: null pointer");
+    if (n == 0) return AH_OK;
+    cudaError_t e = ah::launch_test_trig_fast(dev_x, dev_sin, dev_cos, dev_small_sin, n, (cudaStream_t)cuda_stream);
+    if (e != cudaSuccess) return cuda_fail(e, "fast trig test kernel launch");
+    return AH_OK;
+}
+
 }  // extern "C"

@@ -113,6 +113,41 @@ __device__ __forceinline__ float sin_poly_f32(float x)
     return __uint_as_float(__float_as_uint(sr) ^ (__float_as_uint(t) << 31));   // (-1)^k
 }
 
+// Tiled-kernel variants (fewer instructions, no quadrant logic): reduce by multiples of pi to |r| <= pi/2,
+// evaluate sin (degree 9) and cos (degree 10) there and flip both signs for odd multiples.  Absolute error
+// <= 1.5e-7 for |x| < 2^18 (two-term Cody-Waite with FMA: pi = C1 + C2 to 48 bits).
+__device__ __forceinline__ void sincos_pi_f32(float x, float &s, float &c)
+{
+    const float magic = 12582912.0f;                          // 1.5 * 2^23
+    const float t = fmaf(x, 0.31830987334251404f, magic);     // low mantissa bits = rint(x/pi)
+    const float k = t - magic;
+    float r = fmaf(k, -3.1415927410125732f, x);               // fl32(pi)
+    r = fmaf(k, 8.742277657347586e-08f, r);                   // fl32(pi - fl32(pi)) (negative)
+    const float r2 = r * r;
+    float ps = fmaf(r2, 2.5971810373448534e-06f, -0.00019805048941634595f);
+    ps = fmaf(ps, r2, 0.008332990109920502f);
+    ps = fmaf(ps, r2, -0.16666655242443085f);
+    const float sr = fmaf(ps * r2, r, r);
+    float pc = fmaf(r2, -2.605479494377505e-07f, 2.4762006432865746e-05f);
+    pc = fmaf(pc, r2, -0.0013888449175283313f);
+    pc = fmaf(pc, r2, 0.04166664928197861f);
+    pc = fmaf(pc, r2, -0.5f);
+    const float cr = fmaf(pc, r2, 1.0f);
+    const unsigned sign = __float_as_uint(t) << 31;           // (-1)^k
+    s = __uint_as_float(__float_as_uint(sr) ^ sign);
+    c = __uint_as_float(__float_as_uint(cr) ^ sign);
+}
+
+// sin(x) for |x| < AH_SMALL_ANGLE = 0.5: x - x^3/6 + x^5/120 - x^7/5040, truncation x^9/9! <= 1.1e-8 |x|
+#define AH_SMALL_ANGLE 0.5f
+__device__ __forceinline__ float sin_small_f32(float x)
+{
+    const float x2 = x * x;
+    float p = fmaf(x2, -1.9841270e-4f, 8.3333333e-3f);
+    p = fmaf(p, x2, -1.6666667e-1f);
+    return fmaf(p * x2, x, x);
+}
+
 // libm slow paths kept out of line: the hot loops stay small enough for the 32 KB instruction cache
 static __device__ __noinline__ void sincos_slow_f32(float th, float *s, float *c) { sincosf(th, s, c); }
 static __device__ __noinline__ float sin_slow_f32(float x) { return sinf(x); }

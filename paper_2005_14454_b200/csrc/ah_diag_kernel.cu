@@ -195,6 +195,23 @@ __global__ void test_trig_kernel(const float *x, float *s, float *c, float *ps, 
     ps[i] = plaq_sin(x[i]);
 }
 
+__global__ void test_trig_fast_kernel(const float *x, float *s, float *c, float *ss, size_t n)
+{
+    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    float sv, cv;
+    sincos_pi_f32(x[i], sv, cv);
+    s[i] = sv;
+    c[i] = cv;
+    ss[i] = sin_small_f32(x[i]);
+}
+
+cudaError_t launch_test_trig_fast(const float *x, float *s, float *c, float *ss, size_t n, cudaStream_t st)
+{
+    test_trig_fast_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(x, s, c, ss, n);
+    return cudaGetLastError();
+}
+
 cudaError_t launch_test_trig(const float *x, float *s, float *c, float *ps, size_t n, cudaStream_t st)
 {
     test_trig_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(x, s, c, ps, n);

@@ -46,5 +46,6 @@ cudaError_t launch_diag_final(const DiagPartial *partials, int n, DiagPartial *r
 
 // tests only: evaluate the fp32 trig helpers on device arrays
 cudaError_t launch_test_trig(const float *x, float *s, float *c, float *ps, size_t n, cudaStream_t st);
+cudaError_t launch_test_trig_fast(const float *x, float *s, float *c, float *ss, size_t n, cudaStream_t st);
 
 }  // namespace ah

@@ -180,19 +180,6 @@ namespace {
 // redoes the step with the libm-based site kernel (ah_api.cu: one_step).
 #define AH_TILED_TH_LIMIT 65536.0f
 
-// sin(x) for |x| < AH_SMALL_ANGLE = 0.5: x - x^3/6 + x^5/120 - x^7/5040, truncation x^9/9! <= 1.1e-8 |x|
-#define AH_SMALL_ANGLE 0.5f
-__device__ __forceinline__ float sin_small_f32(float x)
-{
-    const float x2 = x * x;
-    float p = fmaf(x2, -1.9841270e-4f, 8.3333333e-3f);
-    p = fmaf(p, x2, -1.6666667e-1f);
-    return fmaf(p * x2, x, x);
-}
-
-// Shared quantities a site hands to its +x / +y / +z neighbours (all from OLD fields):
-//   b_i  = conj(U_i(s)) phi(s)      the backward hop of Eq. 13 as seen from s+i
-//   S_ij = sin Phi_ij(s)            Eqs. 14-15 (or Phi_ij itself when !COMPACT)
 //
 // DIAG = true (SURVEY 8(a) row D-fuse): the same step, plus the read-outs D1-D3 of the ENTRY snapshot of every
 // site, evaluated by diag_site() from what is already staged for the step (phi, th planes with their (+,+)
@@ -357,7 +344,7 @@ tiled_step_kernel(ConstFields<float> in, Fields<float> out, StepCoef<float> k, i
 #pragma unroll
         for (int j = 0; j < 4; ++j) {
             float s, c;
-            sincos_poly_f32(m_tz.v[j], s, c);
+            sincos_pi_f32(m_tz.v[j], s, c);
             const float tz_xp = (j < 3) ? m_tz.v[j < 3 ? j + 1 : 3] : me_tz;
             const float a_xz = m_tx.v[j] + tz_xp - c_tx.v[j] - m_tz.v[j];
             const float a_yz = m_ty.v[j] + my_tz.v[j] - c_ty.v[j] - m_tz.v[j];
@@ -403,7 +390,7 @@ tiled_step_kernel(ConstFields<float> in, Fields<float> out, StepCoef<float> k, i
 #pragma unroll
             for (int j = 0; j < 4; ++j) {
                 float s, c;
-                sincos_poly_f32(h_ty.v[j], s, c);
+                sincos_pi_f32(h_ty.v[j], s, c);
                 const float ty_xp = (j < 3) ? h_ty.v[j < 3 ? j + 1 : 3] : hr_ty;
                 const float a_xy = h_tx.v[j] + ty_xp - hy_tx.v[j] - h_ty.v[j];
                 const float a_yz = h_ty.v[j] + hy_tz.v[j] - hn_ty.v[j] - h_tz.v[j];
@@ -428,7 +415,7 @@ tiled_step_kernel(ConstFields<float> in, Fields<float> out, StepCoef<float> k, i
                 const float ty_r = sm.raw[so][3][r][cw + 1], tz_r = sm.raw[so][4][r][cw + 1];
                 const float tx_yp = sm.raw[so][2][r + 1][cw], tx_zp = sm.raw[sf][2][r][cw];
                 float s, c;
-                sincos_poly_f32(tx, s, c);
+                sincos_pi_f32(tx, s, c);
                 const float a_xy = tx + ty_r - tx_yp - ty, a_xz = tx + tz_r - tx_zp - tz;
                 const float sxy_ = plaq_f<COMPACT>(a_xy), sxz_ = plaq_f<COMPACT>(a_xz);
                 sm.col[buf][lane] = make_float4(c * pr - s * pi, c * pi + s * pr, sxy_, sxz_);
@@ -528,9 +515,9 @@ tiled_step_kernel(ConstFields<float> in, Fields<float> out, StepCoef<float> k, i
                 const float xr = (j < 3) ? c_pr.v[jn] : r_pr, xi = (j < 3) ? c_pi.v[jn] : r_pi;
                 const float Sxy = S_xy.v[j], Sxz = S_xz.v[j], Syz = S_yz.v[j];
                 float sx, cx, sy, cy, sz, cz;
-                sincos_poly_f32(tx, sx, cx);          // Eq. 12
-                sincos_poly_f32(ty, sy, cy);
-                sincos_poly_f32(tz, sz, cz);
+                sincos_pi_f32(tx, sx, cx);          // Eq. 12
+                sincos_pi_f32(ty, sy, cy);
+                sincos_pi_f32(tz, sz, cz);
                 // forward hops U_i(s) phi(s+i)                                   (Eq. 13)
                 const float fxr = cx * xr + sx * xi, fxi = cx * xi - sx * xr;
                 const float fyr = cy * y_pr.v[j] + sy * y_pi.v[j], fyi = cy * y_pi.v[j] - sy * y_pr.v[j];

@@ -74,6 +74,24 @@ def test_trig_against_fp64(ah):
     assert rel.max() <= 2.0e-7   # plaquette sines keep RELATIVE accuracy for small angles
 
 
+def test_tiled_kernel_trig_against_fp64(ah):
+    """The tiled kernel's polynomial pair (reduction by multiples of pi) over its whole domain |th| < 2^16 and up
+    to the 2^18 its plaquette angles can reach, and its Taylor sine for |Phi| < 0.5."""
+    import torch
+    rng = np.random.default_rng(6)
+    parts = [rng.uniform(-s, s, 400_000) for s in (1e-3, 0.5, 4.0, 100.0, 6.5e4, 2.6e5)]
+    parts.append(np.array([0.0, -0.0, np.pi, -np.pi, np.pi / 2, -np.pi / 2, 65535.9, -65535.9, 1e-30]))
+    x = np.concatenate(parts).astype(np.float32)
+    s, c, ss = ah.test_trig_fast(torch.from_numpy(x).cuda())
+    s, c, ss = s.cpu().numpy(), c.cpu().numpy(), ss.cpu().numpy()
+    xd = x.astype(np.float64)
+    assert np.abs(s - np.sin(xd)).max() <= 1.6e-7
+    assert np.abs(c - np.cos(xd)).max() <= 1.6e-7
+    small = np.abs(xd) < 0.5
+    rel = np.abs(ss[small] - np.sin(xd[small])) / np.maximum(np.abs(np.sin(xd[small])), 1e-30)
+    assert rel.max() <= 1.5e-7   # relative accuracy: these feed the gauge force directly
+
+
 # ------------------------------------------------------------------------------------- I0
 
 @pytest.mark.parametrize("fp64", [False, True])
