@@ -254,6 +254,34 @@ def test_parity_tiled_128cubed_physical_width(ah, oracle):
 
 # ------------------------------------------------------------------------------ diagnostics
 
+def test_parity_config2_256cubed_winding_every_20(ah, oracle):
+    """BASELINE configs[1] (256^3, radiation, s=1, winding every 20 steps), first 40 of its 640 steps: the fused
+    step+diagnostics path on the tiled kernel against the oracle advanced from the same device-generated I0."""
+    n, nsteps, every, tau0, dt = 256, 40, 20, 1.0, 0.1
+    model = dict(p=1.0, s=1.0, tau_ref=tau0 + 640 * dt)
+    sim, Po = both(ah, oracle, (n, n, n), **model)
+    assert sim.get_kernel() == ah.KERNEL_TILED
+    sim.init_fields(1)
+    ref = sim.get_fields().astype(np.float64)
+    assert np.abs(ref - oracle.init_fields(Po, 1)).max() <= 1.2e-7
+    recs = sim.step_diag(nsteps, tau0, dt, every)
+    assert [r["tau"] for r in recs] == pytest.approx([1.0, 3.0])
+    got = sim.get_fields()
+    # record 0 is the initial condition: winding of random phases with th = 0, exact integers
+    od = oracle.diagnostics(Po, ref, tau0, dt)
+    assert abs(recs[0]["n_wind"] - od["n_wind"]) <= recs[0]["n_near_branch"] + od["n_near_branch"]
+    assert recs[0]["n_wind"] / (3.0 * n ** 3) == pytest.approx(1.0 / 3.0, abs=2e-3)
+    oracle.step(Po, ref, every, tau0, dt)
+    od = oracle.diagnostics(Po, ref, tau0 + every * dt, dt)
+    # different snapshots here (fp32-evolved vs fp64-evolved): counts agree statistically, not bit for bit
+    assert recs[1]["n_wind"] == pytest.approx(od["n_wind"], rel=2e-3)
+    assert recs[1]["gauss_rel"] <= 2e-5
+    oracle.step(Po, ref, nsteps - every, tau0 + every * dt, dt)
+    r = rel_max(got, ref)
+    assert r["phi"] <= 1e-4 and r["ep"] <= 1e-4 and r["pi"] <= 1e-4 and r["th"] <= 1e-4, r
+    sim.close()
+
+
 def _evolved_snapshot(ah, oracle, n, steps, seed, **model):
     sim, Po = both(ah, oracle, (n, n, n), **model)
     sim.init_fields(seed)
