@@ -39,6 +39,11 @@ struct GlobalSiteAccessor {
     __device__ __forceinline__ real phi_re(int dx, int dy, int dz) const { return in.f[PHI_RE][at(dx, dy, dz)]; }
     __device__ __forceinline__ real phi_im(int dx, int dy, int dz) const { return in.f[PHI_IM][at(dx, dy, dz)]; }
     __device__ __forceinline__ real th(int i, int dx, int dy, int dz) const { return in.f[TH_X + i][at(dx, dy, dz)]; }
+    __device__ __forceinline__ real alpha(int dx, int dy, int dz) const
+    {
+        const size_t c = at(dx, dy, dz);
+        return site_phase<real>(in.f[PHI_RE][c], in.f[PHI_IM][c]);
+    }
     __device__ __forceinline__ real pi_re() const { return in.f[PI_RE][at(0, 0, 0)]; }
     __device__ __forceinline__ real pi_im() const { return in.f[PI_IM][at(0, 0, 0)]; }
     __device__ __forceinline__ real ep(int i) const { return in.f[EP_X + i][at(0, 0, 0)]; }

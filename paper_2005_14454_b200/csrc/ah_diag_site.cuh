@@ -7,12 +7,21 @@
 //   D2 <v^2>_phi   sums of |Pi|^2 L, sum_i |D+_i phi|^2 L, L          (Eqs. 17-18)
 //   D3 Gauss       G = div ep / dx^2 - 2 e0^2 kappa Im(conj(phi) Pi)  (Eq. 5)
 //
+// Link phases.  d_i(x) = Arg(conj(phi(x)) U_i(x) phi(x+i)) is evaluated as the principal value of
+// alpha(x+i) - alpha(x) - th_i(x) with alpha = Arg(phi): the same number up to rounding (a few 1e-7 rad in
+// fp32, far inside the 1e-5 rad band that flags a plaquette as near-branch), but with ONE atan2 per site,
+// shareable between the twelve links that touch it, instead of one sincos + atan2 per link use.  th is first
+// reduced modulo 2 pi with a two-term Cody-Waite step so that large link angles lose nothing.  A site with
+// phi == 0 exactly has no phase: alpha is NaN there and every link touching it gets d = 0 (the oracle's
+// atan2(0,0) := 0 convention).
+//
 // Per-site terms are evaluated in the state's precision (the winding decision is taken in that precision on
 // both sides of a parity test; the Gauss residual, a difference of nearly equal numbers, is evaluated in fp64
 // from the stored values) and accumulated in fp64.
 //
 // The accessor A supplies the snapshot around the site (offsets are 0 or 1 in each direction):
 //   a.phi_re(dx,dy,dz), a.phi_im(dx,dy,dz), a.th(i,dx,dy,dz)   old phi, th at x + (dx,dy,dz)
+//   a.alpha(dx,dy,dz)                                           site_phase() of phi at x + (dx,dy,dz)
 //   a.pi_re(), a.pi_im(), a.ep(i)                               Pi, ep_i at x
 //   a.ep_back(i)                                                ep_i at x - i
 #pragma once
@@ -35,6 +44,42 @@ template <> struct DiagConsts<double> {
     static __device__ __forceinline__ double rintr(double x) { return rint(x); }
 };
 
+// alpha = Arg(phi) in (-pi, pi], NaN when phi == 0
+template <typename real>
+__device__ __forceinline__ real site_phase(real re, real im)
+{
+    if (re == (real)0 && im == (real)0) return (real)NAN;
+    return DiagConsts<real>::atan2r(im, re);
+}
+
+// y - 2 pi rint(y / 2 pi)
+__device__ __forceinline__ float wrap_2pi(float y)
+{
+    const float magic = 12582912.0f;                          // 1.5 * 2^23
+    const float k = fmaf(y, 0.15915494309189535f, magic) - magic;
+    float r = fmaf(k, -6.2831854820251465f, y);               // fl32(2 pi)
+    return fmaf(k, 1.7484555314695172e-07f, r);               // fl32(2 pi - fl32(2 pi)) (negative)
+}
+__device__ __forceinline__ double wrap_2pi(double y)
+{
+    return y - 6.283185307179586476925 * rint(y * 0.15915494309189533577);
+}
+// link angle modulo 2 pi (two-term Cody-Waite is exact enough for |th| < 2^20; beyond that, in fp64)
+__device__ __forceinline__ float reduce_2pi(float th)
+{
+    if (!(fabsf(th) < 1048576.0f)) return (float)wrap_2pi((double)th);
+    return wrap_2pi(th);
+}
+__device__ __forceinline__ double reduce_2pi(double th) { return wrap_2pi(th); }
+
+// d = principal value of alpha_head - alpha_tail - th; 0 when either end has no phase
+template <typename real>
+__device__ __forceinline__ real diag_link_phase(real a_tail, real a_head, real th)
+{
+    const real y = (a_head - a_tail) - reduce_2pi(th);
+    return (y == y) ? wrap_2pi(y) : (real)0;
+}
+
 // forward hop U_i(a) phi(b) with U = cos th - i sin th
 template <typename real>
 __device__ __forceinline__ void diag_hop(real th, real br, real bi, real &hr, real &hi)
@@ -43,16 +88,6 @@ __device__ __forceinline__ void diag_hop(real th, real br, real bi, real &hr, re
     link_sincos(th, s, c);
     hr = c * br + s * bi;
     hi = c * bi - s * br;
-}
-
-// d = Arg(conj(phi_a) h)
-template <typename real>
-__device__ __forceinline__ real diag_link_phase(real ar, real ai, real hr, real hi)
-{
-    const real re = ar * hr + ai * hi;
-    const real im = ar * hi - ai * hr;
-    if (re == (real)0 && im == (real)0) return (real)0;
-    return DiagConsts<real>::atan2r(im, re);
 }
 
 // Adds the site's contributions to cnt[DS_NINT], acc[DS_NFLT]; wi[3], nearf[3] receive the per-plaquette
@@ -67,12 +102,15 @@ __device__ __forceinline__ void diag_site(const A &a, const DiagCoef &k, long lo
     const real nr[3] = {a.phi_re(1, 0, 0), a.phi_re(0, 1, 0), a.phi_re(0, 0, 1)};
     const real ni[3] = {a.phi_im(1, 0, 0), a.phi_im(0, 1, 0), a.phi_im(0, 0, 1)};
 
-    // own forward hops and link phases d_i(x)
+    const real a0 = a.alpha(0, 0, 0);
+    const real an[3] = {a.alpha(1, 0, 0), a.alpha(0, 1, 0), a.alpha(0, 0, 1)};
+
+    // own forward hops (for the gradient energy) and link phases d_i(x)
     real hr[3], hi[3], d0[3];
 #pragma unroll
     for (int i = 0; i < 3; ++i) {
         diag_hop<real>(t0[i], nr[i], ni[i], hr[i], hi[i]);
-        d0[i] = diag_link_phase<real>(fr, fi, hr[i], hi[i]);
+        d0[i] = diag_link_phase<real>(a0, an[i], t0[i]);
     }
 
     // ---- D1: three plaquettes (xy, xz, yz)
@@ -84,16 +122,11 @@ __device__ __forceinline__ void diag_site(const A &a, const DiagCoef &k, long lo
         const int j = (pq == 0) ? 1 : 2;
         const int ix = (i == 0), iy = (i == 1);                 // unit vector of direction i (i is x or y)
         const int jy = (j == 1), jz = (j == 2);                 // unit vector of direction j (j is y or z)
-        const real cr = a.phi_re(ix, iy + jy, jz), ci = a.phi_im(ix, iy + jy, jz);   // phi(x+i+j)
+        const real ac = a.alpha(ix, iy + jy, jz);               // alpha(x+i+j)
         const real th_j_i = a.th(j, ix, iy, 0);                 // th_j(x+i)
         const real th_i_j = a.th(i, 0, jy, jz);                 // th_i(x+j)
-        real gr, gi;
-        // d_j(x+i): link j leaving x+i, ending at x+i+j
-        diag_hop<real>(th_j_i, cr, ci, gr, gi);
-        const real d2 = diag_link_phase<real>(nr[i], ni[i], gr, gi);
-        // d_i(x+j): link i leaving x+j, ending at x+i+j
-        diag_hop<real>(th_i_j, cr, ci, gr, gi);
-        const real d3 = diag_link_phase<real>(nr[j], ni[j], gr, gi);
+        const real d2 = diag_link_phase<real>(an[i], ac, th_j_i);   // d_j(x+i): link j from x+i to x+i+j
+        const real d3 = diag_link_phase<real>(an[j], ac, th_i_j);   // d_i(x+j): link i from x+j to x+i+j
         const real d1 = d0[i], d4 = d0[j];
         Phi[pq] = t0[i] + th_j_i - th_i_j - t0[j];              // Eqs. 14-15, un-wrapped
         const real w = DiagConsts<real>::rintr((d1 + d2 - d3 - d4 + Phi[pq]) * DiagConsts<real>::inv2pi());

@@ -157,11 +157,16 @@ __device__ __forceinline__ float plaq_f(float phi)
     return COMPACT ? sin_poly_f32(phi) : phi;   // reading #10; range check by the caller
 }
 
-template <int TY>
+template <int TY, bool DIAG>
 struct Smem {
     float raw[NST][NRAW][TY + 2][ROWF];   // staged planes; row r <-> y0 - 1 + r, column c <-> x0 - HALO + c
     float qe[TY][NRAW][TILE_X];           // staged old Pi, ep of the own rows (one plane): pi_re, pi_im, ep_x, ep_y, ep_z
-    float4 row[2][TY][4][32];             // y hand-over: (b_y.re, b_y.im, S_xy, S_yz); row 0 = halo row y0-1, row w+1 from warp w
+    // y hand-over: (b_y.re, b_y.im, S_xy, S_yz); row 0 = halo row y0-1, row w+1 from warp w.  Double buffered
+    // (one barrier per plane); the DIAG instantiation has a second barrier per plane anyway and gives the
+    // space to the site phases below
+    float4 row[DIAG ? 1 : 2][TY][4][32];
+    // DIAG: alpha = Arg(phi) (diag_site.cuh) of the staged rows 1 .. TY+1 of the own and the forward plane
+    float alpha[DIAG ? 2 : 1][DIAG ? TY + 1 : 1][DIAG ? ROWF : 4];
     float4 col[2][TY];                    // x hand-over of the site x0-1: (b_x.re, b_x.im, S_xy, S_xz)
     unsigned long long full[NST];         // a staged phi, th plane has landed
     unsigned long long qfull[TY];         // a warp's Pi, ep row has landed
@@ -188,14 +193,18 @@ namespace {
 // Staged neighbours from shared memory for diag_site(): the site is column `ci` of staged row `r`
 template <int TY>
 struct StagedSiteAccessor {
-    const Smem<TY> &sm;
-    int so, sf, r, ci, w, qi;          // slots of plane z / z+1, staged row, staged column, warp, column in sm.qe
+    const Smem<TY, true> &sm;
+    int so, sf, ao, af, r, ci, w, qi;  // slots of plane z / z+1 (raw, alpha), staged row / column, warp, column in sm.qe
     float ebx, eby, ebz;               // ep_x(x - x^), ep_y(x - y^), ep_z(x - z^)
     __device__ __forceinline__ float phi_re(int dx, int dy, int dz) const { return sm.raw[dz ? sf : so][0][r + dy][ci + dx]; }
     __device__ __forceinline__ float phi_im(int dx, int dy, int dz) const { return sm.raw[dz ? sf : so][1][r + dy][ci + dx]; }
     __device__ __forceinline__ float th(int i, int dx, int dy, int dz) const
     {
         return sm.raw[dz ? sf : so][2 + i][r + dy][ci + dx];
+    }
+    __device__ __forceinline__ float alpha(int dx, int dy, int dz) const
+    {
+        return sm.alpha[dz ? af : ao][r - 1 + dy][ci + dx];
     }
     __device__ __forceinline__ float pi_re() const { return sm.qe[w][0][qi]; }
     __device__ __forceinline__ float pi_im() const { return sm.qe[w][1][qi]; }
@@ -209,7 +218,7 @@ tiled_step_kernel(ConstFields<float> in, Fields<float> out, StepCoef<float> k, i
                   int *overflow, DiagCoef dk, DiagPartial *partials)
 {
     extern __shared__ __align__(128) unsigned char smem_bytes[];
-    Smem<TY> &sm = *reinterpret_cast<Smem<TY> *>(smem_bytes);
+    Smem<TY, DIAG> &sm = *reinterpret_cast<Smem<TY, DIAG> *>(smem_bytes);
 
     const int lane = threadIdx.x & 31;
     const int w = __shfl_sync(FULL, (int)(threadIdx.x >> 5), 0);   // warp-uniform by construction
@@ -322,6 +331,18 @@ tiled_step_kernel(ConstFields<float> in, Fields<float> out, StepCoef<float> k, i
     // ---- helper-warp geometry: halo row (staged row 0) and halo column x0-1 (staged column HALO-1)
     const bool col_act = !is_main && lane < TY;
 
+    // DIAG: site phases of this warp's staged row (helper: halo row TY+1) of the plane in `slot` -> sm.alpha[ab]
+    auto stage_alpha = [&](int slot, int ab) {
+        if constexpr (DIAG) {
+            const int r = is_main ? w + 1 : TY + 1;
+            const V4 pr = lds4(&sm.raw[slot][0][r][cofs]), pi = lds4(&sm.raw[slot][1][r][cofs]);
+#pragma unroll 1
+            for (int j = 0; j < 4; ++j) sm.alpha[ab][r - 1][cofs + j] = site_phase<float>(pr.v[j], pi.v[j]);
+            if (lane == 31)
+                sm.alpha[ab][r - 1][cofs + 4] = site_phase<float>(sm.raw[slot][0][r][cofs + 4], sm.raw[slot][1][r][cofs + 4]);
+        }
+    };
+
     // ---- prologue: hand-down of the plane below the chunk (needs loads 0 and 1)
     V4 c_pr, c_pi, c_tx, c_ty, c_tz;        // own old phi, th of the current plane
     V4 g_bzr, g_bzi, g_sxz, g_syz;          // b_z, S_xz, S_yz of the site below (z-1)
@@ -355,9 +376,11 @@ tiled_step_kernel(ConstFields<float> in, Fields<float> out, StepCoef<float> k, i
             g_syz.v[j] = syz;
         }
     }
+    stage_alpha(1, 0);
     __syncthreads();   // slot 0 (load 0) is free from here on
 
     int sf = 1, sf_par = 0;                           // slot and mbarrier parity of the forward plane (load n + 1)
+    int af = 0;                                       // DIAG: sm.alpha buffer of the forward plane
     size_t oc = (size_t)z0 * sxy + ro - sxy;          // this thread's element offset in plane z0 + n - 1
     long long d_cnt[DS_NINT] = {0, 0, 0, 0, 0};      // DIAG only: this thread's partial read-outs
     double d_acc[DS_NFLT] = {0, 0, 0, 0, 0, 0, 0};
@@ -372,12 +395,17 @@ tiled_step_kernel(ConstFields<float> in, Fields<float> out, StepCoef<float> k, i
     if (!is_main) {
 #pragma unroll 1
         for (int n = 1; n <= nplanes; ++n) {
-            const int buf = n & 1;
+            const int buf = DIAG ? 0 : (n & 1);
             const int so = sf;
             if (++sf == NST) { sf = 0; sf_par ^= 1; }
             wait_iter(sm.p1, TY - 1, n - 1);
             if (n + 2 <= nplanes + 1) produce();
             mbar_wait(&sm.full[sf], sf_par);
+            if constexpr (DIAG) {
+                af ^= 1;
+                stage_alpha(sf, af);
+                __syncthreads();
+            }
             // helper: shared quantities of the halo row y0-1 (staged row 0) at this plane
             const V4 h_pr = lds4(&sm.raw[so][0][0][cofs]), h_pi = lds4(&sm.raw[so][1][0][cofs]);
             const V4 h_tx = lds4(&sm.raw[so][2][0][cofs]), h_ty = lds4(&sm.raw[so][3][0][cofs]);
@@ -428,6 +456,13 @@ tiled_step_kernel(ConstFields<float> in, Fields<float> out, StepCoef<float> k, i
 #pragma unroll 1
         for (int n = 1; n <= nplanes; ++n) {
             if (n + 2 <= nplanes + 1) produce();
+            if constexpr (DIAG) {   // the row above the last active one is this warp's (periodic wrap): its phases are needed
+                if (++sf == NST) { sf = 0; sf_par ^= 1; }
+                mbar_wait(&sm.full[sf], sf_par);
+                af ^= 1;
+                stage_alpha(sf, af);
+                __syncthreads();
+            }
             warp_arrive(&sm.p1[n & 1][w], lane);
             if (AH_CTA_BARRIER) __syncthreads();
             if (w > 0) wait_iter(sm.p1, w - 1, n);
@@ -437,7 +472,7 @@ tiled_step_kernel(ConstFields<float> in, Fields<float> out, StepCoef<float> k, i
     } else {
 #pragma unroll 1
         for (int n = 1; n <= nplanes; ++n) {
-            const int buf = n & 1;
+            const int buf = DIAG ? 0 : (n & 1);
             const int so = sf;
             if (++sf == NST) { sf = 0; sf_par ^= 1; }
             oc += sxy;
@@ -445,18 +480,25 @@ tiled_step_kernel(ConstFields<float> in, Fields<float> out, StepCoef<float> k, i
             if (n + 2 <= nplanes + 1) produce();
             mbar_wait(&sm.full[sf], sf_par);
             if constexpr (DIAG) {
+                // site phases of the forward plane, shared by every link phase that needs them
+                af ^= 1;
+                stage_alpha(sf, af);
+                __syncthreads();
                 // read-outs of the entry snapshot of this plane (before anything of it is overwritten)
                 mbar_wait(&sm.qfull[w], (n - 1) & 1);
                 const int z = z0 + n - 1, zm = (z == 0) ? nz - 1 : z - 1, ym = (y == 0) ? ny - 1 : y - 1;
                 const int xw = (x0 == 0) ? nx - 1 : x0 - 1;
-                const V4 eby = ld4(in.f[EP_Y] + (size_t)z * sxy + (size_t)ym * nx + x0 + 4 * lane);
-                const V4 ebz = ld4(in.f[EP_Z] + (size_t)zm * sxy + ro);
+                const float *eby = in.f[EP_Y] + (size_t)z * sxy + (size_t)ym * nx + x0 + 4 * lane;
+                const float *ebz = in.f[EP_Z] + (size_t)zm * sxy + ro;
                 const float ebx0 = (lane == 0) ? __ldg(in.f[EP_X] + (size_t)z * sxy + (size_t)y * nx + xw)
                                                : sm.qe[w][2][4 * lane - 1];
-#pragma unroll
+                // one site at a time, NOT unrolled: the read-outs are long (atan2, libm fall-backs) and four
+                // copies of them would not fit the instruction cache
+#pragma unroll 1
                 for (int j = 0; j < 4; ++j) {
-                    const StagedSiteAccessor<TY> a{sm, so, sf, r_own, cofs + j, w, 4 * lane + j,
-                                                   j == 0 ? ebx0 : sm.qe[w][2][4 * lane + j - 1], eby.v[j], ebz.v[j]};
+                    const StagedSiteAccessor<TY> a{sm, so, sf, af ^ 1, af, r_own, cofs + j, w, 4 * lane + j,
+                                                   j == 0 ? ebx0 : sm.qe[w][2][4 * lane + j - 1], __ldg(eby + j),
+                                                   __ldg(ebz + j)};
                     int wi[3], nearf[3];
                     diag_site<float>(a, dk, d_cnt, d_acc, wi, nearf);
                 }
@@ -676,7 +718,7 @@ template <bool COMPACT, bool DIAG>
 static cudaError_t setup_one()
 {
     cudaError_t e = cudaFuncSetAttribute(tiled_step_kernel<TILE_Y, COMPACT, DIAG>,
-                                         cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Smem<TILE_Y>));
+                                         cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Smem<TILE_Y, DIAG>));
     if (e != cudaSuccess) return e;
     return cudaFuncSetAttribute(tiled_step_kernel<TILE_Y, COMPACT, DIAG>,
                                 cudaFuncAttributePreferredSharedMemoryCarveout, 100);
@@ -727,8 +769,8 @@ cudaError_t launch_tiled_step(const ConstFields<float> &in, const Fields<float> 
     dim3 grid(nx / TILE_X, (ny + TILE_Y - 1) / TILE_Y, (nz + zc - 1) / zc);
     dim3 block((TILE_Y + 1) * 32);
     if (grid.y > 65535u || grid.z > 65535u) return cudaErrorInvalidConfiguration;
-    const size_t smem = sizeof(Smem<TILE_Y>);
     const bool diag = partials != nullptr && dk != nullptr;
+    const size_t smem = diag ? sizeof(Smem<TILE_Y, true>) : sizeof(Smem<TILE_Y, false>);
     const DiagCoef d = diag ? *dk : DiagCoef{};
     if (k.compact) {
         if (diag)
