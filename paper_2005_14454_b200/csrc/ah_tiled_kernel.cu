@@ -736,19 +736,34 @@ cudaError_t tiled_setup()
 // Planes per CTA: long chunks amortise the prologue (two extra planes of staging and a third of a
 // plane of arithmetic), but the grid should still be many waves of 148 SMs x 2 resident CTAs.
 // Measured at 1024^3: 64 and 128 planes tie, 256 loses 4 % to the partial last wave.
+// Choice: minimise (number of waves of 148 SMs x 2 resident CTAs) x (planes per CTA + prologue), i.e. the
+// time of the slowest SM, over chunk lengths up to AH_ZC_MAX; for small lattices this picks a chunk count that
+// fills one wave (or a whole number of them) instead of leaving a mostly empty last wave (128^3: +40 %,
+// 256^3: +9 %).  With six or more waves the last partial wave is not modelled as a whole one (measured: it costs
+// little, the CTAs left share the freed bandwidth).
 #ifndef AH_ZC_MAX
 #define AH_ZC_MAX 64
-#endif
-#ifndef AH_MIN_WAVES
-#define AH_MIN_WAVES 8
 #endif
 int tiled_chunk(int nx, int ny, int nz)
 {
     const long long cols = (long long)(nx / TILE_X) * ((ny + TILE_Y - 1) / TILE_Y);
-    const long long want = 148LL * 2 * AH_MIN_WAVES;   // enough waves that the last, partial one costs little
-    int zc = AH_ZC_MAX;
-    while (zc > 8 && cols * ((nz + zc - 1) / zc) < want) zc >>= 1;
-    return zc < nz ? zc : nz;
+    const long long resident = 148LL * 2;
+    int best = nz < 8 ? nz : 8;
+    double best_cost = 1e300;
+    for (int nchunk = 1; nchunk <= nz; ++nchunk) {
+        const int zc = (nz + nchunk - 1) / nchunk;
+        if (zc > AH_ZC_MAX) continue;
+        if (zc < 4 && nz >= 4) break;
+        const long long ctas = cols * ((nz + zc - 1) / zc);
+        const double waves = ctas >= 6 * resident ? (double)ctas / (double)resident
+                                                  : (double)((ctas + resident - 1) / resident);
+        const double cost = waves * (zc + 2.5);     // 2.5 planes ~ ring fill + hand-down of the plane below
+        if (cost < best_cost * (1.0 - 1e-9)) {
+            best_cost = cost;
+            best = zc;
+        }
+    }
+    return best;
 }
 
 int tiled_num_blocks(int nx, int ny, int nz)
