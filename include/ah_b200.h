@@ -71,6 +71,8 @@ typedef struct {
     double sum_pi2_L, sum_grad2_L, sum_L, v2_phi; /* Eqs. 17-18                                      */
     double gauss_max, gauss_l2, gauss_rel;        /* Eq. 5 residual                                  */
     double gauss_div_l2, gauss_charge_l2;
+    double xi_l; /* Lagrangian estimator sqrt(-mu V / sum_x L_x dx^3), mu = 2 pi sigma^2 (Eq. 16 left,
+                    PAPER.md:102; reading #16); +inf when the sum is not negative                        */
 } ah_diag;
 
 /*

@@ -58,6 +58,7 @@ typedef struct {
     double sum_pi2_L, sum_grad2_L, sum_L, v2_phi;
     double gauss_max, gauss_l2, gauss_rel;
     double gauss_div_l2, gauss_charge_l2;
+    double xi_l;
 } ahref_diag;
 
 #define AHREF_PI 3.14159265358979323846264338327950288
@@ -439,6 +440,9 @@ int ahref_diagnostics(const ahref_params *P, const double *f10, double tau, doub
     out->sum_pi2_L = s_pi;
     out->sum_grad2_L = s_gr;
     out->sum_L = s_L;
+    /* Eq. 16 left: xi_L = sqrt(-mu V / integral of L), mu = 2 pi sigma^2 (beta = 1);
+     * V = N dx^3 and the integral is sum_x L_x dx^3, so the dx^3 cancel. */
+    out->xi_l = (s_L < 0.0) ? sqrt(-(2.0 * AHREF_PI * P->sigma * P->sigma) * ((double)nx * ny * nz) / s_L) : INFINITY;
     {
         const double R = s_pi / s_gr;
         out->v2_phi = (s_gr != 0.0) ? 2.0 * R / (1.0 + R) : 0.0;

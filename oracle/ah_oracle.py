@@ -44,6 +44,7 @@ class Diag(C.Structure):
         ("v2_phi", C.c_double),
         ("gauss_max", C.c_double), ("gauss_l2", C.c_double), ("gauss_rel", C.c_double),
         ("gauss_div_l2", C.c_double), ("gauss_charge_l2", C.c_double),
+        ("xi_l", C.c_double),
     ]
 
     def asdict(self):

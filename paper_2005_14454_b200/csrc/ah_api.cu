@@ -233,6 +233,11 @@ void finish_diag(const ah_ctx *c, const ah::DiagPartial &r, double tau, ah_diag 
     out->sum_pi2_L = r.f[ah::DF_SPI];
     out->sum_grad2_L = r.f[ah::DF_SGR];
     out->sum_L = r.f[ah::DF_SL];
+    {   // Eq. 16 left: xi_L = sqrt(-mu V / int L), int L = sum_x L_x dx^3, V = N dx^3, mu = 2 pi sigma^2
+        const double mu = 2.0 * 3.14159265358979323846 * P.sigma * P.sigma;
+        const double nsites = (double)P.nx * P.ny * P.nz;
+        out->xi_l = out->sum_L < 0.0 ? std::sqrt(-mu * nsites / out->sum_L) : std::numeric_limits<double>::infinity();
+    }
     if (out->sum_grad2_L != 0.0) {
         const double R = out->sum_pi2_L / out->sum_grad2_L;   // Eq. 18
         out->v2_phi = 2.0 * R / (1.0 + R);                    // Eq. 17 left

@@ -16,6 +16,9 @@ import sys
 import numpy as np
 
 
+KEYS = ("tau", "n_wind", "xi_w", "xi_l", "v2_phi", "gauss_rel", "sum_L")
+
+
 def main(argv=None):
     ap = argparse.ArgumentParser()
     ap.add_argument("--size", type=int, default=256)
@@ -46,15 +49,16 @@ def main(argv=None):
             n = min(chunk, steps - done)
             for r in sim.step_diag(n, tau0 + done * args.dt, args.dt, args.diag_every):
                 recs.append(r)
-                print(json.dumps({k: r[k] for k in ("tau", "n_wind", "xi_w", "v2_phi", "gauss_rel", "sum_L")}), flush=True)
+                print(json.dumps({k: r[k] for k in KEYS}), flush=True)
             done += n
         last = sim.diagnostics(tau_end, args.dt)
         recs.append(last)
-        print(json.dumps({k: last[k] for k in ("tau", "n_wind", "xi_w", "v2_phi", "gauss_rel", "sum_L")}), flush=True)
+        print(json.dumps({k: last[k] for k in KEYS}), flush=True)
 
     tau = np.array([r["tau"] for r in recs])
     xi = np.array([r["xi_w"] for r in recs])
     v2 = np.array([r["v2_phi"] for r in recs])
+    xl = np.array([r["xi_l"] for r in recs])
     lo = args.fit_from if args.fit_from is not None else tau0 + 0.4 * (tau_end - tau0)
     m = (tau >= lo) & np.isfinite(xi)
     summary = {"summary": True, "size": args.size, "era": args.era, "s": args.s, "steps": steps, "fit_from": lo}
@@ -63,6 +67,9 @@ def main(argv=None):
         # xi_w uses the raw plaquette count L_W = dx * n_W (reading #13).  Counting plaquettes
         # over-estimates the length of a smooth string by the Manhattan factor 6/pi (Hindmarsh et al. 2017, the
         # paper's reference for this estimator), i.e. xi by sqrt(pi/6); the corrected slope is printed beside it.
+        ml = m & np.isfinite(xl)
+        if ml.sum() >= 3:
+            summary.update(xi_l_slope=float(np.polyfit(tau[ml], xl[ml], 1)[0]))
         summary.update(xi_w_slope=float(slope), xi_w_intercept=float(icpt),
                        xi_w_slope_manhattan_corrected=float(slope * np.sqrt(6.0 / np.pi)),
                        v2_phi_mean=float(v2[m].mean()), v2_phi_std=float(v2[m].std()), n_fit=int(m.sum()))

@@ -306,6 +306,12 @@ def test_winding_bit_exact_on_snapshot(ah, oracle, model):
     assert d_gpu["n_big_plaq"] == d_or["n_big_plaq"] == 0
     assert abs(d_gpu["n_near_branch"] - d_or["n_near_branch"]) <= 2
     assert d_gpu["xi_w"] == pytest.approx(np.sqrt(48**3 * 0.5**3 / (0.5 * d_gpu["n_wind"])), rel=1e-14)
+    # Eq. 16 left from the returned sum (mu = 2 pi sigma^2), and against the oracle's own evaluation
+    if d_gpu["sum_L"] < 0:
+        assert d_gpu["xi_l"] == pytest.approx(np.sqrt(-2 * np.pi * 48**3 / d_gpu["sum_L"]), rel=1e-14)
+        assert d_gpu["xi_l"] == pytest.approx(d_or["xi_l"], rel=1e-5)
+    else:
+        assert np.isinf(d_gpu["xi_l"]) and np.isinf(d_or["xi_l"])
     sim.close()
 
 

@@ -139,6 +139,10 @@ def test_vortex_pair_static_and_tension(oracle):
     mu, Lz = 2 * np.pi, 0.5
     deficit_coarse = 1 - (-d["sum_L"] * 0.5**3) / (2 * mu * Lz)
     assert 0.005 < deficit_coarse < 0.02
+    # Eq. 16 left: xi_L = sqrt(-mu V / int L) must agree with the winding estimator for two straight strings of
+    # length Lz (the paper finds the two "fully consistent"), up to the same O(dx^2) deficit
+    assert d["xi_l"] == pytest.approx(np.sqrt(mu * 48 * 48 * 0.5**3 / (-d["sum_L"] * 0.5**3)), rel=1e-12)
+    assert d["xi_l"] == pytest.approx(d["xi_w"] * (1 + 0.5 * deficit_coarse), rel=1e-3)
     # energy from the independent numpy expression agrees
     assert indep.energy(f, 0.5, 2.0, 1.0, 1.0) == pytest.approx(-d["sum_L"] * 0.5**3, rel=1e-6)
     # stays static under undamped Minkowski evolution
