@@ -114,6 +114,14 @@ int ah_current_bufs(ah_ctx *ctx, void *dev_ptrs_out[AH_NFIELDS]);
  */
 int ah_step(ah_ctx *ctx, int n, double tau, double dt);
 
+/*
+ * ah_step_cooling — n leapfrog steps with a CONSTANT artificial damping delta on both Pi and ep and the couplings at
+ * their a = 1 values (the "artificial damping (cooling) period" of PAPER.md:63; used to relax initial conditions,
+ * e.g. onto a static string).  Identical to ah_step on a context with p = 1, s = 0, alpha = 2 called n times at the
+ * fixed time tau = dt / delta.  AH_EINVAL if n < 0, dt <= 0 or delta <= 0 or delta >= 1.
+ */
+int ah_step_cooling(ah_ctx *ctx, int n, double delta, double dt);
+
 /* Diagnostics D1-D3 of the current snapshot (fields at tau, momenta at tau - dt/2).
  * Synchronous: returns after the result is in *host_out. */
 int ah_diagnostics(ah_ctx *ctx, double tau, double dt, ah_diag *host_out);

@@ -29,7 +29,7 @@ FIELD_NAMES = ("phi_re", "phi_im", "pi_re", "pi_im", "th_x", "th_y", "th_z", "ep
 # every symbol include/ah_b200.h declares (checked by tests/test_abi.py)
 EXPORTS = (
     "ah_create", "ah_destroy", "ah_init_fields", "ah_set_fields", "ah_get_fields", "ah_current_bufs",
-    "ah_step", "ah_diagnostics", "ah_step_diag", "ah_winding_field", "ah_set_kernel", "ah_get_kernel",
+    "ah_step", "ah_step_cooling", "ah_diagnostics", "ah_step_diag", "ah_winding_field", "ah_set_kernel", "ah_get_kernel",
     "ah_launch_count", "ah_coeffs", "ah_test_trig", "ah_test_trig_fast", "ah_last_error", "ah_version",
 )
 
@@ -90,6 +90,7 @@ def lib():
     L.ah_get_fields.argtypes = [vp, vp]
     L.ah_current_bufs.argtypes = [vp, C.POINTER(vp)]
     L.ah_step.argtypes = [vp, ip, dp, dp]
+    L.ah_step_cooling.argtypes = [vp, ip, dp, dp]
     L.ah_diagnostics.argtypes = [vp, dp, dp, C.POINTER(Diag)]
     L.ah_step_diag.argtypes = [vp, ip, dp, dp, ip, C.POINTER(Diag), ip, C.POINTER(ip)]
     L.ah_winding_field.argtypes = [vp, vp, vp]
@@ -213,6 +214,10 @@ class Simulation:
     def step(self, n: int, tau: float, dt: float):
         with self._dev():
             _check(lib().ah_step(self._ctx, int(n), float(tau), float(dt)))
+
+    def step_cooling(self, n: int, delta: float, dt: float):
+        with self._dev():
+            _check(lib().ah_step_cooling(self._ctx, int(n), float(delta), float(dt)))
 
     def diagnostics(self, tau: float, dt: float) -> dict:
         d = Diag()

@@ -420,6 +420,24 @@ int ah_step(ah_ctx *c, int n, double tau, double dt)
     return AH_OK;
 }
 
+int ah_step_cooling(ah_ctx *c, int n, double delta, double dt)
+{
+    if (!c) return fail(AH_EINVAL, "ah_step_cooling: null context");
+    if (n < 0) return fail(AH_EINVAL, "ah_step_cooling: n must be >= 0 (got %d)", n);
+    if (!c->have_fields) return fail(AH_ESTATE, "ah_step_cooling: no fields were set");
+    if (!(dt > 0.0) || !std::isfinite(dt) || !(delta > 0.0) || !(delta < 1.0))
+        return fail(AH_EINVAL, "ah_step_cooling: need dt > 0 and 0 < delta < 1 (dt=%g, delta=%g)", dt, delta);
+    // constant damping = the Hubble term frozen at tau = dt/delta with p = 1, alpha = 2; s = 0 keeps q = 1
+    const ah_params saved = c->P;
+    c->P.p = 1.0;
+    c->P.s = 0.0;
+    c->P.alpha = 2.0;
+    int rc = AH_OK;
+    for (int j = 0; j < n && rc == AH_OK; ++j) rc = one_step(c, dt / delta, dt);
+    c->P = saved;
+    return rc;
+}
+
 int ah_diagnostics(ah_ctx *c, double tau, double dt, ah_diag *out)
 {
     if (!c || !out) return fail(AH_EINVAL, "ah_diagnostics: null pointer");

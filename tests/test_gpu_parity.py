@@ -315,6 +315,50 @@ def test_winding_bit_exact_on_snapshot(ah, oracle, model):
     sim.close()
 
 
+def test_static_vortex_pair_cooling_on_the_tiled_kernel(ah, oracle):
+    """north_star's static Nielsen-Olesen string on the CUDA path: a vortex-antivortex pair (a single winding cannot
+    live on a periodic lattice) relaxed with ah_step_cooling (the paper's artificial damping) on the
+    tiled kernel, against the oracle doing the same sequence; then evolved undamped in Minkowski space."""
+    nx, ny, dx = 128, 128, 0.5      # square: a flatter box puts a spurious second pair on the y seam
+    Pr = oracle.make_params(nx, ny, 1, dx=dx, p=1.0, s=0.0)          # the oracle's constant damping: tau = dt/delta
+    f = oracle.empty_fields(Pr)
+    y, x = np.meshgrid(np.arange(ny), np.arange(nx), indexing="ij")
+    c1, c2 = (nx / 4 + 0.5, ny / 2 + 0.5), (3 * nx / 4 + 0.5, ny / 2 + 0.5)
+    r1, r2 = np.hypot(x - c1[0], y - c1[1]) * dx, np.hypot(x - c2[0], y - c2[1]) * dx
+    a1, a2 = np.arctan2(y - c1[1], x - c1[0]), np.arctan2(y - c2[1], x - c2[0])
+    phi = np.tanh(r1 / 1.2) * np.tanh(r2 / 1.2) * np.exp(1j * (a1 - a2))
+    f[0, 0], f[1, 0] = phi.real, phi.imag
+    f = f.astype(np.float32).astype(np.float64)
+    dt, delta, nrelax = 0.1, 0.15, 1500
+    sim = ah.Simulation(params=ah.make_params(nx, ny, 1, dx=dx, p=0.0, s=0.0))   # Minkowski context
+    assert sim.get_kernel() == ah.KERNEL_TILED
+    sim.set_fields(f)
+    sim.step_cooling(nrelax, delta, dt)
+    for _ in range(nrelax):
+        oracle.step(Pr, f, 1, dt / delta, dt)
+    g = sim.get_fields()
+    r = rel_max(g, f)
+    # a contraction: fp32 errors do not grow (Pi, ep relax to the fp32 noise floor and are not compared)
+    assert r["phi"] <= 5e-5 and r["th"] <= 1e-4, r
+    d = sim.diagnostics(1.0, dt)
+    assert d["n_wind"] == 2 and d["n_wind_xy"] == 2 and d["n_near_branch"] == 0
+    w, _ = sim.winding_field()
+    assert sorted(w[0][w[0] != 0].tolist()) == [-1, 1] and not w[1].any() and not w[2].any()
+    # tension: -sum L dx^3 = 2 mu Lz (1 - O(dx^2)), mu = 2 pi sigma^2, Lz = dx; and xi_L ~ xi_W
+    deficit = 1 - (-d["sum_L"] * dx**3) / (2 * 2 * np.pi * dx)
+    assert 0.005 < deficit < 0.02, deficit
+    assert d["xi_l"] == pytest.approx(d["xi_w"] * (1 + 0.5 * deficit), rel=2e-3)
+    assert d["v2_phi"] < 1e-6
+    # static: 300 undamped Minkowski steps move nothing beyond the relaxation residual
+    eps = max(np.abs(g[2:4]).max(), np.abs(g[7:10]).max())
+    sim.step(300, 1.0, dt)
+    h = sim.get_fields()
+    assert np.abs(h[0:2] - g[0:2]).max() <= 10 * (delta / dt) * eps * (300 * dt) ** 2 + 2e-5
+    w2, _ = sim.winding_field()
+    assert np.array_equal(w, w2)
+    sim.close()
+
+
 def test_winding_with_exactly_zero_phi_sites(ah, oracle):
     """The library takes link phases as wrapped differences of site phases alpha = Arg(phi); a site with phi == 0
     has none, and the oracle's convention (Arg of a zero link product := 0) must still come out, on both kernels
