@@ -158,18 +158,19 @@ struct Smem {
 namespace {
 
 // Domain of this kernel: every |th_i| < AH_TILED_TH_LIMIT (2^16 rad), so that every plaquette angle is below
-// 2^18, where the two-term Cody-Waite reductions of sincos_poly_f32 / sin_poly_f32 still hold their 1e-7
+// 2^18, where the two-term Cody-Waite reductions of sincos_pi_f32 / sin_poly_f32 still hold their 1.5e-7
 // absolute accuracy (ah_common.cuh).  Each thread checks the 12 link angles it owns (every link of the
 // input state is owned by exactly one thread) and raises *overflow if one is outside; the API then
 // redoes the step with the libm-based site kernel (ah_api.cu: one_step).
 #define AH_TILED_TH_LIMIT 65536.0f
 
-//
 // DIAG = true (SURVEY 8(a) row D-fuse): the same step, plus the read-outs D1-D3 of the ENTRY snapshot of every
 // site, evaluated by diag_site() from what is already staged for the step (phi, th planes with their (+,+)
-// corners, the warp's Pi, ep row); the only extra global reads are the backward ep neighbours.  Per-thread
-// sums are reduced per CTA into partials[linear CTA index]; diag_final_kernel adds them in a fixed order.
-// Staged neighbours from shared memory for diag_site(): the site is column `ci` of staged row `r`
+// corners, the warp's Pi, ep row) and from the site phases alpha = Arg(phi), computed once per staged site into
+// sm.alpha; the only extra global reads are the backward ep neighbours.  Per-thread sums are reduced per CTA
+// into partials[linear CTA index]; diag_final_kernel adds them in a fixed order.
+//
+// Neighbours from shared memory for diag_site(): the site is column `ci` of staged row `r`
 template <int TY>
 struct StagedSiteAccessor {
     const Smem<TY, true> &sm;
@@ -208,10 +209,9 @@ tiled_step_kernel(ConstFields<float> in, Fields<float> out, StepCoef<float> k, i
     const bool is_main = w < TY;
 
     // ------------------------------------------------------------------ producers
-    // load n  <->  plane z0 - 1 + n (periodic), slot n % NST.  Every main warp copies its own staged row
-    // (lanes 0..4: one field each), the helper warp the two halo rows 0 and TY+1 (lanes 0..9) and arms
-    // the slot's mbarrier with the byte count of the whole plane.
-    // One elected lane per warp issues them, with warp-uniform operands (no per-lane serialisation).
+    // load n  <->  plane z0 - 1 + n (periodic), slot n % NST.  Every main warp copies its own staged row (one
+    // copy per field), the helper warp the two halo rows 0 and TY+1, and it arms the slot's mbarrier with the
+    // byte count of the whole plane.  One elected lane per warp issues them, with warp-uniform operands.
     const bool interior = (x0 > 0) && (x0 + TILE_X < nx);
     auto wrap_y = [&](int yy) {
         yy %= ny;
