@@ -148,6 +148,82 @@ __device__ __forceinline__ float sin_small_f32(float x)
     return fmaf(p * x2, x, x);
 }
 
+// ---- packed pairs (sm_100a fma.rn.f32x2 -> SASS FFMA2: two fp32 FMAs per issued instruction; each half is the
+// IEEE operation of the scalar code above, so results are bit-identical; constants are broadcast operands)
+typedef unsigned long long f32x2;
+__device__ __forceinline__ f32x2 pack2(float lo, float hi)
+{
+    f32x2 r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+    return r;
+}
+__device__ __forceinline__ void unpack2(f32x2 v, float &lo, float &hi)
+{
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
+}
+__device__ __forceinline__ f32x2 fma2(f32x2 a, f32x2 b, f32x2 c)
+{
+    f32x2 r;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c));
+    return r;
+}
+__device__ __forceinline__ f32x2 mul2(f32x2 a, f32x2 b)
+{
+    f32x2 r;
+    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+    return r;
+}
+__device__ __forceinline__ f32x2 add2(f32x2 a, f32x2 b)
+{
+    f32x2 r;
+    asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+    return r;
+}
+#define AH_C2(x) pack2((x), (x))
+
+// sincos_pi_f32 on two angles at once
+__device__ __forceinline__ void sincos_pi_f32x2(f32x2 x, f32x2 &s, f32x2 &c)
+{
+    const f32x2 t = fma2(x, AH_C2(0.31830987334251404f), AH_C2(12582912.0f));
+    const f32x2 k = add2(t, AH_C2(-12582912.0f));
+    f32x2 r = fma2(k, AH_C2(-3.1415927410125732f), x);
+    r = fma2(k, AH_C2(8.742277657347586e-08f), r);
+    const f32x2 r2 = mul2(r, r);
+    f32x2 ps = fma2(r2, AH_C2(2.5971810373448534e-06f), AH_C2(-0.00019805048941634595f));
+    ps = fma2(ps, r2, AH_C2(0.008332990109920502f));
+    ps = fma2(ps, r2, AH_C2(-0.16666655242443085f));
+    const f32x2 sr = fma2(mul2(ps, r2), r, r);
+    f32x2 pc = fma2(r2, AH_C2(-2.605479494377505e-07f), AH_C2(2.4762006432865746e-05f));
+    pc = fma2(pc, r2, AH_C2(-0.0013888449175283313f));
+    pc = fma2(pc, r2, AH_C2(0.04166664928197861f));
+    pc = fma2(pc, r2, AH_C2(-0.5f));
+    const f32x2 cr = fma2(pc, r2, AH_C2(1.0f));
+    const f32x2 sign = (t << 31) & 0x8000000080000000ull;     // (-1)^k of each half
+    s = sr ^ sign;
+    c = cr ^ sign;
+}
+// sin_small_f32 / sin_poly_f32 on two angles at once
+__device__ __forceinline__ f32x2 sin_small_f32x2(f32x2 x)
+{
+    const f32x2 x2 = mul2(x, x);
+    f32x2 p = fma2(x2, AH_C2(-1.9841270e-4f), AH_C2(8.3333333e-3f));
+    p = fma2(p, x2, AH_C2(-1.6666667e-1f));
+    return fma2(mul2(p, x2), x, x);
+}
+__device__ __forceinline__ f32x2 sin_poly_f32x2(f32x2 x)
+{
+    const f32x2 t = fma2(x, AH_C2(0.31830987334251404f), AH_C2(12582912.0f));
+    const f32x2 k = add2(t, AH_C2(-12582912.0f));
+    f32x2 r = fma2(k, AH_C2(-3.1415927410125732f), x);
+    r = fma2(k, AH_C2(8.742277657347586e-08f), r);
+    const f32x2 r2 = mul2(r, r);
+    f32x2 ps = fma2(r2, AH_C2(2.5971810373448534e-06f), AH_C2(-0.00019805048941634595f));
+    ps = fma2(ps, r2, AH_C2(0.008332990109920502f));
+    ps = fma2(ps, r2, AH_C2(-0.16666655242443085f));
+    const f32x2 sr = fma2(mul2(ps, r2), r, r);
+    return sr ^ ((t << 31) & 0x8000000080000000ull);
+}
+
 // libm slow paths kept out of line: the hot loops stay small enough for the 32 KB instruction cache
 static __device__ __noinline__ void sincos_slow_f32(float th, float *s, float *c) { sincosf(th, s, c); }
 static __device__ __noinline__ float sin_slow_f32(float x) { return sinf(x); }

@@ -497,23 +497,37 @@ tiled_step_kernel(ConstFields<float> in, Fields<float> out, StepCoef<float> k, i
                 amax = fmaxf(amax, fmaxf(fmaxf(fabsf(S_xy.v[j]), fabsf(S_xz.v[j])), fabsf(S_yz.v[j])));
             }
             if (COMPACT) {
+                // two angles per issued instruction (FFMA2); bit-identical to the scalar polynomials
+                auto sines = [&](V4 &a, bool small) {
+#pragma unroll
+                    for (int h = 0; h < 4; h += 2) {
+                        const f32x2 x = pack2(a.v[h], a.v[h + 1]);
+                        unpack2(small ? sin_small_f32x2(x) : sin_poly_f32x2(x), a.v[h], a.v[h + 1]);
+                    }
+                };
                 if (__all_sync(FULL, amax < AH_SMALL_ANGLE)) {
-#pragma unroll
-                    for (int j = 0; j < 4; ++j) {
-                        S_xy.v[j] = sin_small_f32(S_xy.v[j]);
-                        S_xz.v[j] = sin_small_f32(S_xz.v[j]);
-                        S_yz.v[j] = sin_small_f32(S_yz.v[j]);
-                    }
+                    sines(S_xy, true); sines(S_xz, true); sines(S_yz, true);
                 } else {
-#pragma unroll
-                    for (int j = 0; j < 4; ++j) {
-                        S_xy.v[j] = sin_poly_f32(S_xy.v[j]);
-                        S_xz.v[j] = sin_poly_f32(S_xz.v[j]);
-                        S_yz.v[j] = sin_poly_f32(S_yz.v[j]);
-                    }
+                    sines(S_xy, false); sines(S_xz, false); sines(S_yz, false);
                 }
             }
 
+            // link variables of the 4 sites (Eq. 12), two angles per issued instruction
+            V4 s_x, c_x, s_y, c_y, s_z, c_z;
+            {
+                auto sincos4 = [&](const V4 &t, V4 &sn, V4 &cs) {
+#pragma unroll
+                    for (int h = 0; h < 4; h += 2) {
+                        f32x2 s2, c2;
+                        sincos_pi_f32x2(pack2(t.v[h], t.v[h + 1]), s2, c2);
+                        unpack2(s2, sn.v[h], sn.v[h + 1]);
+                        unpack2(c2, cs.v[h], cs.v[h + 1]);
+                    }
+                };
+                sincos4(c_tx, s_x, c_x);
+                sincos4(c_ty, s_y, c_y);
+                sincos4(c_tz, s_z, c_z);
+            }
 #pragma unroll
             for (int j = 0; j < 4; ++j) {
                 const float fr = c_pr.v[j], fi = c_pi.v[j];
@@ -521,10 +535,7 @@ tiled_step_kernel(ConstFields<float> in, Fields<float> out, StepCoef<float> k, i
                 const int jn = (j < 3) ? j + 1 : 3;
                 const float xr = (j < 3) ? c_pr.v[jn] : r_pr, xi = (j < 3) ? c_pi.v[jn] : r_pi;
                 const float Sxy = S_xy.v[j], Sxz = S_xz.v[j], Syz = S_yz.v[j];
-                float sx, cx, sy, cy, sz, cz;
-                sincos_pi_f32(tx, sx, cx);          // Eq. 12
-                sincos_pi_f32(ty, sy, cy);
-                sincos_pi_f32(tz, sz, cz);
+                const float sx = s_x.v[j], cx = c_x.v[j], sy = s_y.v[j], cy = c_y.v[j], sz = s_z.v[j], cz = c_z.v[j];
                 // forward hops U_i(s) phi(s+i)                                   (Eq. 13)
                 const float fxr = cx * xr + sx * xi, fxi = cx * xi - sx * xr;
                 const float fyr = cy * y_pr.v[j] + sy * y_pi.v[j], fyi = cy * y_pi.v[j] - sy * y_pr.v[j];
