@@ -43,13 +43,6 @@ struct V4 {
     float v[4];
 };
 
-__device__ __forceinline__ V4 ld4(const float *__restrict__ p)
-{
-    const float4 t = __ldg(reinterpret_cast<const float4 *>(p));
-    V4 r;
-    r.v[0] = t.x; r.v[1] = t.y; r.v[2] = t.z; r.v[3] = t.w;
-    return r;
-}
 __device__ __forceinline__ V4 lds4(const float *p)
 {
     const float4 t = *reinterpret_cast<const float4 *>(p);
