@@ -146,6 +146,10 @@ int ah_set_kernel(ah_ctx *ctx, int kernel);
  * AH_EINVAL for a null context. */
 int ah_get_kernel(const ah_ctx *ctx);
 
+/* Launch geometry the tiled kernel would use for a lattice (host logic only, no device needed; for tests and
+ * reports): planes per CTA and number of CTAs.  Returns AH_EINVAL when the lattice does not allow the tiled kernel. */
+int ah_tiled_launch_info(int nx, int ny, int nz, int *planes_per_cta, int *n_ctas);
+
 /* Number of kernel launches this context has enqueued since creation (bench.py's gpu_launches). */
 int64_t ah_launch_count(const ah_ctx *ctx);
 

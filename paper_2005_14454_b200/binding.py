@@ -30,7 +30,7 @@ FIELD_NAMES = ("phi_re", "phi_im", "pi_re", "pi_im", "th_x", "th_y", "th_z", "ep
 EXPORTS = (
     "ah_create", "ah_destroy", "ah_init_fields", "ah_set_fields", "ah_get_fields", "ah_current_bufs",
     "ah_step", "ah_step_cooling", "ah_diagnostics", "ah_step_diag", "ah_winding_field", "ah_set_kernel", "ah_get_kernel",
-    "ah_launch_count", "ah_coeffs", "ah_test_trig", "ah_test_trig_fast", "ah_last_error", "ah_version",
+    "ah_launch_count", "ah_tiled_launch_info", "ah_coeffs", "ah_test_trig", "ah_test_trig_fast", "ah_last_error", "ah_version",
 )
 
 
@@ -97,6 +97,7 @@ def lib():
     L.ah_set_kernel.argtypes = [vp, ip]
     L.ah_get_kernel.argtypes = [vp]
     L.ah_launch_count.argtypes = [vp]
+    L.ah_tiled_launch_info.argtypes = [ip, ip, ip, C.POINTER(ip), C.POINTER(ip)]
     L.ah_launch_count.restype = C.c_int64
     L.ah_coeffs.argtypes = [C.POINTER(Params), dp, dp] + [C.POINTER(dp)] * 4
     L.ah_test_trig.argtypes = [vp, vp, vp, vp, C.c_size_t, vp]
@@ -119,6 +120,13 @@ def make_params(nx, ny=None, nz=None, dx=0.5, lambda0=2.0, e0=1.0, sigma=1.0, s=
     nz = nx if nz is None else nz
     return Params(int(nx), int(ny), int(nz), float(dx), float(lambda0), float(e0), float(sigma),
                   float(s), float(p), float(tau_ref), float(alpha), int(compact), int(bool(fp64)))
+
+
+def tiled_launch_info(nx, ny, nz):
+    """(planes per CTA, number of CTAs) of the tiled kernel for this lattice; host logic, no device needed."""
+    zc, n = C.c_int(0), C.c_int(0)
+    _check(lib().ah_tiled_launch_info(int(nx), int(ny), int(nz), C.byref(zc), C.byref(n)))
+    return zc.value, n.value
 
 
 def coeffs(P: Params, tau: float, dt: float):

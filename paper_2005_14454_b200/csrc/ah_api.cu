@@ -361,6 +361,15 @@ int ah_get_kernel(const ah_ctx *c)
     return c->P.fp64 ? AH_KERNEL_SITE : c->kernel;
 }
 
+int ah_tiled_launch_info(int nx, int ny, int nz, int *planes_per_cta, int *n_ctas)
+{
+    if (!planes_per_cta || !n_ctas) return fail(AH_EINVAL, "ah_tiled_launch_info: null pointer");
+    if (!ah::tiled_supported(nx, ny, nz)) return fail(AH_EINVAL, "ah_tiled_launch_info: tiled kernel needs nx %% 128 == 0");
+    *planes_per_cta = ah::tiled_chunk(nx, ny, nz);
+    *n_ctas = ah::tiled_num_blocks(nx, ny, nz);
+    return AH_OK;
+}
+
 int64_t ah_launch_count(const ah_ctx *c) { return c ? c->launches : 0; }
 
 int ah_init_fields(ah_ctx *c, uint64_t seed)

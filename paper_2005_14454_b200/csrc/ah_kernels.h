@@ -26,6 +26,7 @@ cudaError_t launch_tiled_step(const ConstFields<float> &in, const Fields<float> 
                               const StepCoef<float> &k, int nx, int ny, int nz, int *overflow, cudaStream_t st,
                               const DiagCoef *dk = nullptr, DiagPartial *partials = nullptr);
 int tiled_num_blocks(int nx, int ny, int nz);
+int tiled_chunk(int nx, int ny, int nz);   // z planes per CTA
 // after a tiled step: redo it with the site kernel iff *flag != 0; clears *clear (the next step's flag)
 cudaError_t launch_site_redo(const int *flag, int *clear, const ConstFields<float> &in, const Fields<float> &out,
                              const StepCoef<float> &k, int nx, int ny, int nz, cudaStream_t st);

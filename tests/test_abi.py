@@ -47,6 +47,29 @@ def test_struct_layouts_match_header(ahlib):
     assert C.sizeof(ahlib.Diag) == 8 * 19
 
 
+def test_tiled_launch_geometry(ahlib):
+    """Host logic of the tiled kernel's launch: the z extent is covered, chunks are at most 64 planes, small
+    lattices fill whole waves of 148 SMs x 2 resident CTAs, and unsupported lattices are refused."""
+    resident = 148 * 2
+    for n in (128, 256, 384, 512, 768, 1024):
+        zc, ctas = ahlib.tiled_launch_info(n, n, n)
+        cols = (n // 128) * -(-n // 6)
+        assert 1 <= zc <= 64 and ctas == cols * -(-n // zc)
+        if ctas < 6 * resident:                       # few waves: the last one must not be mostly empty
+            waves = -(-ctas // resident)
+            assert ctas / (waves * resident) >= 0.85, (n, zc, ctas)
+    assert ahlib.tiled_launch_info(128, 128, 128) == (10, 286)      # one wave
+    assert ahlib.tiled_launch_info(1024, 1024, 1024)[0] == 64
+    zc, ctas = ahlib.tiled_launch_info(128, 1, 1)
+    assert (zc, ctas) == (1, 1)
+    zc, ctas = ahlib.tiled_launch_info(256, 16, 11)
+    assert zc * -(-11 // zc) >= 11 and ctas == 2 * 3 * -(-11 // zc)
+    with pytest.raises(ahlib.AhError):
+        ahlib.tiled_launch_info(64, 64, 64)
+    with pytest.raises(ahlib.AhError):
+        ahlib.tiled_launch_info(200, 8, 8)
+
+
 def test_coeffs_closed_forms(ahlib):
     """delta = (alpha/2) p dt/tau, omega = (1-s) delta, a = (tau/tau_ref)^p, q = a^{2s}."""
     P = ahlib.make_params(8, s=1.0, p=2.0, tau_ref=129.0, alpha=2.0)
