@@ -595,8 +595,6 @@ tiled_step_kernel(ConstFields<float> in, Fields<float> out, StepCoef<float> k, i
             const V4 q_r = lds4(&sm.qe[w][0][4 * lane]), q_i = lds4(&sm.qe[w][1][4 * lane]);
             const V4 e_x = lds4(&sm.qe[w][2][4 * lane]), e_y = lds4(&sm.qe[w][3][4 * lane]);
             const V4 e_z = lds4(&sm.qe[w][4][4 * lane]);
-            __syncwarp();
-            if (n + 1 <= nplanes) produce_q();
             V4 f_r, f_i, t_x, t_y, t_z;
 #pragma unroll
             for (int j = 0; j < 4; ++j) {
@@ -611,6 +609,10 @@ tiled_step_kernel(ConstFields<float> in, Fields<float> out, StepCoef<float> k, i
                 t_y.v[j] = c_ty.v[j] + k.dt * E_y.v[j];
                 t_z.v[j] = c_tz.v[j] + k.dt * E_z.v[j];
             }
+            // the staged Pi, ep row has been consumed (its values went through the arithmetic above): refill it
+            // with the next plane's row, which then has almost a whole iteration to land
+            __syncwarp();
+            if (n + 1 <= nplanes) produce_q();
             st4(out.f[PI_RE] + oc, P_r);
             st4(out.f[PI_IM] + oc, P_i);
             st4(out.f[EP_X] + oc, E_x);
