@@ -14,10 +14,12 @@
  * Pins (tests/test_oracle_*.py): Gauss law to round-off, gauge covariance,
  * plane-wave dispersion (closed form), Minkowski energy conservation with an
  * energy written independently in numpy, vortex-antivortex pair (static,
- * mu = 2 pi sigma^2), brute-force winding, naive numpy <v^2> sums, splitmix
- * known answers.  Parity-unpinned items (stated in DESIGN.md): the
- * normalisation a(tau_ref) = 1 and the tau grid (the paper fixes neither), and
- * <v^2>_phi beyond its static limit and the naive re-evaluation.
+ * mu = 2 pi sigma^2), brute-force winding (including |Phi_ij| > pi, where the
+ * un-wrapped plaquette angle decides the integer), closed forms of L_x and
+ * <v^2>_phi on uniform states (kinetic, electric, potential, gradient and
+ * magnetic terms each fixed by arithmetic) besides the naive numpy <v^2> sums,
+ * splitmix known answers.  Parity-unpinned items (stated in DESIGN.md): the
+ * normalisation a(tau_ref) = 1 and the tau grid (the paper fixes neither).
  *
  * Conventions:
  *   site x = (x,y,z), linear index x + nx*(y + ny*z), periodic in all three;

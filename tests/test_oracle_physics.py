@@ -9,7 +9,9 @@
    energy -> 2 mu L_z with mu = 2 pi sigma^2 at O(dx^2), <v^2> = 0.
  * Winding (Eq. 16): brute-force integer formulation, flux
    conservation, zero net flux through periodic planes, 1/3 density for random phases.
- * Lagrangian-weighted sums (Eqs. 17-18): naive numpy evaluation.
+ * Lagrangian-weighted sums (Eqs. 17-18): naive numpy evaluation, and CLOSED FORMS on
+   uniform states (every |Pi|^2, ep^2, potential, gradient and plaquette term of L_x fixed by arithmetic,
+   <v^2>_phi = 2R/(1+R) away from its static limit).
 """
 import numpy as np
 import pytest
@@ -183,6 +185,35 @@ def test_winding_bruteforce(oracle, shape):
         assert (d["n_wind_xy"], d["n_wind_xz"], d["n_wind_yz"]) == tuple(np.abs(wb[k]).sum() for k in range(3))
 
 
+@pytest.mark.parametrize("shape", [(4, 4, 4), (6, 5, 4), (8, 8, 8)])
+def test_winding_bruteforce_large_plaquette_angles(oracle, shape):
+    """Reading #13 (un-wrapped Phi_ij in Eq. 16 right): with link angles of order 1.5 rad many
+    plaquettes have |Phi| > pi, where the `+ Phi` term decides the integer.  The brute-force formulation never
+    forms Phi at all (pure integer link shifts), so dropping or wrapping the term in the oracle fails here."""
+    o = oracle
+    nx, ny, nz = shape
+    P = o.make_params(nx, ny, nz)
+    n_big = 0
+    for seed in range(3):
+        f = inputs.random_state(nx, ny, nz, seed=300 + seed, th_amp=1.6, round_to_f32=False)
+        th = [f[4], f[5], f[6]]
+        Phi = np.stack([indep.plaquette(th, i, j) for i, j in ((0, 1), (0, 2), (1, 2))])
+        big = np.abs(Phi) > np.pi
+        assert big.sum() > 0.1 * big.size          # the branch is really exercised
+        w, near = o.winding(P, f)
+        wb = indep.winding_bruteforce(f)
+        ok = near == 0
+        assert np.array_equal(w.astype(np.int64)[ok], wb[ok])
+        assert ok.mean() > 0.999
+        # the term matters: without it the integers differ on the big plaquettes
+        assert np.abs(wb[big & ok]).sum() > 0
+        d = o.diagnostics(P, f, 1.0, 0.1)
+        assert d["n_big_plaq"] == (np.abs(Phi) > np.pi - 1e-5).sum()
+        assert abs(d["n_wind"] - np.abs(wb).sum()) <= (~ok).sum()
+        n_big += int(big.sum())
+    assert n_big > 0
+
+
 def test_winding_flux_conservation_and_planes(oracle):
     o = oracle
     n = 16
@@ -247,3 +278,83 @@ def test_lagrangian_sums_naive(oracle, case):
     assert d["gauss_l2"] == pytest.approx(np.sqrt((G**2).sum()), rel=1e-12)
     assert d["gauss_rel"] == pytest.approx(
         np.sqrt((G**2).sum()) / (np.sqrt((div**2).sum()) + np.sqrt((ch**2).sum())), rel=1e-12)
+
+
+# ------------------------------------------------- closed forms for the Lagrangian density (reading #15)
+
+UNIFORM_MODELS = [dict(p=1.0, s=1.0, tau_ref=3.0), dict(p=2.0, s=0.5, tau_ref=2.0), dict(p=0.0, s=0.0)]
+
+
+@pytest.mark.parametrize("model", UNIFORM_MODELS)
+def test_lagrangian_closed_form_uniform_state(oracle, model):
+    """phi = rho e^{i beta}, th_i = t_i, Pi = c, ep_i = e_i, all uniform in space (Eqs. 17-18):
+    every plaquette angle vanishes, U_i phi(x+i) - phi = (e^{-i t_i} - 1) phi, so per site
+
+        |Pi|^2 = |c|^2,   sum_i |D_i phi|^2 = sum_i 2 (1 - cos t_i) rho^2 / dx^2,
+        L = |c|^2 - sum_i|D_i phi|^2 - (lambda0 q / 4)(rho^2 - sigma^2)^2 + sum_i e_i^2 / (2 e0^2 q dx^2),
+
+    with q = a^{2s} != 1.  Pins sign and factor of the kinetic, electric, potential and gradient terms and
+    <v^2>_phi = 2R/(1+R), R = |c|^2 / sum_i|D_i phi|^2, away from the static limit."""
+    o = oracle
+    nx, ny, nz = 5, 4, 3
+    dx, lam, e0, sig = 0.5, 1.7, 0.8, 1.1
+    P = o.make_params(nx, ny, nz, dx=dx, lambda0=lam, e0=e0, sigma=sig, **model)
+    tau, dt = 1.7, 0.1
+    _, q, _, _ = o.coeffs(P, tau, dt)
+    if model["s"] != 0.0:
+        assert abs(q - 1.0) > 0.1
+    rho, beta = 0.9, 0.4
+    t = (0.3, -0.7, 1.9)
+    c = 0.35 - 0.2j
+    e = (0.21, -0.4, 0.13)
+    f = o.empty_fields(P)
+    f[0], f[1] = rho * np.cos(beta), rho * np.sin(beta)
+    f[2], f[3] = c.real, c.imag
+    for i in range(3):
+        f[4 + i] = t[i]
+        f[7 + i] = e[i]
+    N = nx * ny * nz
+    pi2 = abs(c) ** 2
+    grad2 = sum(2.0 * (1.0 - np.cos(ti)) * rho**2 for ti in t) / dx**2
+    L = pi2 - grad2 - 0.25 * lam * q * (rho**2 - sig**2) ** 2 + sum(ei**2 for ei in e) / (2.0 * e0**2 * q * dx**2)
+    d = o.diagnostics(P, f, tau, dt)
+    assert d["sum_L"] == pytest.approx(N * L, rel=1e-12)
+    assert d["sum_pi2_L"] == pytest.approx(N * pi2 * L, rel=1e-12)
+    assert d["sum_grad2_L"] == pytest.approx(N * grad2 * L, rel=1e-12)
+    R = pi2 / grad2
+    assert d["v2_phi"] == pytest.approx(2 * R / (1 + R), rel=1e-12)
+    assert d["n_wind"] == 0 and d["n_big_plaq"] == 0
+    # the electric and kinetic terms enter with a PLUS sign: L grows with |c| and with |e|
+    g = f.copy()
+    g[2:4] *= 2.0
+    assert o.diagnostics(P, g, tau, dt)["sum_L"] == pytest.approx(N * (L + 3.0 * pi2), rel=1e-12)
+    g = f.copy()
+    g[7:10] *= 2.0
+    assert o.diagnostics(P, g, tau, dt)["sum_L"] == pytest.approx(
+        N * (L + 3.0 * sum(ei**2 for ei in e) / (2.0 * e0**2 * q * dx**2)), rel=1e-12)
+
+
+@pytest.mark.parametrize("compact", [1, 0])
+def test_lagrangian_closed_form_uniform_magnetic_field(oracle, compact):
+    """th_x = B*y on the vacuum phi = sigma, Pi = ep = 0: Phi_xy = th_x(y) - th_x(y+1) = -B on every plaquette
+    except the periodic seam y = ny-1, where it is +B(ny-1); Phi_xz = Phi_yz = 0.  The magnetic energy
+    2(1 - cos Phi)/dx^4 (compact; Phi^2/dx^4 non-compact, reading #10) enters L with a MINUS sign and the factor
+    1/(2 e0^2 q); the gradient term is 2(1 - cos(B y)) sigma^2/dx^2 on the x links."""
+    o = oracle
+    nx, ny, nz = 4, 6, 3
+    dx, lam, e0, sig = 0.5, 2.0, 0.8, 1.0
+    P = o.make_params(nx, ny, nz, dx=dx, lambda0=lam, e0=e0, sigma=sig, p=1.0, s=1.0, tau_ref=2.5, compact=compact)
+    tau, dt = 1.3, 0.1
+    _, q, _, _ = o.coeffs(P, tau, dt)
+    B = 0.37
+    f = o.empty_fields(P)
+    f[0] = sig
+    f[4] = B * np.arange(ny)[None, :, None]
+    en = (lambda ph: 2.0 * (1.0 - np.cos(ph))) if compact else (lambda ph: ph * ph)
+    b2_rows = np.array([en(-B)] * (ny - 1) + [en(B * (ny - 1))]) / dx**4
+    g2_rows = 2.0 * (1.0 - np.cos(B * np.arange(ny))) * sig**2 / dx**2
+    L_rows = -g2_rows - b2_rows / (2.0 * e0**2 * q)
+    d = o.diagnostics(P, f, tau, dt)
+    assert d["sum_L"] == pytest.approx(nx * nz * L_rows.sum(), rel=1e-12)
+    assert d["sum_grad2_L"] == pytest.approx(nx * nz * (g2_rows * L_rows).sum(), rel=1e-12)
+    assert d["sum_pi2_L"] == 0.0 and d["v2_phi"] == 0.0
