@@ -23,6 +23,8 @@
  *     calling thread's most recent failure.
  *   - Nothing here falls back to the CPU: without a CUDA device every compute
  *     entry point returns AH_ECUDA.
+ *   - Test and measurement hooks (kernel selection, launch counters, launch geometry, the device trig
+ *     evaluators) are NOT part of this interface: they live in ah_b200_test.h.
  */
 #ifndef AH_B200_H
 #define AH_B200_H
@@ -40,11 +42,6 @@ extern "C" {
 #define AH_ESTATE (-3) /* call made in the wrong state (e.g. stepping before any fields)  */
 
 #define AH_NFIELDS 10
-
-/* kernel selection for ah_set_kernel */
-#define AH_KERNEL_AUTO 0  /* fused tiled kernel when the lattice allows it, else the site kernel */
-#define AH_KERNEL_SITE 1  /* one thread per site, neighbours through L1/L2 (any nx,ny,nz >= 1) */
-#define AH_KERNEL_TILED 2 /* z-marching register/shared-memory tiled kernel (needs nx % 128 == 0) */
 
 typedef struct ah_ctx ah_ctx; /* opaque */
 
@@ -118,12 +115,14 @@ int ah_step(ah_ctx *ctx, int n, double tau, double dt);
  * ah_step_cooling — n leapfrog steps with a CONSTANT artificial damping delta on both Pi and ep and the couplings at
  * their a = 1 values (the "artificial damping (cooling) period" of PAPER.md:63; used to relax initial conditions,
  * e.g. onto a static string).  Identical to ah_step on a context with p = 1, s = 0, alpha = 2 called n times at the
- * fixed time tau = dt / delta.  AH_EINVAL if n < 0, dt <= 0 or delta <= 0 or delta >= 1.
+ * fixed time tau = dt / delta; the context's own parameters are not modified (re-entrant with respect to
+ * them).  AH_EINVAL if n < 0, dt <= 0 or delta <= 0 or delta >= 1.
  */
 int ah_step_cooling(ah_ctx *ctx, int n, double delta, double dt);
 
 /* Diagnostics D1-D3 of the current snapshot (fields at tau, momenta at tau - dt/2).
- * Synchronous: returns after the result is in *host_out. */
+ * Synchronous: returns after the result is in *host_out.  AH_EINVAL when omega = (1-s) delta = 1 at tau
+ * (the Gauss coefficient kappa = q (1-delta)/(1-omega) of DESIGN.md reading #18 does not exist there). */
 int ah_diagnostics(ah_ctx *ctx, double tau, double dt, ah_diag *host_out);
 
 /*
@@ -139,34 +138,9 @@ int ah_step_diag(ah_ctx *ctx, int n, double tau, double dt, int every, ah_diag *
  * of nx*ny*nz int8; host_near3 (may be NULL) the near-branch flags as uint8.  Synchronous. */
 int ah_winding_field(ah_ctx *ctx, int8_t *host_w3, uint8_t *host_near3);
 
-/* Choose the step kernel (AH_KERNEL_*).  AH_EINVAL if the lattice does not allow it. */
-int ah_set_kernel(ah_ctx *ctx, int kernel);
-
-/* The step kernel the context currently launches: AH_KERNEL_SITE or AH_KERNEL_TILED (never AUTO);
- * AH_EINVAL for a null context. */
-int ah_get_kernel(const ah_ctx *ctx);
-
-/* Launch geometry the tiled kernel would use for a lattice (host logic only, no device needed; for tests and
- * reports): planes per CTA and number of CTAs.  Returns AH_EINVAL when the lattice does not allow the tiled kernel. */
-int ah_tiled_launch_info(int nx, int ny, int nz, int *planes_per_cta, int *n_ctas);
-
-/* Number of kernel launches this context has enqueued since creation (bench.py's gpu_launches). */
-int64_t ah_launch_count(const ah_ctx *ctx);
-
 /* Host-side coefficients as the kernels receive them (for tests): a, q = a^{2s}, delta, omega. */
 int ah_coeffs(const ah_params *params, double tau, double dt, double *a, double *q, double *delta,
               double *omega);
-
-/* Device-side evaluation of the library's fp32 sin/cos kernels' math (tests only): for each of the
- * n device floats in dev_x writes sin and cos as used for link variables, and the plaquette sine. */
-int ah_test_trig(const float *dev_x, float *dev_sin, float *dev_cos, float *dev_plaq_sin, size_t n,
-                 void *cuda_stream);
-
-/* Same for the tiled step kernel's own trigonometry (tests only): sin/cos of the pi-reduced polynomial pair it
- * uses for link variables (valid for |x| < 2^18; the kernel's domain is |th| < 2^16) and the un-reduced Taylor
- * sine it uses for plaquette angles when a whole warp has |Phi| < 0.5 (dev_small_sin; meaningful for |x| < 0.5). */
-int ah_test_trig_fast(const float *dev_x, float *dev_sin, float *dev_cos, float *dev_small_sin, size_t n,
-                      void *cuda_stream);
 
 /* Message for the calling thread's most recent error ("" if none).  Never NULL. */
 const char *ah_last_error(void);

@@ -17,7 +17,7 @@ PKG = Path(__file__).resolve().parent
 CSRC = PKG / "csrc"
 LIB = PKG / "libah_b200.so"
 SOURCES = ["ah_api.cu", "ah_site_kernel.cu", "ah_tiled_kernel.cu", "ah_diag_kernel.cu"]
-HEADERS = ["ah_common.cuh", "ah_diag_site.cuh", "ah_kernels.h", "../../include/ah_b200.h"]
+HEADERS = ["ah_common.cuh", "ah_diag_site.cuh", "ah_kernels.h", "../../include/ah_b200.h", "../../include/ah_b200_test.h"]
 
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",

@@ -1,6 +1,7 @@
 // ah_api.cu — the C ABI of include/ah_b200.h: argument checking, per-step coefficients on the
 // host in fp64, kernel launches on the caller's stream.  No field arithmetic happens here.
 #include "../../include/ah_b200.h"
+#include "../../include/ah_b200_test.h"
 
 #include <cmath>
 #include <cstdarg>
@@ -75,7 +76,9 @@ ah::DiagCoef make_diag_coef(const ah_params &P, double tau, double dt)
     k.quarter_lam_q = 0.25 * P.lambda0 * q;
     k.sig2 = P.sigma * P.sigma;
     k.inv_2e2q = 1.0 / (2.0 * P.e0 * P.e0 * q);
-    k.two_e2_kappa = 2.0 * P.e0 * P.e0 * q * (1.0 - d) / (1.0 - w);  // reading #18
+    // reading #18; omega == 1 (the momentum half step would sit on the damping pole) has no Gauss coefficient:
+    // callers check it (ah_diagnostics returns AH_EINVAL); 0 keeps the kernel's sums finite
+    k.two_e2_kappa = (w == 1.0) ? 0.0 : 2.0 * P.e0 * P.e0 * q * (1.0 - d) / (1.0 - w);
     k.compact = P.compact;
     return k;
 }
@@ -135,14 +138,18 @@ int check_time(const ah_ctx *c, double tau, double dt)
 }
 
 // diag_slot >= 0 (tiled fp32 kernel only): the fused DIAG instantiation also leaves the read-outs of the entry
-// snapshot in d_results[diag_slot] (SURVEY 8(a) row D-fuse)
-int one_step(ah_ctx *c, double tau, double dt, int diag_slot = -1)
+// snapshot in d_results[diag_slot] (SURVEY 8(a) row D-fuse).
+// Context state (ping-pong parity, flag parity, launch count) changes only after EVERY launch of the step was
+// accepted; a failed launch leaves the context on the entry snapshot with both overflow flags cleared.
+// P: the model the step uses (the context's own, or ah_step_cooling's constant-damping copy of it)
+int one_step(ah_ctx *c, const ah_params &P, double tau, double dt, int diag_slot = -1)
 {
     cudaError_t e;
-    const ah_params &P = c->P;
+    int n_launched = 0;
     if (P.fp64) {
         e = ah::launch_site_step<double>(cur_fields<double>(c), next_fields<double>(c),
                                          make_coef<double>(P, tau, dt), P.nx, P.ny, P.nz, c->st);
+        n_launched = 1;
     } else if (c->kernel == AH_KERNEL_TILED) {
         // fast path, then a conditional redo with the libm-based site kernel (runs only if the fast
         // path flagged a link angle beyond its polynomial range; two flags alternate between steps)
@@ -152,24 +159,32 @@ int one_step(ah_ctx *c, double tau, double dt, int diag_slot = -1)
             const ah::DiagCoef dk = make_diag_coef(P, tau, dt);
             e = ah::launch_tiled_step(cur_fields<float>(c), next_fields<float>(c), k, P.nx, P.ny, P.nz, flag, c->st,
                                       &dk, c->d_partials);
-            if (e == cudaSuccess)
+            if (e == cudaSuccess) {
+                ++n_launched;
                 e = ah::launch_diag_final(c->d_partials, ah::tiled_num_blocks(P.nx, P.ny, P.nz),
                                           c->d_results + diag_slot, c->st);
-            c->launches += 1;
+            }
         } else {
             e = ah::launch_tiled_step(cur_fields<float>(c), next_fields<float>(c), k, P.nx, P.ny, P.nz, flag, c->st);
         }
-        if (e == cudaSuccess)
+        if (e == cudaSuccess) {
+            ++n_launched;
             e = ah::launch_site_redo(flag, next_flag, cur_fields<float>(c), next_fields<float>(c), k, P.nx, P.ny,
                                      P.nz, c->st);
-        c->step_parity = 1 - c->step_parity;
-        c->launches += 1;
+        }
+        if (e == cudaSuccess) {
+            ++n_launched;
+            c->step_parity = 1 - c->step_parity;
+        } else {
+            cudaMemsetAsync(c->d_overflow, 0, 2 * sizeof(int), c->st);   // a half-issued step must not leave a stale flag
+        }
     } else {
         e = ah::launch_site_step<float>(cur_fields<float>(c), next_fields<float>(c),
                                         make_coef<float>(P, tau, dt), P.nx, P.ny, P.nz, c->st);
+        n_launched = 1;
     }
     if (e != cudaSuccess) return cuda_fail(e, "step kernel launch");
-    c->launches += 1;
+    c->launches += n_launched;
     c->cur = 1 - c->cur;
     return AH_OK;
 }
@@ -200,9 +215,23 @@ int ensure_diag_scratch(ah_ctx *c, int records)
     return AH_OK;
 }
 
-int enqueue_diag(ah_ctx *c, double tau, double dt, int slot, int8_t *w3, uint8_t *near3)
+// the Gauss coefficient kappa = q (1 - delta) / (1 - omega) of reading #18 needs omega != 1
+int check_diag_time(const ah_ctx *c, double tau, double dt)
 {
-    const ah_params &P = c->P;
+    int rc = check_time(c, tau, dt);
+    if (rc != AH_OK) return rc;
+    double a, q, d, w;
+    coeffs(c->P, tau, dt, a, q, d, w);
+    if (w == 1.0)
+        return fail(AH_EINVAL, "diagnostics: omega = (1-s) delta = 1 at tau=%g, dt=%g: no Gauss coefficient", tau, dt);
+    return AH_OK;
+}
+
+// winding_only: coefficients of the static a = 1 model (the winding integers depend on none of them)
+int enqueue_diag(ah_ctx *c, double tau, double dt, int slot, int8_t *w3, uint8_t *near3, bool winding_only = false)
+{
+    ah_params P = c->P;
+    if (winding_only) P.p = 0.0, P.s = 0.0;
     const ah::DiagCoef k = make_diag_coef(P, tau, dt);
     cudaError_t e;
     if (P.fp64)
@@ -423,7 +452,7 @@ int ah_step(ah_ctx *c, int n, double tau, double dt)
     int rc = check_time(c, tau, dt);
     if (rc != AH_OK) return rc;
     for (int j = 0; j < n; ++j) {
-        rc = one_step(c, tau + (double)j * dt, dt);
+        rc = one_step(c, c->P, tau + (double)j * dt, dt);
         if (rc != AH_OK) return rc;
     }
     return AH_OK;
@@ -437,13 +466,12 @@ int ah_step_cooling(ah_ctx *c, int n, double delta, double dt)
     if (!(dt > 0.0) || !std::isfinite(dt) || !(delta > 0.0) || !(delta < 1.0))
         return fail(AH_EINVAL, "ah_step_cooling: need dt > 0 and 0 < delta < 1 (dt=%g, delta=%g)", dt, delta);
     // constant damping = the Hubble term frozen at tau = dt/delta with p = 1, alpha = 2; s = 0 keeps q = 1
-    const ah_params saved = c->P;
-    c->P.p = 1.0;
-    c->P.s = 0.0;
-    c->P.alpha = 2.0;
+    ah_params P = c->P;   // a copy: the context's own model is never touched
+    P.p = 1.0;
+    P.s = 0.0;
+    P.alpha = 2.0;
     int rc = AH_OK;
-    for (int j = 0; j < n && rc == AH_OK; ++j) rc = one_step(c, dt / delta, dt);
-    c->P = saved;
+    for (int j = 0; j < n && rc == AH_OK; ++j) rc = one_step(c, P, dt / delta, dt);
     return rc;
 }
 
@@ -451,7 +479,7 @@ int ah_diagnostics(ah_ctx *c, double tau, double dt, ah_diag *out)
 {
     if (!c || !out) return fail(AH_EINVAL, "ah_diagnostics: null pointer");
     if (!c->have_fields) return fail(AH_ESTATE, "ah_diagnostics: no fields were set");
-    int rc = check_time(c, tau, dt);
+    int rc = check_diag_time(c, tau, dt);
     if (rc != AH_OK) return rc;
     rc = ensure_diag_scratch(c, 1);
     if (rc != AH_OK) return rc;
@@ -470,6 +498,7 @@ int ah_step_diag(ah_ctx *c, int n, double tau, double dt, int every, ah_diag *ou
     if (n < 0 || every < 1) return fail(AH_EINVAL, "ah_step_diag: need n >= 0 and every >= 1");
     if (!c->have_fields) return fail(AH_ESTATE, "ah_step_diag: no fields were set");
     int rc = check_time(c, tau, dt);
+    for (int j = 0; j < n && rc == AH_OK; j += every) rc = check_diag_time(c, tau + (double)j * dt, dt);
     if (rc != AH_OK) return rc;
     const int records = (n + every - 1) / every;
     if (cap < records) return fail(AH_EINVAL, "ah_step_diag: cap=%d < %d records", cap, records);
@@ -484,7 +513,7 @@ int ah_step_diag(ah_ctx *c, int n, double tau, double dt, int every, ah_diag *ou
             rc = enqueue_diag(c, tj, dt, r, nullptr, nullptr);
             if (rc != AH_OK) return rc;
         }
-        rc = one_step(c, tj, dt, fused ? r : -1);
+        rc = one_step(c, c->P, tj, dt, fused ? r : -1);
         if (rc != AH_OK) return rc;
         if (diag) ++r;
     }
@@ -513,8 +542,8 @@ int ah_winding_field(ah_ctx *c, int8_t *host_w3, uint8_t *host_near3)
             return cuda_fail(e, "cudaMalloc near flags");
         }
     }
-    // winding does not depend on tau; any admissible time gives the same integers
-    rc = enqueue_diag(c, 1.0, 1.0, 0, d_w, d_near);
+    // winding does not depend on tau or on the couplings
+    rc = enqueue_diag(c, 1.0, 1.0, 0, d_w, d_near, /*winding_only=*/true);
     cudaError_t e = cudaSuccess;
     if (rc == AH_OK) e = cudaMemcpyAsync(host_w3, d_w, 3 * c->n, cudaMemcpyDeviceToHost, c->st);
     if (rc == AH_OK && e == cudaSuccess && host_near3)
