@@ -90,6 +90,11 @@ def test_coeffs_closed_forms(ahlib):
     assert q == 1.0 and d == pytest.approx(0.025) and w == pytest.approx(0.025)
     P = ahlib.make_params(8, s=0.25, p=0.0)
     assert ahlib.coeffs(P, -3.0, 0.1) == (1.0, 1.0, 0.0, 0.0)
+    # s < 0, the core-growth phase of PAPER.md:57: q = a^{2s} > 1 for a < 1, omega = (1-s) delta > delta
+    P = ahlib.make_params(8, s=-0.5, p=1.0, tau_ref=8.0)
+    a, q, d, w = ahlib.coeffs(P, 2.0, 0.1)
+    assert a == pytest.approx(0.25, rel=1e-14) and q == pytest.approx(4.0, rel=1e-14)
+    assert d == pytest.approx(0.05, rel=1e-14) and w == pytest.approx(0.075, rel=1e-14)
     with pytest.raises(ahlib.AhError) as ei:
         ahlib.coeffs(ahlib.make_params(8, p=1.0), 0.0, 0.1)
     assert ei.value.code == ahlib.AH_EINVAL

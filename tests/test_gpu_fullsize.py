@@ -16,6 +16,8 @@ pytestmark = pytest.mark.gpu
 N = 1024
 MODEL = dict(dx=0.5, lambda0=2.0, e0=1.0, sigma=1.0, s=1.0, p=1.0, tau_ref=1.0 + 0.1 * 220, alpha=2.0, compact=1)
 TAU0, DT = 1.0, 0.1
+# fused vs standalone read-outs: identical per-site fp32 terms, fp64 accumulation in a different order
+FUSED_SUM_RTOL = 1e-11
 
 
 def _samples(rng):
@@ -81,6 +83,16 @@ def test_1024_cubed_sampled_step_parity_and_invariants(oracle):
         sim.step(1, tau, DT)
         after = _gather_sites(torch, sim.current_bufs(), pts)
         d1 = sim.diagnostics(tau + DT, DT)
+        # fused DIAG instantiation in the bench launch configuration (21,888 CTAs, 64-plane chunks): its record for
+        # the entry snapshot must be ah_diagnostics of that snapshot (integers exactly, fp64 sums to the order of
+        # summation), and the step it performs must be the plain step
+        before2 = _gather_blocks(torch, sim.current_bufs(), pts)
+        rec = sim.step_diag(1, tau + DT, DT, 1)[0]
+        after2 = _gather_sites(torch, sim.current_bufs(), pts)
+        sim.step(1, tau + 2 * DT, DT)            # back to the ping-pong half that held the d1 snapshot ...
+        # per-plaquette winding integers of the current snapshot on the sampled blocks
+        blocks_w = _gather_blocks(torch, sim.current_bufs(), pts)
+        w_gpu, near_gpu = sim.winding_field()
 
     Po = oracle.make_params(5, 5, 5, **MODEL)
     scale = {}
@@ -95,6 +107,37 @@ def test_1024_cubed_sampled_step_parity_and_invariants(oracle):
             worst[name] = max(worst[name], float(np.abs(after[i, sl] - ref[sl]).max() / scale[name]))
     # one fp32 step from identical inputs: a few ulps of the field's scale (same bound as the small-lattice tests)
     assert all(v <= 2e-6 for v in worst.values()), worst
+
+    # fused record == standalone read-outs of the same snapshot
+    for key in ("n_wind", "n_wind_xy", "n_wind_xz", "n_wind_yz", "n_near_branch", "n_big_plaq"):
+        assert rec[key] == d1[key], (key, rec[key], d1[key])
+    assert rec["gauss_max"] == d1["gauss_max"]
+    for key in ("sum_pi2_L", "sum_grad2_L", "sum_L", "gauss_l2", "gauss_div_l2", "gauss_charge_l2", "v2_phi"):
+        assert rec[key] == pytest.approx(d1[key], rel=FUSED_SUM_RTOL), key
+    # ... and the fused step moved the sampled sites exactly as the oracle says (same bound as the plain step)
+    Po5 = oracle.make_params(5, 5, 5, **MODEL)
+    worst2 = dict.fromkeys(worst, 0.0)
+    for i in range(len(pts)):
+        ref = oracle.step(Po5, np.ascontiguousarray(before2[i]), 1, tau + DT, DT)[:, 2, 2, 2]
+        for name, sl in groups:
+            worst2[name] = max(worst2[name], float(np.abs(after2[i, sl] - ref[sl]).max() / scale[name]))
+    assert all(v <= 2e-6 for v in worst2.values()), worst2
+    # winding integers on the sampled blocks against the oracle (plaquettes whose corners stay inside the block)
+    n_checked = n_wound = 0
+    for i, (x, y, z) in enumerate(pts):
+        w_or, near_or = oracle.winding(Po5, np.ascontiguousarray(blocks_w[i]))
+        for dz in range(4):
+            for dy in range(4):
+                for dx_ in range(4):
+                    X, Y, Z = (x - 2 + dx_) % N, (y - 2 + dy) % N, (z - 2 + dz) % N
+                    for k in range(3):
+                        if near_or[k, dz, dy, dx_] or near_gpu[k, Z, Y, X]:
+                            continue
+                        assert w_gpu[k, Z, Y, X] == w_or[k, dz, dy, dx_], (x, y, z, k, dz, dy, dx_)
+                        n_checked += 1
+                        n_wound += int(w_or[k, dz, dy, dx_] != 0)
+    assert n_checked > 0.99 * len(pts) * 192 and n_wound > 0
+    del w_gpu, near_gpu
 
     # properties that hold at any size
     assert d0["n_wind"] > 0 and d1["n_wind"] > 0

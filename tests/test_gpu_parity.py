@@ -117,6 +117,7 @@ ONE_STEP_CASES = [
     dict(p=2.0, s=1.0, tau_ref=3.0),
     dict(p=1.0, s=0.5, tau_ref=2.0, lambda0=1.3, e0=0.7, sigma=1.2, dx=0.4, alpha=1.5),
     dict(p=1.0, s=1.0, tau_ref=3.0, compact=0),
+    dict(p=1.0, s=-0.5, tau_ref=3.0),      # s < 0: the core-growth phase of PAPER.md:57
 ]
 
 
@@ -234,6 +235,61 @@ def test_parity_config1_64cubed_100_and_160_steps(ah, oracle):
     sim.close()
 
 
+@pytest.mark.parametrize("model", [dict(p=1.0, s=0.0), dict(p=1.0, s=1.0, tau_ref=1.0 + 160 * 0.1)])
+def test_parity_north_star_gate_on_the_tiled_kernel(ah, oracle, model):
+    """north_star's gate (max rel |d phi|, |d ep| <= 1e-4 after 100 steps) on the PRODUCT kernel: 64^3 is below
+    the tiled kernel's 128-site rows, so the gate is run at 128^3, the smallest cube it takes, for s = 0
+    (BASELINE config 1's model) and s = 1 (configs 2-5), from oracle initial conditions, 100 and 160 steps."""
+    n, dt, tau0 = 128, 0.1, 1.0
+    sim, Po = both(ah, oracle, (n, n, n), **model)
+    assert sim.get_kernel() == ah.KERNEL_TILED
+    f = oracle.init_fields(Po, 1)
+    sim.set_fields(f)
+    f = sim.get_fields().astype(np.float64)
+    sim.step(100, tau0, dt)
+    g100 = sim.get_fields()
+    oracle.step(Po, f, 100, tau0, dt)
+    r100 = rel_max(g100, f)
+    print("tiled 128^3 100 steps rel err:", model, r100)
+    assert r100["phi"] <= 1e-4 and r100["ep"] <= 1e-4, r100
+    assert r100["pi"] <= 1e-4 and r100["th"] <= 1e-4, r100
+    sim.step(60, tau0 + 100 * dt, dt)
+    oracle.step(Po, f, 60, tau0 + 100 * dt, dt)
+    r160 = rel_max(sim.get_fields(), f)
+    print("tiled 128^3 160 steps rel err:", model, r160)
+    assert max(r160.values()) <= 1e-3, r160
+    sim.close()
+
+
+def test_tiled_step_repeats_bit_identically(ah):
+    """Race detector for the tiled kernel's shared-memory protocol (ring slots and the per-warp Pi, ep row are
+    refilled by async-proxy bulk copies after generic-proxy reads, ordered by the CTA barrier / program order):
+    a timing-dependent overwrite would change Pi, ep by O(1) at the sites of the clobbered row, so the same state
+    advanced several times must come out bit-identical, under the plain and under the DIAG instantiation.
+    256 x 66 x 200 covers full 64-plane chunks, a partial last chunk and a ragged y tail (66 = 11 x 6)."""
+    shape = (256, 66, 200)
+    f0 = inputs.random_state(*shape, seed=77, th_amp=0.4)
+    sim = ah.Simulation(params=ah.make_params(*shape, p=1.0, s=1.0, tau_ref=3.0))
+    assert sim.get_kernel() == ah.KERNEL_TILED
+    outs = []
+    for rep in range(4):
+        sim.set_fields(f0)
+        if rep < 3:
+            sim.step(6, 1.0, 0.1)
+        else:
+            sim.step_diag(6, 1.0, 0.1, 1)          # every step through the DIAG instantiation
+        outs.append(sim.get_fields())
+    for o_ in outs[1:]:
+        assert np.array_equal(outs[0], o_)
+    # and against the independent site kernel (different code path, same fp32 algebra up to rounding order)
+    sim.set_kernel(ah.KERNEL_SITE)
+    sim.set_fields(f0)
+    sim.step(6, 1.0, 0.1)
+    r = rel_max(sim.get_fields(), outs[0].astype(np.float64))
+    assert max(r.values()) <= 1e-5, r
+    sim.close()
+
+
 def test_parity_tiled_128cubed_physical_width(ah, oracle):
     """Config-2-like (radiation, s=1, tau_ref = end time) at 128^3 for 40 steps, tiled kernel vs oracle,
     and tiled vs site kernel."""
@@ -280,6 +336,40 @@ def test_parity_config2_256cubed_winding_every_20(ah, oracle):
     r = rel_max(got, ref)
     assert r["phi"] <= 1e-4 and r["ep"] <= 1e-4 and r["pi"] <= 1e-4 and r["th"] <= 1e-4, r
     sim.close()
+
+
+def test_parity_config3_512cubed_matter_fused_record(ah, oracle):
+    """BASELINE configs[2] at its own size (512^3, matter era, s = 1, tau_ref = 129, all three read-outs), first 21
+    of its 1280 steps: the record the fused DIAG instantiation writes for step 20 against oracle.diagnostics of the
+    snapshot downloaded at that step.  Sigma-type sums 1e-5; the Gauss residual is truncation-level in the matter
+    era with s != 0 (reading #18), so it is COMPARED with the oracle's value, not asserted to be round-off."""
+    import torch
+    n, tau0, dt, every = 512, 1.0, 0.1, 20
+    model = dict(p=2.0, s=1.0, tau_ref=tau0 + 1280 * dt)
+    sim, Po = both(ah, oracle, (n, n, n), **model)
+    assert sim.get_kernel() == ah.KERNEL_TILED
+    sim.init_fields(1)
+    sim.step(every, tau0, dt)
+    tau = tau0 + every * dt
+    snap = sim.get_fields()
+    rec = sim.step_diag(1, tau, dt, 1)[0]
+    sim.close()
+    torch.cuda.empty_cache()
+    od = oracle.diagnostics(Po, snap.astype(np.float64), tau, dt)
+    del snap
+    slack = rec["n_near_branch"] + od["n_near_branch"]
+    for key in ("n_wind", "n_wind_xy", "n_wind_xz", "n_wind_yz"):
+        assert abs(rec[key] - od[key]) <= slack, (key, rec[key], od[key], slack)
+    assert rec["n_wind"] > 1000
+    assert rec["n_big_plaq"] == od["n_big_plaq"]
+    for key in ("sum_pi2_L", "sum_grad2_L", "sum_L"):
+        assert rec[key] == pytest.approx(od[key], rel=1e-5), (key, rec[key], od[key])
+    assert rec["v2_phi"] == pytest.approx(od["v2_phi"], abs=1e-5)
+    assert rec["xi_l"] == pytest.approx(od["xi_l"], rel=1e-5)
+    for key in ("gauss_max", "gauss_l2", "gauss_div_l2", "gauss_charge_l2"):
+        assert rec[key] == pytest.approx(od[key], rel=1e-9), (key, rec[key], od[key])
+    assert rec["gauss_rel"] == pytest.approx(od["gauss_rel"], rel=1e-8)
+    print("config 3 record at step 20:", {k: rec[k] for k in ("n_wind", "xi_w", "xi_l", "v2_phi", "gauss_rel")})
 
 
 def _evolved_snapshot(ah, oracle, n, steps, seed, **model):
