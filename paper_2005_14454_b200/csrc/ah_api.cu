@@ -80,6 +80,11 @@ ah::DiagCoef make_diag_coef(const ah_params &P, double tau, double dt)
     // callers check it (ah_diagnostics returns AH_EINVAL); 0 keeps the kernel's sums finite
     k.two_e2_kappa = (w == 1.0) ? 0.0 : 2.0 * P.e0 * P.e0 * q * (1.0 - d) / (1.0 - w);
     k.compact = P.compact;
+    k.f_idx2 = (float)k.idx2;
+    k.f_idx4 = (float)(k.idx2 * k.idx2);
+    k.f_quarter_lam_q = (float)k.quarter_lam_q;
+    k.f_sig2 = (float)k.sig2;
+    k.f_inv_2e2q = (float)k.inv_2e2q;
     return k;
 }
 
@@ -159,10 +164,17 @@ int one_step(ah_ctx *c, const ah_params &P, double tau, double dt, int diag_slot
             const ah::DiagCoef dk = make_diag_coef(P, tau, dt);
             e = ah::launch_tiled_step(cur_fields<float>(c), next_fields<float>(c), k, P.nx, P.ny, P.nz, flag, c->st,
                                       &dk, c->d_partials);
+            // a link angle outside the tiled kernel's domain spoils its read-outs as well: the standalone kernel
+            // then re-evaluates the entry snapshot (conditional launch, exits at once when the flag is clear)
+            if (e == cudaSuccess) {
+                ++n_launched;
+                e = ah::launch_diag_partials<float>(cur_fields<float>(c), dk, P.nx, P.ny, P.nz, c->d_partials, nullptr,
+                                                    nullptr, flag, c->st);
+            }
             if (e == cudaSuccess) {
                 ++n_launched;
                 e = ah::launch_diag_final(c->d_partials, ah::tiled_num_blocks(P.nx, P.ny, P.nz),
-                                          c->d_results + diag_slot, c->st);
+                                          c->d_results + diag_slot, c->st, ah::diag_num_blocks(P.nx, P.ny, P.nz), flag);
             }
         } else {
             e = ah::launch_tiled_step(cur_fields<float>(c), next_fields<float>(c), k, P.nx, P.ny, P.nz, flag, c->st);

@@ -35,6 +35,8 @@ struct DiagCoef {
     double inv_2e2q;    // 1/(2 e0^2 q)
     double two_e2_kappa;// 2 e0^2 kappa, kappa = q (1-delta)/(1-omega)   reading #18
     int compact;
+    // the same scalars rounded once to fp32 on the host, for the fp32 read-out arithmetic
+    float f_idx2, f_idx4, f_quarter_lam_q, f_sig2, f_inv_2e2q;
 };
 
 template <typename real>
@@ -243,9 +245,37 @@ __device__ __forceinline__ float plaq_sin(float x)
 }
 __device__ __forceinline__ double plaq_sin(double x) { return sin(x); }
 
+// ---- fp32 building blocks with a FIXED rounding sequence (explicit intrinsics, no compiler-chosen FMA
+// contraction): the tiled step kernel, its fused read-outs and the standalone diagnostics kernel all evaluate
+// these, so a quantity computed in two kernels is the same bit pattern in both.
+
+// forward hop U_i(x) phi(x+i), U = cos th - i sin th (Eq. 12), from c = cos th_i(x), s = sin th_i(x)
+__device__ __forceinline__ void hop_fwd_f32(float c, float s, float br, float bi, float &hr, float &hi)
+{
+    hr = __fmaf_rn(c, br, __fmul_rn(s, bi));
+    hi = __fmaf_rn(c, bi, -__fmul_rn(s, br));
+}
+// hand-over conj(U_i(x)) phi(x) for the site x + i
+__device__ __forceinline__ void hop_bwd_f32(float c, float s, float fr, float fi, float &hr, float &hi)
+{
+    hr = __fmaf_rn(c, fr, -__fmul_rn(s, fi));
+    hi = __fmaf_rn(c, fi, __fmul_rn(s, fr));
+}
+// Phi_ij(x) = th_i(x) + th_j(x+i) - th_i(x+j) - th_j(x)   (Eqs. 14-15, reading #9), summed left to right
+__device__ __forceinline__ float plaq_angle_f32(float th_i, float th_j_xi, float th_i_xj, float th_j)
+{
+    return __fadd_rn(__fadd_rn(__fadd_rn(th_i, th_j_xi), -th_i_xj), -th_j);
+}
+
 // ------------------------------------------------------------------------- block reduction
 
 __device__ __forceinline__ double warp_sum(double v)
+{
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+__device__ __forceinline__ int warp_sum(int v)
 {
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);

@@ -53,11 +53,77 @@ struct GlobalSiteAccessor {
     }
 };
 
+// The read-outs of one site into cnt / acc, with the per-plaquette integers in wi / nearf.  fp64 state: diag_site()
+// (libm, neighbours through the accessor).  fp32 state inside the tiled kernel's domain (|th| < 2^16): the
+// fixed-rounding arithmetic of ah_diag_site.cuh on inputs gathered from global memory — the bit patterns the fused
+// DIAG instantiation of the tiled step kernel produces for the same site; outside the domain: diag_site().
+__device__ __forceinline__ void site_readouts(const ConstFields<double> &in, const DiagCoef &k, int nx, int ny, int nz,
+                                              int x, int y, int z, long long *cnt, double *acc, int *wi, int *nearf)
+{
+    const GlobalSiteAccessor<double> a{in, nx, ny, nz, x, y, z};
+    diag_site<double>(a, k, cnt, acc, wi, nearf);
+}
+
+__device__ __forceinline__ void site_readouts(const ConstFields<float> &in, const DiagCoef &k, int nx, int ny, int nz,
+                                              int x, int y, int z, long long *cnt, double *acc, int *wi, int *nearf)
+{
+    const GlobalSiteAccessor<float> a{in, nx, ny, nz, x, y, z};
+    const size_t c = a.at(0, 0, 0), cx = a.at(1, 0, 0), cy = a.at(0, 1, 0), cz = a.at(0, 0, 1);
+    const size_t cxy = a.at(1, 1, 0), cxz = a.at(1, 0, 1), cyz = a.at(0, 1, 1);
+    const float *thx = in.f[TH_X], *thy = in.f[TH_Y], *thz = in.f[TH_Z];
+    const float t0x = thx[c], t0y = thy[c], t0z = thz[c];
+    const float ty_xp = thy[cx], tz_xp = thz[cx], tx_yp = thx[cy], tz_yp = thz[cy], tx_zp = thx[cz], ty_zp = thy[cz];
+    const float tmax = fmaxf(fmaxf(fmaxf(fabsf(t0x), fabsf(t0y)), fmaxf(fabsf(t0z), fabsf(ty_xp))),
+                             fmaxf(fmaxf(fabsf(tz_xp), fabsf(tx_yp)),
+                                   fmaxf(fabsf(tz_yp), fmaxf(fabsf(tx_zp), fabsf(ty_zp)))));
+    if (!(tmax < AH_READOUT_TH_LIMIT)) {
+        diag_site<float>(a, k, cnt, acc, wi, nearf);
+        return;
+    }
+    const float *pr = in.f[PHI_RE], *pi = in.f[PHI_IM];
+    const float fr = pr[c], fi = pi[c];
+    // D1
+    const float Pxy = plaq_angle_f32(t0x, ty_xp, tx_yp, t0y), Pxz = plaq_angle_f32(t0x, tz_xp, tx_zp, t0z);
+    const float Pyz = plaq_angle_f32(t0y, tz_yp, ty_zp, t0z);
+    const SiteWinding sw = readout_winding(
+        site_phase_fast(fr, fi), site_phase_fast(pr[cx], pi[cx]), site_phase_fast(pr[cy], pi[cy]),
+        site_phase_fast(pr[cz], pi[cz]), site_phase_fast(pr[cxy], pi[cxy]), site_phase_fast(pr[cxz], pi[cxz]),
+        site_phase_fast(pr[cyz], pi[cyz]), t0x, t0y, t0z, ty_xp, tz_xp, tx_yp, tz_yp, tx_zp, ty_zp, Pxy, Pxz, Pyz);
+#pragma unroll
+    for (int pq = 0; pq < 3; ++pq) {
+        wi[pq] = sw.w[pq];
+        nearf[pq] = sw.nearf[pq];
+        cnt[pq] += abs(sw.w[pq]);
+        cnt[DS_NEAR] += sw.nearf[pq];
+        cnt[DS_BIG] += sw.big[pq];
+    }
+    // D2: hops with the tiled kernel's link variables
+    float sx, cxv, sy, cyv, sz, czv;
+    sincos_pi_f32(t0x, sx, cxv);
+    sincos_pi_f32(t0y, sy, cyv);
+    sincos_pi_f32(t0z, sz, czv);
+    float hxr, hxi, hyr, hyi, hzr, hzi;
+    hop_fwd_f32(cxv, sx, pr[cx], pi[cx], hxr, hxi);
+    hop_fwd_f32(cyv, sy, pr[cy], pi[cy], hyr, hyi);
+    hop_fwd_f32(czv, sz, pr[cz], pi[cz], hzr, hzi);
+    const float pir = in.f[PI_RE][c], pii = in.f[PI_IM][c];
+    const float ex = in.f[EP_X][c], ey = in.f[EP_Y][c], ez = in.f[EP_Z][c];
+    float pi2L, gr2L, L;
+    readout_lagrangian(fr, fi, readout_grad2(fr, fi, hxr, hxi, hyr, hyi, hzr, hzi, k.f_idx2),
+                       readout_plaq_energy(Pxy, Pxz, Pyz, k.compact, k.f_idx4), pir, pii, ex, ey, ez, k, pi2L, gr2L, L);
+    // D3
+    double G, div, charge;
+    readout_gauss(fr, fi, pir, pii, ex, ey, ez, a.ep_back(0), a.ep_back(1), a.ep_back(2), k, G, div, charge);
+    readout_accumulate(acc, pi2L, gr2L, L, G, div, charge);
+}
+
+// only_if != nullptr: the launch is a conditional re-evaluation (ah_api.cu): nothing happens unless *only_if != 0
 template <typename real>
 __global__ void __launch_bounds__(DBX * DBY)
 diag_kernel(ConstFields<real> in, DiagCoef k, int nx, int ny, int nz, DiagPartial *partials,
-            int8_t *w3, uint8_t *near3)
+            int8_t *w3, uint8_t *near3, const int *only_if)
 {
+    if (only_if != nullptr && *only_if == 0) return;
     const int x = blockIdx.x * DBX + threadIdx.x;
     const int y = blockIdx.y * DBY + threadIdx.y;
     const bool active = (x < nx) && (y < ny);
@@ -68,10 +134,9 @@ diag_kernel(ConstFields<real> in, DiagCoef k, int nx, int ny, int nz, DiagPartia
     const int z_end = min(nz, ((int)blockIdx.z + 1) * DBZ);
     const size_t n = (size_t)nx * ny * nz;
     for (int z = blockIdx.z * DBZ; active && z < z_end; ++z) {
-        const GlobalSiteAccessor<real> a{in, nx, ny, nz, x, y, z};
         int wi[3], nearf[3];
-        diag_site<real>(a, k, cnt, acc, wi, nearf);
-        const size_t c = a.at(0, 0, 0);
+        site_readouts(in, k, nx, ny, nz, x, y, z, cnt, acc, wi, nearf);
+        const size_t c = (size_t)x + (size_t)nx * ((size_t)y + (size_t)ny * (size_t)z);
 #pragma unroll
         for (int pq = 0; pq < 3; ++pq) {
             if (w3) w3[(size_t)pq * n + c] = (int8_t)wi[pq];
@@ -117,10 +182,12 @@ diag_kernel(ConstFields<real> in, DiagCoef k, int nx, int ny, int nz, DiagPartia
 }
 
 // Fixed-order total of the per-block partials: thread t sums partials t, t+1024, ... ; then a
-// shared-memory tree.  One block.
+// shared-memory tree.  One block.  The number of partials is n, or n_alt when *use_alt != 0 (the partials then
+// come from the conditional re-evaluation by diag_kernel, which has its own grid).
 __global__ void __launch_bounds__(1024)
-diag_final_kernel(const DiagPartial *partials, int n, DiagPartial *result)
+diag_final_kernel(const DiagPartial *partials, int n, int n_alt, const int *use_alt, DiagPartial *result)
 {
+    if (use_alt != nullptr && *use_alt != 0) n = n_alt;
     __shared__ long long s_i[1024];
     __shared__ double s_f[1024];
     const int t = threadIdx.x;
@@ -162,9 +229,21 @@ int diag_num_blocks(int nx, int ny, int nz)
     return ((nx + DBX - 1) / DBX) * ((ny + DBY - 1) / DBY) * ((nz + DBZ - 1) / DBZ);
 }
 
-cudaError_t launch_diag_final(const DiagPartial *partials, int n, DiagPartial *result, cudaStream_t st)
+cudaError_t launch_diag_final(const DiagPartial *partials, int n, DiagPartial *result, cudaStream_t st, int n_alt,
+                              const int *use_alt)
 {
-    diag_final_kernel<<<1, 1024, 0, st>>>(partials, n, result);
+    diag_final_kernel<<<1, 1024, 0, st>>>(partials, n, n_alt, use_alt, result);
+    return cudaGetLastError();
+}
+
+template <typename real>
+cudaError_t launch_diag_partials(const ConstFields<real> &in, const DiagCoef &k, int nx, int ny, int nz,
+                                 DiagPartial *partials, int8_t *w3, uint8_t *near3, const int *only_if,
+                                 cudaStream_t st)
+{
+    dim3 block(DBX, DBY, 1);
+    dim3 grid((nx + DBX - 1) / DBX, (ny + DBY - 1) / DBY, (nz + DBZ - 1) / DBZ);
+    diag_kernel<real><<<grid, block, 0, st>>>(in, k, nx, ny, nz, partials, w3, near3, only_if);
     return cudaGetLastError();
 }
 
@@ -173,19 +252,17 @@ cudaError_t launch_diag(const ConstFields<real> &in, const DiagCoef &k, int nx, 
                         DiagPartial *partials, DiagPartial *result, int8_t *w3, uint8_t *near3,
                         cudaStream_t st)
 {
-    dim3 block(DBX, DBY, 1);
-    dim3 grid((nx + DBX - 1) / DBX, (ny + DBY - 1) / DBY, (nz + DBZ - 1) / DBZ);
-    diag_kernel<real><<<grid, block, 0, st>>>(in, k, nx, ny, nz, partials, w3, near3);
-    cudaError_t e = cudaGetLastError();
+    cudaError_t e = launch_diag_partials<real>(in, k, nx, ny, nz, partials, w3, near3, nullptr, st);
     if (e != cudaSuccess) return e;
-    diag_final_kernel<<<1, 1024, 0, st>>>(partials, diag_num_blocks(nx, ny, nz), result);
-    return cudaGetLastError();
+    return launch_diag_final(partials, diag_num_blocks(nx, ny, nz), result, st);
 }
 
 template cudaError_t launch_diag<float>(const ConstFields<float> &, const DiagCoef &, int, int, int,
                                         DiagPartial *, DiagPartial *, int8_t *, uint8_t *, cudaStream_t);
 template cudaError_t launch_diag<double>(const ConstFields<double> &, const DiagCoef &, int, int, int,
                                          DiagPartial *, DiagPartial *, int8_t *, uint8_t *, cudaStream_t);
+template cudaError_t launch_diag_partials<float>(const ConstFields<float> &, const DiagCoef &, int, int, int,
+                                                 DiagPartial *, int8_t *, uint8_t *, const int *, cudaStream_t);
 
 // ------------------------------------------------------------------------- trig test hook
 

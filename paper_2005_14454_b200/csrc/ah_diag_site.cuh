@@ -182,4 +182,169 @@ __device__ __forceinline__ void diag_site(const A &a, const DiagCoef &k, long lo
     acc[DF_GMAX] = fmax(acc[DF_GMAX], fabs(G));
 }
 
+
+// ======================================================================= fp32 read-outs, fixed rounding sequence
+//
+// The fused DIAG instantiation of the tiled step kernel evaluates the read-outs of a site from what the step
+// already holds in registers for that site (own phi, th; forward hops; plaquette angles; the staged Pi, ep) and
+// from a shared-memory table of site phases alpha = Arg(phi).  The routines below are that arithmetic, written
+// with explicit rounding intrinsics so that the standalone diagnostics kernel, which gathers the same inputs from
+// global memory, produces the SAME bit patterns site by site: integers (winding, flags) and max |G| are then equal
+// between the two kernels and the fp64 sums differ only by the order of summation.  Domain: every link angle
+// involved has |th| < 2^16 (the tiled kernel's domain); outside it the standalone kernel takes diag_site() above
+// and the API replaces a fused record by a standalone one (ah_api.cu).
+
+#define AH_READOUT_TH_LIMIT 65536.0f
+
+// alpha = Arg(phi) in (-pi, pi], NaN when phi == 0: atan(t) = t P(t^2) on t = min/max in [0, 1] (own minimax fit,
+// 8 coefficients, |error| <= 1.2e-7 + the 2-ulp division), then the octant / sign fix-ups.  Quadrant and sign come
+// from exact comparisons, so the branch (-pi, pi] is that of atan2f; the value may differ from it by ~2.5e-7 rad,
+// far inside the 1e-5 rad near-branch band of reading #14.
+__device__ __forceinline__ float site_phase_fast(float re, float im)
+{
+    const float ax = fabsf(re), ay = fabsf(im);
+    const float mx = fmaxf(ax, ay), mn = fminf(ax, ay);
+    const float t = __fdividef(mn, mx);                        // 0/0 -> NaN: a site without a phase
+    const float u = __fmul_rn(t, t);
+    float p = __fmaf_rn(u, -0.003687542863190174f, 0.020418046042323112f);
+    p = __fmaf_rn(p, u, -0.05361030250787735f);
+    p = __fmaf_rn(p, u, 0.09452305734157562f);
+    p = __fmaf_rn(p, u, -0.13822640478610992f);
+    p = __fmaf_rn(p, u, 0.19925765693187714f);
+    p = __fmaf_rn(p, u, -0.333274781703949f);
+    p = __fmaf_rn(p, u, 0.9999983906745911f);
+    p = __fmul_rn(p, t);
+    p = (ay > ax) ? __fadd_rn(1.57079637050628662f, -p) : p;
+    p = (re < 0.0f) ? __fadd_rn(3.14159274101257324f, -p) : p;
+    return (mx == 0.0f) ? NAN : copysignf(p, im);
+}
+
+// y - 2 pi rint(y / 2 pi) with the rounding sequence pinned
+__device__ __forceinline__ float wrap_2pi_fix(float y)
+{
+    const float magic = 12582912.0f;                          // 1.5 * 2^23
+    const float k = __fadd_rn(__fmaf_rn(y, 0.15915494309189535f, magic), -magic);
+    const float r = __fmaf_rn(k, -6.2831854820251465f, y);    // fl32(2 pi)
+    return __fmaf_rn(k, 1.7484555314695172e-07f, r);          // fl32(2 pi - fl32(2 pi)) (negative)
+}
+// d = principal value of alpha_head - alpha_tail - th; 0 when either end has no phase.  |th| < 2^16.
+__device__ __forceinline__ float link_phase_fix(float a_tail, float a_head, float th)
+{
+    const float y = __fadd_rn(__fadd_rn(a_head, -a_tail), -wrap_2pi_fix(th));
+    const float d = wrap_2pi_fix(y);
+    return (y == y) ? d : 0.0f;
+}
+
+struct SiteWinding {
+    int w[3];       // W_xy, W_xz, W_yz
+    int nearf[3];   // any of the four link phases within 1e-5 of +-pi
+    int big[3];     // |Phi_ij| > pi - 1e-5
+};
+
+// D1 of one site.  a0 = alpha(x); ax, ay, az = alpha(x+i); axy, axz, ayz = alpha(x+i+j);
+// t0* = th_*(x); t{j}_{i}p = th_j(x+i); P* = Phi_ij(x) (plaq_angle_f32).
+__device__ __forceinline__ SiteWinding readout_winding(float a0, float ax, float ay, float az, float axy, float axz,
+                                                       float ayz, float t0x, float t0y, float t0z, float ty_xp,
+                                                       float tz_xp, float tx_yp, float tz_yp, float tx_zp,
+                                                       float ty_zp, float Pxy, float Pxz, float Pyz)
+{
+    const float lim = 3.14159274101257324f - 1e-5f;
+    const float inv2pi = 0.15915494309189533577f;
+    const float dx0 = link_phase_fix(a0, ax, t0x), dy0 = link_phase_fix(a0, ay, t0y), dz0 = link_phase_fix(a0, az, t0z);
+    SiteWinding r;
+    {   // xy: d_x(x) + d_y(x+x) - d_x(x+y) - d_y(x)
+        const float d2 = link_phase_fix(ax, axy, ty_xp), d3 = link_phase_fix(ay, axy, tx_yp);
+        const float sum = __fadd_rn(__fadd_rn(__fadd_rn(__fadd_rn(dx0, d2), -d3), -dy0), Pxy);
+        r.w[0] = __float2int_rn(__fmul_rn(sum, inv2pi));
+        r.nearf[0] = fmaxf(fmaxf(fabsf(dx0), fabsf(d2)), fmaxf(fabsf(d3), fabsf(dy0))) >= lim;
+        r.big[0] = fabsf(Pxy) > lim;
+    }
+    {   // xz: d_x(x) + d_z(x+x) - d_x(x+z) - d_z(x)
+        const float d2 = link_phase_fix(ax, axz, tz_xp), d3 = link_phase_fix(az, axz, tx_zp);
+        const float sum = __fadd_rn(__fadd_rn(__fadd_rn(__fadd_rn(dx0, d2), -d3), -dz0), Pxz);
+        r.w[1] = __float2int_rn(__fmul_rn(sum, inv2pi));
+        r.nearf[1] = fmaxf(fmaxf(fabsf(dx0), fabsf(d2)), fmaxf(fabsf(d3), fabsf(dz0))) >= lim;
+        r.big[1] = fabsf(Pxz) > lim;
+    }
+    {   // yz: d_y(x) + d_z(x+y) - d_y(x+z) - d_z(x)
+        const float d2 = link_phase_fix(ay, ayz, tz_yp), d3 = link_phase_fix(az, ayz, ty_zp);
+        const float sum = __fadd_rn(__fadd_rn(__fadd_rn(__fadd_rn(dy0, d2), -d3), -dz0), Pyz);
+        r.w[2] = __float2int_rn(__fmul_rn(sum, inv2pi));
+        r.nearf[2] = fmaxf(fmaxf(fabsf(dy0), fabsf(d2)), fmaxf(fabsf(d3), fabsf(dz0))) >= lim;
+        r.big[2] = fabsf(Pyz) > lim;
+    }
+    return r;
+}
+
+// sum_{i<j} [2 (1 - cos Phi_ij)] / dx^4 of the three plaquettes owned by the site (compact; Phi^2 otherwise):
+// 2(1 - cos Phi) = 4 sin^2(Phi/2), no cancellation in fp32
+__device__ __forceinline__ float readout_plaq_energy(float Pxy, float Pxz, float Pyz, int compact, float idx4)
+{
+    float e0, e1, e2;
+    if (compact) {
+        const float s0 = sin_poly_f32(__fmul_rn(Pxy, 0.5f)), s1 = sin_poly_f32(__fmul_rn(Pxz, 0.5f));
+        const float s2 = sin_poly_f32(__fmul_rn(Pyz, 0.5f));
+        e0 = __fmul_rn(__fmul_rn(4.0f, s0), s0);
+        e1 = __fmul_rn(__fmul_rn(4.0f, s1), s1);
+        e2 = __fmul_rn(__fmul_rn(4.0f, s2), s2);
+    } else {
+        e0 = __fmul_rn(Pxy, Pxy);
+        e1 = __fmul_rn(Pxz, Pxz);
+        e2 = __fmul_rn(Pyz, Pyz);
+    }
+    return __fmul_rn(__fadd_rn(__fadd_rn(e0, e1), e2), idx4);
+}
+
+// sum_i |U_i phi(x+i) - phi|^2 / dx^2 from the three forward hops
+__device__ __forceinline__ float readout_grad2(float fr, float fi, float hxr, float hxi, float hyr, float hyi,
+                                               float hzr, float hzi, float idx2)
+{
+    const float ar = __fadd_rn(hxr, -fr), ai = __fadd_rn(hxi, -fi);
+    const float br = __fadd_rn(hyr, -fr), bi = __fadd_rn(hyi, -fi);
+    const float cr = __fadd_rn(hzr, -fr), ci = __fadd_rn(hzi, -fi);
+    float g = __fmaf_rn(ar, ar, __fmul_rn(ai, ai));
+    g = __fadd_rn(g, __fmaf_rn(br, br, __fmul_rn(bi, bi)));
+    g = __fadd_rn(g, __fmaf_rn(cr, cr, __fmul_rn(ci, ci)));
+    return __fmul_rn(g, idx2);
+}
+
+// D2 of one site (reading #15): L and its two weighted companions |Pi|^2 L, grad2 L (fp32 terms, summed in fp64)
+__device__ __forceinline__ void readout_lagrangian(float fr, float fi, float grad2, float b2, float pir, float pii,
+                                                   float ex, float ey, float ez, const DiagCoef &k, float &pi2L,
+                                                   float &gr2L, float &L)
+{
+    const float pi2 = __fmaf_rn(pir, pir, __fmul_rn(pii, pii));
+    const float e2 = __fmul_rn(__fmaf_rn(ez, ez, __fmaf_rn(ey, ey, __fmul_rn(ex, ex))), k.f_idx2);
+    const float m2 = __fadd_rn(__fmaf_rn(fr, fr, __fmul_rn(fi, fi)), -k.f_sig2);
+    const float pot = __fmul_rn(__fmul_rn(k.f_quarter_lam_q, m2), m2);
+    L = __fmaf_rn(__fadd_rn(e2, -b2), k.f_inv_2e2q, __fadd_rn(__fadd_rn(pi2, -grad2), -pot));
+    pi2L = __fmul_rn(pi2, L);
+    gr2L = __fmul_rn(grad2, L);
+}
+
+// D3 of one site, in fp64 from the stored fp32 values (a difference of nearly equal numbers)
+__device__ __forceinline__ void readout_gauss(float fr, float fi, float pir, float pii, float ex, float ey, float ez,
+                                              float exb, float eyb, float ezb, const DiagCoef &k, double &G,
+                                              double &div, double &charge)
+{
+    div = __dmul_rn(__dadd_rn(__dadd_rn(__dadd_rn((double)ex, -(double)exb), __dadd_rn((double)ey, -(double)eyb)),
+                              __dadd_rn((double)ez, -(double)ezb)),
+                    k.idx2);
+    charge = __dmul_rn(k.two_e2_kappa, __fma_rn((double)fr, (double)pii, -__dmul_rn((double)fi, (double)pir)));
+    G = __dadd_rn(div, -charge);
+}
+
+// adds one site's D2 + D3 terms to the fp64 accumulators
+__device__ __forceinline__ void readout_accumulate(double *acc, float pi2L, float gr2L, float L, double G, double div,
+                                                   double charge)
+{
+    acc[DF_SPI] += (double)pi2L;
+    acc[DF_SGR] += (double)gr2L;
+    acc[DF_SL] += (double)L;
+    acc[DF_GSQ] = __fma_rn(G, G, acc[DF_GSQ]);
+    acc[DF_DIVSQ] = __fma_rn(div, div, acc[DF_DIVSQ]);
+    acc[DF_CHSQ] = __fma_rn(charge, charge, acc[DF_CHSQ]);
+    acc[DF_GMAX] = fmax(acc[DF_GMAX], fabs(G));
+}
+
 }  // namespace ah

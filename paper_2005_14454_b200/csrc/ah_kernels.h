@@ -42,8 +42,16 @@ cudaError_t launch_diag(const ConstFields<real> &in, const DiagCoef &k, int nx, 
                         DiagPartial *partials, DiagPartial *result, int8_t *w3, uint8_t *near3,
                         cudaStream_t st);
 
-// fixed-order total of n per-block partials into *result (one block)
-cudaError_t launch_diag_final(const DiagPartial *partials, int n, DiagPartial *result, cudaStream_t st);
+// the per-block partials alone; only_if != nullptr makes the launch conditional on *only_if != 0 (the redo of a
+// fused record whose tiled kernel met a link angle outside its domain)
+template <typename real>
+cudaError_t launch_diag_partials(const ConstFields<real> &in, const DiagCoef &k, int nx, int ny, int nz,
+                                 DiagPartial *partials, int8_t *w3, uint8_t *near3, const int *only_if,
+                                 cudaStream_t st);
+
+// fixed-order total of n per-block partials into *result (one block); of n_alt partials when *use_alt != 0
+cudaError_t launch_diag_final(const DiagPartial *partials, int n, DiagPartial *result, cudaStream_t st, int n_alt = 0,
+                              const int *use_alt = nullptr);
 
 // tests only: evaluate the fp32 trig helpers on device arrays
 cudaError_t launch_test_trig(const float *x, float *s, float *c, float *ps, size_t n, cudaStream_t st);

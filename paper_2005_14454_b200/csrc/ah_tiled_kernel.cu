@@ -158,33 +158,14 @@ namespace {
 #define AH_TILED_TH_LIMIT 65536.0f
 
 // DIAG = true (SURVEY 8(a) row D-fuse): the same step, plus the read-outs D1-D3 of the ENTRY snapshot of every
-// site, evaluated by diag_site() from what is already staged for the step (phi, th planes with their (+,+)
-// corners, the warp's Pi, ep row) and from the site phases alpha = Arg(phi), computed once per staged site into
-// sm.alpha; the only extra global reads are the backward ep neighbours.  Per-thread sums are reduced per CTA
-// into partials[linear CTA index]; diag_final_kernel adds them in a fixed order.
-//
-// Neighbours from shared memory for diag_site(): the site is column `ci` of staged row `r`
-template <int TY>
-struct StagedSiteAccessor {
-    const Smem<TY, true> &sm;
-    int so, sf, ao, af, r, ci, w, qi;  // slots of plane z / z+1 (raw, alpha), staged row / column, warp, column in sm.qe
-    float ebx, eby, ebz;               // ep_x(x - x^), ep_y(x - y^), ep_z(x - z^)
-    __device__ __forceinline__ float phi_re(int dx, int dy, int dz) const { return sm.raw[dz ? sf : so][0][r + dy][ci + dx]; }
-    __device__ __forceinline__ float phi_im(int dx, int dy, int dz) const { return sm.raw[dz ? sf : so][1][r + dy][ci + dx]; }
-    __device__ __forceinline__ float th(int i, int dx, int dy, int dz) const
-    {
-        return sm.raw[dz ? sf : so][2 + i][r + dy][ci + dx];
-    }
-    __device__ __forceinline__ float alpha(int dx, int dy, int dz) const
-    {
-        return sm.alpha[dz ? af : ao][r - 1 + dy][ci + dx];
-    }
-    __device__ __forceinline__ float pi_re() const { return sm.qe[w][0][qi]; }
-    __device__ __forceinline__ float pi_im() const { return sm.qe[w][1][qi]; }
-    __device__ __forceinline__ float ep(int i) const { return sm.qe[w][2 + i][qi]; }
-    __device__ __forceinline__ float ep_back(int i) const { return i == 0 ? ebx : (i == 1 ? eby : ebz); }
-};
-
+// site.  They are fed by what the step holds for the site anyway — own phi, th and the forward neighbours' in
+// registers, the plaquette angles before their sines are taken, the forward hops, the staged Pi, ep row — plus
+// a shared-memory table of site phases alpha = Arg(phi) (one polynomial atan2 per staged site) from which the
+// nine link phases of a site's three plaquettes are wrapped differences (ah_diag_site.cuh).  Everything is read
+// as 128-bit rows, four sites per thread like the step itself.  The only extra global reads are the backward
+// ep_y row (ep_z of the plane below is carried in registers, ep_x of the left neighbour comes by shuffle).
+// Per-thread partial sums (int32 counts, fp64 sums) are reduced per CTA into partials[linear CTA index];
+// diag_final_kernel adds them in a fixed order.
 template <int TY, bool COMPACT, bool DIAG>
 __global__ void __launch_bounds__((TY + 1) * 32, ((TY + 1) * 32 <= 256) ? 2 : 1)
 tiled_step_kernel(ConstFields<float> in, Fields<float> out, StepCoef<float> k, int nx, int ny, int nz, int zc,
@@ -304,10 +285,12 @@ tiled_step_kernel(ConstFields<float> in, Fields<float> out, StepCoef<float> k, i
         if constexpr (DIAG) {
             const int r = is_main ? w + 1 : TY + 1;
             const V4 pr = lds4(&sm.raw[slot][0][r][cofs]), pi = lds4(&sm.raw[slot][1][r][cofs]);
-#pragma unroll 1
-            for (int j = 0; j < 4; ++j) sm.alpha[ab][r - 1][cofs + j] = site_phase<float>(pr.v[j], pi.v[j]);
+            V4 al;
+#pragma unroll
+            for (int j = 0; j < 4; ++j) al.v[j] = site_phase_fast(pr.v[j], pi.v[j]);
+            *reinterpret_cast<float4 *>(&sm.alpha[ab][r - 1][cofs]) = f4(al);
             if (lane == 31)
-                sm.alpha[ab][r - 1][cofs + 4] = site_phase<float>(sm.raw[slot][0][r][cofs + 4], sm.raw[slot][1][r][cofs + 4]);
+                sm.alpha[ab][r - 1][cofs + 4] = site_phase_fast(sm.raw[slot][0][r][cofs + 4], sm.raw[slot][1][r][cofs + 4]);
         }
     };
 
@@ -350,8 +333,16 @@ tiled_step_kernel(ConstFields<float> in, Fields<float> out, StepCoef<float> k, i
     int sf = 1, sf_par = 0;                           // slot and mbarrier parity of the forward plane (load n + 1)
     int af = 0;                                       // DIAG: sm.alpha buffer of the forward plane
     size_t oc = (size_t)z0 * sxy + ro - sxy;          // this thread's element offset in plane z0 + n - 1
-    long long d_cnt[DS_NINT] = {0, 0, 0, 0, 0};      // DIAG only: this thread's partial read-outs
-    double d_acc[DS_NFLT] = {0, 0, 0, 0, 0, 0, 0};
+    int d_cnt[DS_NINT] = {0, 0, 0, 0, 0};            // DIAG only: this thread's partial read-outs (a chunk of
+    double d_acc[DS_NFLT] = {0, 0, 0, 0, 0, 0, 0};   // <= 64 planes x 4 sites x 3 plaquettes fits int32)
+    V4 eb_z;                                         // DIAG only: ep_z of the own sites in the plane below
+    if constexpr (DIAG) {
+        if (act) {
+            const int zb = (z0 == 0) ? nz - 1 : z0 - 1;
+            const float4 t = __ldg(reinterpret_cast<const float4 *>(in.f[EP_Z] + (size_t)zb * sxy + ro));
+            eb_z.v[0] = t.x; eb_z.v[1] = t.y; eb_z.v[2] = t.z; eb_z.v[3] = t.w;
+        }
+    }
 
     // ---- march: iteration n updates plane z0 + n - 1 (slot n % 3), forward plane in slot (n + 1) % 3.
     // One __syncthreads per plane separates phase 1 (hand-overs written, staged planes read) from phase 2 (hand-overs
@@ -437,29 +428,20 @@ tiled_step_kernel(ConstFields<float> in, Fields<float> out, StepCoef<float> k, i
             V4 P_r, P_i, E_x, E_y, E_z;   // Pi+, ep+ still lacking the old Pi, ep and the terms from row y-1 / site x0-1
             if (n + 2 <= nplanes + 1) produce();
             mbar_wait(&sm.full[sf], sf_par);
+            float4 eb_y4 = make_float4(0.f, 0.f, 0.f, 0.f);
+            float eb_x0 = 0.f;
             if constexpr (DIAG) {
                 // site phases of the forward plane, shared by every link phase that needs them
                 af ^= 1;
                 stage_alpha(sf, af);
-                __syncthreads();
-                // read-outs of the entry snapshot of this plane (before anything of it is overwritten)
-                mbar_wait(&sm.qfull[w], (n - 1) & 1);
-                const int z = z0 + n - 1, zm = (z == 0) ? nz - 1 : z - 1, ym = (y == 0) ? ny - 1 : y - 1;
-                const int xw = (x0 == 0) ? nx - 1 : x0 - 1;
-                const float *eby = in.f[EP_Y] + (size_t)z * sxy + (size_t)ym * nx + x0 + 4 * lane;
-                const float *ebz = in.f[EP_Z] + (size_t)zm * sxy + ro;
-                const float ebx0 = (lane == 0) ? __ldg(in.f[EP_X] + (size_t)z * sxy + (size_t)y * nx + xw)
-                                               : sm.qe[w][2][4 * lane - 1];
-                // one site at a time, NOT unrolled: the read-outs are long (atan2, libm fall-backs) and four
-                // copies of them would not fit the instruction cache
-#pragma unroll 1
-                for (int j = 0; j < 4; ++j) {
-                    const StagedSiteAccessor<TY> a{sm, so, sf, af ^ 1, af, r_own, cofs + j, w, 4 * lane + j,
-                                                   j == 0 ? ebx0 : sm.qe[w][2][4 * lane + j - 1], __ldg(eby + j),
-                                                   __ldg(ebz + j)};
-                    int wi[3], nearf[3];
-                    diag_site<float>(a, dk, d_cnt, d_acc, wi, nearf);
+                // backward ep neighbours that are not on chip: the row y-1 of this plane, and (lane 0) the site x0-1
+                const int z = z0 + n - 1, ym = (y == 0) ? ny - 1 : y - 1;
+                eb_y4 = __ldg(reinterpret_cast<const float4 *>(in.f[EP_Y] + (size_t)z * sxy + (size_t)ym * nx + x0 + 4 * lane));
+                if (lane == 0) {
+                    const int xw = (x0 == 0) ? nx - 1 : x0 - 1;
+                    eb_x0 = __ldg(in.f[EP_X] + (size_t)z * sxy + (size_t)y * nx + xw);
                 }
+                __syncthreads();
             }
             V4 o_byr, o_byi, o_sxy, o_syz;   // for row y+1, through shared memory
             V4 h_bzr, h_bzi, h_sxz;          // this plane's hand-down to z+1 (with S_yz in o_syz)
@@ -484,10 +466,42 @@ tiled_step_kernel(ConstFields<float> in, Fields<float> out, StepCoef<float> k, i
             for (int j = 0; j < 4; ++j) {
                 const int jn = (j < 3) ? j + 1 : 3;
                 const float ty_xp = (j < 3) ? c_ty.v[jn] : r_ty, tz_xp = (j < 3) ? c_tz.v[jn] : r_tz;
-                S_xy.v[j] = c_tx.v[j] + ty_xp - y_tx.v[j] - c_ty.v[j];
-                S_xz.v[j] = c_tx.v[j] + tz_xp - n_tx.v[j] - c_tz.v[j];
-                S_yz.v[j] = c_ty.v[j] + y_tz.v[j] - n_ty.v[j] - c_tz.v[j];
+                S_xy.v[j] = plaq_angle_f32(c_tx.v[j], ty_xp, y_tx.v[j], c_ty.v[j]);
+                S_xz.v[j] = plaq_angle_f32(c_tx.v[j], tz_xp, n_tx.v[j], c_tz.v[j]);
+                S_yz.v[j] = plaq_angle_f32(c_ty.v[j], y_tz.v[j], n_ty.v[j], c_tz.v[j]);
                 amax = fmaxf(amax, fmaxf(fmaxf(fabsf(S_xy.v[j]), fabsf(S_xz.v[j])), fabsf(S_yz.v[j])));
+            }
+            V4 d_b2;   // DIAG: magnetic energy of the three plaquettes each site owns
+            if constexpr (DIAG) {
+                // D1 (winding, Eq. 16 right) from the site phases, and the plaquette energies, while the angles are
+                // still angles
+                const int ao = af ^ 1;
+                const V4 a_0 = lds4(&sm.alpha[ao][w][cofs]), a_y = lds4(&sm.alpha[ao][w + 1][cofs]);
+                const V4 a_z = lds4(&sm.alpha[af][w][cofs]), a_yz = lds4(&sm.alpha[af][w + 1][cofs]);
+                float a_0r = __shfl_down_sync(FULL, a_0.v[0], 1), a_yr = __shfl_down_sync(FULL, a_y.v[0], 1);
+                float a_zr = __shfl_down_sync(FULL, a_z.v[0], 1);
+                if (lane == 31) {
+                    a_0r = sm.alpha[ao][w][cofs + 4]; a_yr = sm.alpha[ao][w + 1][cofs + 4];
+                    a_zr = sm.alpha[af][w][cofs + 4];
+                }
+#pragma unroll
+                for (int j = 0; j < 4; ++j) {
+                    const int jn = (j < 3) ? j + 1 : 3;
+                    const float ty_xp = (j < 3) ? c_ty.v[jn] : r_ty, tz_xp = (j < 3) ? c_tz.v[jn] : r_tz;
+                    const float ax = (j < 3) ? a_0.v[jn] : a_0r, axy = (j < 3) ? a_y.v[jn] : a_yr;
+                    const float axz = (j < 3) ? a_z.v[jn] : a_zr;
+                    const SiteWinding sw = readout_winding(a_0.v[j], ax, a_y.v[j], a_z.v[j], axy, axz, a_yz.v[j],
+                                                           c_tx.v[j], c_ty.v[j], c_tz.v[j], ty_xp, tz_xp, y_tx.v[j],
+                                                           y_tz.v[j], n_tx.v[j], n_ty.v[j], S_xy.v[j], S_xz.v[j],
+                                                           S_yz.v[j]);
+#pragma unroll
+                    for (int pq = 0; pq < 3; ++pq) {
+                        d_cnt[pq] += abs(sw.w[pq]);
+                        d_cnt[DS_NEAR] += sw.nearf[pq];
+                        d_cnt[DS_BIG] += sw.big[pq];
+                    }
+                    d_b2.v[j] = readout_plaq_energy(S_xy.v[j], S_xz.v[j], S_yz.v[j], COMPACT ? 1 : 0, dk.f_idx4);
+                }
             }
             if (COMPACT) {
                 // two angles per issued instruction (FFMA2); bit-identical to the scalar polynomials
@@ -521,6 +535,15 @@ tiled_step_kernel(ConstFields<float> in, Fields<float> out, StepCoef<float> k, i
                 sincos4(c_ty, s_y, c_y);
                 sincos4(c_tz, s_z, c_z);
             }
+            V4 dq_r, dq_i, dq_ex, dq_ey, dq_ez;   // DIAG: the old Pi, ep of the own sites (read again after the barrier)
+            if constexpr (DIAG) {
+                mbar_wait(&sm.qfull[w], (n - 1) & 1);
+                dq_r = lds4(&sm.qe[w][0][4 * lane]); dq_i = lds4(&sm.qe[w][1][4 * lane]);
+                dq_ex = lds4(&sm.qe[w][2][4 * lane]); dq_ey = lds4(&sm.qe[w][3][4 * lane]);
+                dq_ez = lds4(&sm.qe[w][4][4 * lane]);
+                const float el = __shfl_up_sync(FULL, dq_ex.v[3], 1);   // ep_x of the site to the left of the first one
+                if (lane > 0) eb_x0 = el;
+            }
 #pragma unroll
             for (int j = 0; j < 4; ++j) {
                 const float fr = c_pr.v[j], fi = c_pi.v[j];
@@ -530,13 +553,27 @@ tiled_step_kernel(ConstFields<float> in, Fields<float> out, StepCoef<float> k, i
                 const float Sxy = S_xy.v[j], Sxz = S_xz.v[j], Syz = S_yz.v[j];
                 const float sx = s_x.v[j], cx = c_x.v[j], sy = s_y.v[j], cy = c_y.v[j], sz = s_z.v[j], cz = c_z.v[j];
                 // forward hops U_i(s) phi(s+i)                                   (Eq. 13)
-                const float fxr = cx * xr + sx * xi, fxi = cx * xi - sx * xr;
-                const float fyr = cy * y_pr.v[j] + sy * y_pi.v[j], fyi = cy * y_pi.v[j] - sy * y_pr.v[j];
-                const float fzr = cz * n_pr.v[j] + sz * n_pi.v[j], fzi = cz * n_pi.v[j] - sz * n_pr.v[j];
+                float fxr, fxi, fyr, fyi, fzr, fzi;
+                hop_fwd_f32(cx, sx, xr, xi, fxr, fxi);
+                hop_fwd_f32(cy, sy, y_pr.v[j], y_pi.v[j], fyr, fyi);
+                hop_fwd_f32(cz, sz, n_pr.v[j], n_pi.v[j], fzr, fzi);
                 // hand-overs conj(U_i(s)) phi(s)
-                const float bxr = cx * fr - sx * fi, bxi = cx * fi + sx * fr;
-                o_byr.v[j] = cy * fr - sy * fi; o_byi.v[j] = cy * fi + sy * fr;
-                h_bzr.v[j] = cz * fr - sz * fi; h_bzi.v[j] = cz * fi + sz * fr;
+                float bxr, bxi;
+                hop_bwd_f32(cx, sx, fr, fi, bxr, bxi);
+                hop_bwd_f32(cy, sy, fr, fi, o_byr.v[j], o_byi.v[j]);
+                hop_bwd_f32(cz, sz, fr, fi, h_bzr.v[j], h_bzi.v[j]);
+                if constexpr (DIAG) {
+                    // D2, D3 of the site (Eqs. 17-18, Eq. 5) from the hops just formed and the staged Pi, ep
+                    const float exb = (j == 0) ? eb_x0 : dq_ex.v[j > 0 ? j - 1 : 0];
+                    const float eyb = (j == 0) ? eb_y4.x : (j == 1) ? eb_y4.y : (j == 2) ? eb_y4.z : eb_y4.w;
+                    float pi2L, gr2L, L;
+                    readout_lagrangian(fr, fi, readout_grad2(fr, fi, fxr, fxi, fyr, fyi, fzr, fzi, dk.f_idx2), d_b2.v[j],
+                                       dq_r.v[j], dq_i.v[j], dq_ex.v[j], dq_ey.v[j], dq_ez.v[j], dk, pi2L, gr2L, L);
+                    double G, div, charge;
+                    readout_gauss(fr, fi, dq_r.v[j], dq_i.v[j], dq_ex.v[j], dq_ey.v[j], dq_ez.v[j], exb, eyb,
+                                  eb_z.v[j], dk, G, div, charge);
+                    readout_accumulate(d_acc, pi2L, gr2L, L, G, div, charge);
+                }
                 o_sxy.v[j] = Sxy; o_syz.v[j] = Syz; h_sxz.v[j] = Sxz;
                 // Eq. 7 without the x-1 (j == 0) and y-1 hops
                 float ar = (fxr + fyr) + (fzr + g_bzr.v[j]) - 6.0f * fr;
@@ -595,6 +632,7 @@ tiled_step_kernel(ConstFields<float> in, Fields<float> out, StepCoef<float> k, i
             const V4 q_r = lds4(&sm.qe[w][0][4 * lane]), q_i = lds4(&sm.qe[w][1][4 * lane]);
             const V4 e_x = lds4(&sm.qe[w][2][4 * lane]), e_y = lds4(&sm.qe[w][3][4 * lane]);
             const V4 e_z = lds4(&sm.qe[w][4][4 * lane]);
+            if constexpr (DIAG) eb_z = e_z;   // the plane below the next one
             V4 f_r, f_i, t_x, t_y, t_z;
 #pragma unroll
             for (int j = 0; j < 4; ++j) {
@@ -643,13 +681,13 @@ tiled_step_kernel(ConstFields<float> in, Fields<float> out, StepCoef<float> k, i
         double *s_f = reinterpret_cast<double *>(&sm.row[0][0][0][0]);       // [TY + 1][DS_NFLT]
         long long *s_i = reinterpret_cast<long long *>(s_f + (TY + 1) * DS_NFLT);   // [TY + 1][DS_NINT]
 #pragma unroll
-        for (int a = 0; a < DS_NINT; ++a) d_cnt[a] = warp_sum(d_cnt[a]);
+        for (int a = 0; a < DS_NINT; ++a) d_cnt[a] = warp_sum(d_cnt[a]);   // <= 32 x 64 x 12: fits int32
 #pragma unroll
         for (int a = 0; a < DS_NFLT - 1; ++a) d_acc[a] = warp_sum(d_acc[a]);
         d_acc[DF_GMAX] = warp_max(d_acc[DF_GMAX]);
         if (lane == 0) {
 #pragma unroll
-            for (int a = 0; a < DS_NINT; ++a) s_i[w * DS_NINT + a] = d_cnt[a];
+            for (int a = 0; a < DS_NINT; ++a) s_i[w * DS_NINT + a] = (long long)d_cnt[a];
 #pragma unroll
             for (int a = 0; a < DS_NFLT; ++a) s_f[w * DS_NFLT + a] = d_acc[a];
         }
