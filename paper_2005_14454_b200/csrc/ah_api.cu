@@ -173,7 +173,7 @@ int one_step(ah_ctx *c, const ah_params &P, double tau, double dt, int diag_slot
             }
             if (e == cudaSuccess) {
                 ++n_launched;
-                e = ah::launch_diag_final(c->d_partials, ah::tiled_num_blocks(P.nx, P.ny, P.nz),
+                e = ah::launch_diag_final(c->d_partials, ah::tiled_num_blocks(P.nx, P.ny, P.nz, true),
                                           c->d_results + diag_slot, c->st, ah::diag_num_blocks(P.nx, P.ny, P.nz), flag);
             }
         } else {
@@ -204,7 +204,7 @@ int one_step(ah_ctx *c, const ah_params &P, double tau, double dt, int diag_slot
 int ensure_diag_scratch(ah_ctx *c, int records)
 {
     int nb = ah::diag_num_blocks(c->P.nx, c->P.ny, c->P.nz);
-    const int nbt = ah::tiled_num_blocks(c->P.nx, c->P.ny, c->P.nz);
+    const int nbt = ah::tiled_num_blocks(c->P.nx, c->P.ny, c->P.nz, true);
     if (nbt > nb) nb = nbt;
     if (c->n_partials < nb) {
         if (c->d_partials) cudaFree(c->d_partials);

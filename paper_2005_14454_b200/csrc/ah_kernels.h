@@ -25,8 +25,8 @@ bool tiled_supported(int nx, int ny, int nz);
 cudaError_t launch_tiled_step(const ConstFields<float> &in, const Fields<float> &out,
                               const StepCoef<float> &k, int nx, int ny, int nz, int *overflow, cudaStream_t st,
                               const DiagCoef *dk = nullptr, DiagPartial *partials = nullptr);
-int tiled_num_blocks(int nx, int ny, int nz);
-int tiled_chunk(int nx, int ny, int nz);   // z planes per CTA
+int tiled_num_blocks(int nx, int ny, int nz, bool diag = false);   // the DIAG instantiation has its own tile height
+int tiled_chunk(int nx, int ny, int nz, bool diag = false);        // z planes per CTA
 // after a tiled step: redo it with the site kernel iff *flag != 0; clears *clear (the next step's flag)
 cudaError_t launch_site_redo(const int *flag, int *clear, const ConstFields<float> &in, const Fields<float> &out,
                              const StepCoef<float> &k, int nx, int ny, int nz, cudaStream_t st);

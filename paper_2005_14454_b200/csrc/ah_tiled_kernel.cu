@@ -136,11 +136,16 @@ struct Smem {
     float raw[NST][NRAW][TY + 2][ROWF];   // staged planes; row r <-> y0 - 1 + r, column c <-> x0 - HALO + c
     float qe[TY][NRAW][TILE_X];           // staged old Pi, ep of the own rows (one plane): pi_re, pi_im, ep_x, ep_y, ep_z
     // y hand-over: (b_y.re, b_y.im, S_xy, S_yz); row 0 = halo row y0-1, row w+1 from warp w.  Double buffered
-    // (one barrier per plane); the DIAG instantiation has a second barrier per plane anyway and gives the
-    // space to the site phases below
-    float4 row[DIAG ? 1 : 2][TY][4][32];
-    // DIAG: alpha = Arg(phi) (diag_site.cuh) of the staged rows 1 .. TY+1 of the own and the forward plane
-    float alpha[DIAG ? 2 : 1][DIAG ? TY + 1 : 1][DIAG ? ROWF : 4];
+    // (one barrier per plane).  DIAG: after warp w has consumed row w of a buffer it re-uses the first 128 floats
+    // of that row as scratch (the sites' gradient energies, handed from the step to the read-out loop)
+    float4 row[2][TY][4][32];
+    // DIAG: alpha = Arg(phi) (ah_diag_site.cuh) of the staged rows 1 .. TY+1 (columns HALO .. HALO+128) of the
+    // plane held by the ring slot of the same index
+    float alpha[DIAG ? NST : 1][DIAG ? TY + 1 : 1][DIAG ? ROWF : 4];
+    // DIAG: per-thread partial sums of the main warps, parked here between read-out loops so that they do not
+    // occupy registers during the step's arithmetic
+    double dacc[DIAG ? DS_NFLT : 1][DIAG ? TY * 32 : 1];
+    int dcnt[DIAG ? DS_NINT : 1][DIAG ? TY * 32 : 1];
     float4 col[2][TY];                    // x hand-over of the site x0-1: (b_x.re, b_x.im, S_xy, S_xz)
     unsigned long long full[NST];         // a staged phi, th plane has landed
     unsigned long long qfull[TY];         // a warp's Pi, ep row has landed
@@ -158,14 +163,22 @@ namespace {
 #define AH_TILED_TH_LIMIT 65536.0f
 
 // DIAG = true (SURVEY 8(a) row D-fuse): the same step, plus the read-outs D1-D3 of the ENTRY snapshot of every
-// site.  They are fed by what the step holds for the site anyway — own phi, th and the forward neighbours' in
-// registers, the plaquette angles before their sines are taken, the forward hops, the staged Pi, ep row — plus
-// a shared-memory table of site phases alpha = Arg(phi) (one polynomial atan2 per staged site) from which the
-// nine link phases of a site's three plaquettes are wrapped differences (ah_diag_site.cuh).  Everything is read
-// as 128-bit rows, four sites per thread like the step itself.  The only extra global reads are the backward
-// ep_y row (ep_z of the plane below is carried in registers, ep_x of the left neighbour comes by shuffle).
-// Per-thread partial sums (int32 counts, fp64 sums) are reduced per CTA into partials[linear CTA index];
-// diag_final_kernel adds them in a fixed order.
+// site, evaluated in a separate, ROLLED loop at the end of each plane's iteration (after the outputs of the
+// plane have been stored, when nothing of the step's arithmetic is live any more):
+//   * phase 1 additionally computes the site phases alpha = Arg(phi) (one polynomial atan2 per staged site) of
+//     the forward plane into a 3-plane ring in shared memory, and the step's own forward hops give each site's
+//     gradient energy, which is handed over through a scratch row;
+//   * the read-out loop gives lane l the sites l, l+32, l+64, l+96 of the warp's row (NOT the step's 4l .. 4l+3),
+//     so that every scalar it needs — phi, th of the site and its forward neighbours, the seven site phases,
+//     the staged Pi, ep, the gradient energy — is a conflict-free shared-memory read; the nine link phases of the
+//     site's three plaquettes are wrapped differences of site phases (ah_diag_site.cuh);
+//   * both staged planes the read-outs use (own and forward) must therefore survive phase 2: the ring slot of
+//     the plane below is refilled after the CTA barrier instead of before it (the longer iteration of a
+//     diagnostic step leaves the copy ample time), and the warp's Pi, ep row is refilled after the loop;
+//   * the only extra global reads are the backward neighbours ep_y(x-y), ep_z(x-z) (coalesced rows, L2 hits)
+//     and one ep_x per row.
+// Per-thread partial sums (int32 counts, fp64 sums) live in shared memory between loops, are reduced per CTA
+// into partials[linear CTA index]; diag_final_kernel adds them in a fixed order.
 template <int TY, bool COMPACT, bool DIAG>
 __global__ void __launch_bounds__((TY + 1) * 32, ((TY + 1) * 32 <= 256) ? 2 : 1)
 tiled_step_kernel(ConstFields<float> in, Fields<float> out, StepCoef<float> k, int nx, int ny, int nz, int zc,
@@ -280,17 +293,19 @@ tiled_step_kernel(ConstFields<float> in, Fields<float> out, StepCoef<float> k, i
     // ---- helper-warp geometry: halo row (staged row 0) and halo column x0-1 (staged column HALO-1)
     const bool col_act = !is_main && lane < TY;
 
-    // DIAG: site phases of this warp's staged row (helper: halo row TY+1) of the plane in `slot` -> sm.alpha[ab]
-    auto stage_alpha = [&](int slot, int ab) {
+    // DIAG: site phases of this warp's staged row (helper: halo row TY+1, and the column x0+128 of every row) of
+    // the plane in ring slot `slot` -> sm.alpha[slot].  Lane l takes columns l, l+32, ... (conflict-free).
+    auto stage_alpha = [&](int slot) {
         if constexpr (DIAG) {
             const int r = is_main ? w + 1 : TY + 1;
-            const V4 pr = lds4(&sm.raw[slot][0][r][cofs]), pi = lds4(&sm.raw[slot][1][r][cofs]);
-            V4 al;
 #pragma unroll
-            for (int j = 0; j < 4; ++j) al.v[j] = site_phase_fast(pr.v[j], pi.v[j]);
-            *reinterpret_cast<float4 *>(&sm.alpha[ab][r - 1][cofs]) = f4(al);
-            if (lane == 31)
-                sm.alpha[ab][r - 1][cofs + 4] = site_phase_fast(sm.raw[slot][0][r][cofs + 4], sm.raw[slot][1][r][cofs + 4]);
+            for (int j = 0; j < 4; ++j) {
+                const int c = HALO + lane + 32 * j;
+                sm.alpha[slot][r - 1][c] = site_phase_fast(sm.raw[slot][0][r][c], sm.raw[slot][1][r][c]);
+            }
+            if (!is_main && lane <= TY)
+                sm.alpha[slot][lane][HALO + TILE_X] =
+                    site_phase_fast(sm.raw[slot][0][lane + 1][HALO + TILE_X], sm.raw[slot][1][lane + 1][HALO + TILE_X]);
         }
     };
 
@@ -327,20 +342,17 @@ tiled_step_kernel(ConstFields<float> in, Fields<float> out, StepCoef<float> k, i
             g_syz.v[j] = syz;
         }
     }
-    stage_alpha(1, 0);
+    stage_alpha(1);
     __syncthreads();   // slot 0 (load 0) is free from here on
 
     int sf = 1, sf_par = 0;                           // slot and mbarrier parity of the forward plane (load n + 1)
-    int af = 0;                                       // DIAG: sm.alpha buffer of the forward plane
     size_t oc = (size_t)z0 * sxy + ro - sxy;          // this thread's element offset in plane z0 + n - 1
-    int d_cnt[DS_NINT] = {0, 0, 0, 0, 0};            // DIAG only: this thread's partial read-outs (a chunk of
-    double d_acc[DS_NFLT] = {0, 0, 0, 0, 0, 0, 0};   // <= 64 planes x 4 sites x 3 plaquettes fits int32)
-    V4 eb_z;                                         // DIAG only: ep_z of the own sites in the plane below
     if constexpr (DIAG) {
-        if (act) {
-            const int zb = (z0 == 0) ? nz - 1 : z0 - 1;
-            const float4 t = __ldg(reinterpret_cast<const float4 *>(in.f[EP_Z] + (size_t)zb * sxy + ro));
-            eb_z.v[0] = t.x; eb_z.v[1] = t.y; eb_z.v[2] = t.z; eb_z.v[3] = t.w;
+        if (is_main) {
+#pragma unroll
+            for (int a = 0; a < DS_NFLT; ++a) sm.dacc[a][threadIdx.x] = 0.0;
+#pragma unroll
+            for (int a = 0; a < DS_NINT; ++a) sm.dcnt[a][threadIdx.x] = 0;
         }
     }
 
@@ -348,21 +360,19 @@ tiled_step_kernel(ConstFields<float> in, Fields<float> out, StepCoef<float> k, i
     // One __syncthreads per plane separates phase 1 (hand-overs written, staged planes read) from phase 2 (hand-overs
     // consumed, outputs stored); the three roles run separate loops with the same barrier count.
     // Re-use of a ring slot: the slot of load n+2 held plane n-1, last read in phase 1 of iteration n-1, i.e. before
-    // the barrier that every warp has passed when it issues its copies at the top of iteration n.
+    // the barrier that every warp has passed when it issues its copies at the top of iteration n.  DIAG reads the
+    // planes n and n+1 in phase 2 as well (read-out loop), so there the copies of load n+2 are issued right after
+    // the barrier of iteration n instead.
     // (A warp-to-warp mbarrier protocol without the CTA barrier was measured 15 % slower and removed.)
     if (!is_main) {
 #pragma unroll 1
         for (int n = 1; n <= nplanes; ++n) {
-            const int buf = DIAG ? 0 : (n & 1);
+            const int buf = n & 1;
             const int so = sf;
             if (++sf == NST) { sf = 0; sf_par ^= 1; }
-            if (n + 2 <= nplanes + 1) produce();
+            if (!DIAG && n + 2 <= nplanes + 1) produce();
             mbar_wait(&sm.full[sf], sf_par);
-            if constexpr (DIAG) {
-                af ^= 1;
-                stage_alpha(sf, af);
-                __syncthreads();
-            }
+            stage_alpha(sf);
             // helper: shared quantities of the halo row y0-1 (staged row 0) at this plane
             const V4 h_pr = lds4(&sm.raw[so][0][0][cofs]), h_pi = lds4(&sm.raw[so][1][0][cofs]);
             const V4 h_tx = lds4(&sm.raw[so][2][0][cofs]), h_ty = lds4(&sm.raw[so][3][0][cofs]);
@@ -403,46 +413,42 @@ tiled_step_kernel(ConstFields<float> in, Fields<float> out, StepCoef<float> k, i
                 sm.col[buf][lane] = make_float4(c * pr - s * pi, c * pi + s * pr, sxy_, sxz_);
             }
             __syncthreads();
+            if (DIAG && n + 2 <= nplanes + 1) produce();
         }
     } else if (!act) {
         // a row beyond ny (ragged last tile): keeps the protocol going, computes nothing
 #pragma unroll 1
         for (int n = 1; n <= nplanes; ++n) {
-            if (n + 2 <= nplanes + 1) produce();
+            if (!DIAG && n + 2 <= nplanes + 1) produce();
             if constexpr (DIAG) {   // the row above the last active one is this warp's (periodic wrap): its phases are needed
                 if (++sf == NST) { sf = 0; sf_par ^= 1; }
                 mbar_wait(&sm.full[sf], sf_par);
-                af ^= 1;
-                stage_alpha(sf, af);
-                __syncthreads();
+                stage_alpha(sf);
             }
             __syncthreads();
+            if (DIAG && n + 2 <= nplanes + 1) produce();
         }
     } else {
 #pragma unroll 1
         for (int n = 1; n <= nplanes; ++n) {
-            const int buf = DIAG ? 0 : (n & 1);
+            const int buf = n & 1;
             const int so = sf;
             if (++sf == NST) { sf = 0; sf_par ^= 1; }
             oc += sxy;
             V4 P_r, P_i, E_x, E_y, E_z;   // Pi+, ep+ still lacking the old Pi, ep and the terms from row y-1 / site x0-1
-            if (n + 2 <= nplanes + 1) produce();
-            mbar_wait(&sm.full[sf], sf_par);
-            float4 eb_y4 = make_float4(0.f, 0.f, 0.f, 0.f);
-            float eb_x0 = 0.f;
+            if (!DIAG && n + 2 <= nplanes + 1) produce();
+            // DIAG: the backward ep neighbours that are not on chip (row y-1 of this plane, this row of the plane
+            // below, and - lane 0 - the site x0-1), requested a whole phase before the read-out loop needs them
+            float4 d_eby = make_float4(0.f, 0.f, 0.f, 0.f), d_ebz = d_eby;
+            float d_exl = 0.f;
             if constexpr (DIAG) {
-                // site phases of the forward plane, shared by every link phase that needs them
-                af ^= 1;
-                stage_alpha(sf, af);
-                // backward ep neighbours that are not on chip: the row y-1 of this plane, and (lane 0) the site x0-1
-                const int z = z0 + n - 1, ym = (y == 0) ? ny - 1 : y - 1;
-                eb_y4 = __ldg(reinterpret_cast<const float4 *>(in.f[EP_Y] + (size_t)z * sxy + (size_t)ym * nx + x0 + 4 * lane));
-                if (lane == 0) {
-                    const int xw = (x0 == 0) ? nx - 1 : x0 - 1;
-                    eb_x0 = __ldg(in.f[EP_X] + (size_t)z * sxy + (size_t)y * nx + xw);
-                }
-                __syncthreads();
+                const int z = z0 + n - 1, zm = (z == 0) ? nz - 1 : z - 1, ym = (y == 0) ? ny - 1 : y - 1;
+                d_eby = __ldg(reinterpret_cast<const float4 *>(in.f[EP_Y] + (size_t)z * sxy + (size_t)ym * nx + x0 + 4 * lane));
+                d_ebz = __ldg(reinterpret_cast<const float4 *>(in.f[EP_Z] + (size_t)zm * sxy + ro));
+                if (lane == 0) d_exl = __ldg(in.f[EP_X] + (size_t)z * sxy + (size_t)y * nx + ((x0 == 0) ? nx - 1 : x0 - 1));
             }
+            mbar_wait(&sm.full[sf], sf_par);
+            stage_alpha(sf);   // DIAG: site phases of the forward plane
             V4 o_byr, o_byi, o_sxy, o_syz;   // for row y+1, through shared memory
             V4 h_bzr, h_bzi, h_sxz;          // this plane's hand-down to z+1 (with S_yz in o_syz)
             float l_bxr = 0.f, l_bxi = 0.f, l_sxy = 0.f, l_sxz = 0.f;   // from the site to the left
@@ -470,38 +476,6 @@ tiled_step_kernel(ConstFields<float> in, Fields<float> out, StepCoef<float> k, i
                 S_xz.v[j] = plaq_angle_f32(c_tx.v[j], tz_xp, n_tx.v[j], c_tz.v[j]);
                 S_yz.v[j] = plaq_angle_f32(c_ty.v[j], y_tz.v[j], n_ty.v[j], c_tz.v[j]);
                 amax = fmaxf(amax, fmaxf(fmaxf(fabsf(S_xy.v[j]), fabsf(S_xz.v[j])), fabsf(S_yz.v[j])));
-            }
-            V4 d_b2;   // DIAG: magnetic energy of the three plaquettes each site owns
-            if constexpr (DIAG) {
-                // D1 (winding, Eq. 16 right) from the site phases, and the plaquette energies, while the angles are
-                // still angles
-                const int ao = af ^ 1;
-                const V4 a_0 = lds4(&sm.alpha[ao][w][cofs]), a_y = lds4(&sm.alpha[ao][w + 1][cofs]);
-                const V4 a_z = lds4(&sm.alpha[af][w][cofs]), a_yz = lds4(&sm.alpha[af][w + 1][cofs]);
-                float a_0r = __shfl_down_sync(FULL, a_0.v[0], 1), a_yr = __shfl_down_sync(FULL, a_y.v[0], 1);
-                float a_zr = __shfl_down_sync(FULL, a_z.v[0], 1);
-                if (lane == 31) {
-                    a_0r = sm.alpha[ao][w][cofs + 4]; a_yr = sm.alpha[ao][w + 1][cofs + 4];
-                    a_zr = sm.alpha[af][w][cofs + 4];
-                }
-#pragma unroll
-                for (int j = 0; j < 4; ++j) {
-                    const int jn = (j < 3) ? j + 1 : 3;
-                    const float ty_xp = (j < 3) ? c_ty.v[jn] : r_ty, tz_xp = (j < 3) ? c_tz.v[jn] : r_tz;
-                    const float ax = (j < 3) ? a_0.v[jn] : a_0r, axy = (j < 3) ? a_y.v[jn] : a_yr;
-                    const float axz = (j < 3) ? a_z.v[jn] : a_zr;
-                    const SiteWinding sw = readout_winding(a_0.v[j], ax, a_y.v[j], a_z.v[j], axy, axz, a_yz.v[j],
-                                                           c_tx.v[j], c_ty.v[j], c_tz.v[j], ty_xp, tz_xp, y_tx.v[j],
-                                                           y_tz.v[j], n_tx.v[j], n_ty.v[j], S_xy.v[j], S_xz.v[j],
-                                                           S_yz.v[j]);
-#pragma unroll
-                    for (int pq = 0; pq < 3; ++pq) {
-                        d_cnt[pq] += abs(sw.w[pq]);
-                        d_cnt[DS_NEAR] += sw.nearf[pq];
-                        d_cnt[DS_BIG] += sw.big[pq];
-                    }
-                    d_b2.v[j] = readout_plaq_energy(S_xy.v[j], S_xz.v[j], S_yz.v[j], COMPACT ? 1 : 0, dk.f_idx4);
-                }
             }
             if (COMPACT) {
                 // two angles per issued instruction (FFMA2); bit-identical to the scalar polynomials
@@ -535,15 +509,7 @@ tiled_step_kernel(ConstFields<float> in, Fields<float> out, StepCoef<float> k, i
                 sincos4(c_ty, s_y, c_y);
                 sincos4(c_tz, s_z, c_z);
             }
-            V4 dq_r, dq_i, dq_ex, dq_ey, dq_ez;   // DIAG: the old Pi, ep of the own sites (read again after the barrier)
-            if constexpr (DIAG) {
-                mbar_wait(&sm.qfull[w], (n - 1) & 1);
-                dq_r = lds4(&sm.qe[w][0][4 * lane]); dq_i = lds4(&sm.qe[w][1][4 * lane]);
-                dq_ex = lds4(&sm.qe[w][2][4 * lane]); dq_ey = lds4(&sm.qe[w][3][4 * lane]);
-                dq_ez = lds4(&sm.qe[w][4][4 * lane]);
-                const float el = __shfl_up_sync(FULL, dq_ex.v[3], 1);   // ep_x of the site to the left of the first one
-                if (lane > 0) eb_x0 = el;
-            }
+            V4 d_g2;   // DIAG: gradient energy of the 4 sites, for the read-out loop
 #pragma unroll
             for (int j = 0; j < 4; ++j) {
                 const float fr = c_pr.v[j], fi = c_pi.v[j];
@@ -562,18 +528,7 @@ tiled_step_kernel(ConstFields<float> in, Fields<float> out, StepCoef<float> k, i
                 hop_bwd_f32(cx, sx, fr, fi, bxr, bxi);
                 hop_bwd_f32(cy, sy, fr, fi, o_byr.v[j], o_byi.v[j]);
                 hop_bwd_f32(cz, sz, fr, fi, h_bzr.v[j], h_bzi.v[j]);
-                if constexpr (DIAG) {
-                    // D2, D3 of the site (Eqs. 17-18, Eq. 5) from the hops just formed and the staged Pi, ep
-                    const float exb = (j == 0) ? eb_x0 : dq_ex.v[j > 0 ? j - 1 : 0];
-                    const float eyb = (j == 0) ? eb_y4.x : (j == 1) ? eb_y4.y : (j == 2) ? eb_y4.z : eb_y4.w;
-                    float pi2L, gr2L, L;
-                    readout_lagrangian(fr, fi, readout_grad2(fr, fi, fxr, fxi, fyr, fyi, fzr, fzi, dk.f_idx2), d_b2.v[j],
-                                       dq_r.v[j], dq_i.v[j], dq_ex.v[j], dq_ey.v[j], dq_ez.v[j], dk, pi2L, gr2L, L);
-                    double G, div, charge;
-                    readout_gauss(fr, fi, dq_r.v[j], dq_i.v[j], dq_ex.v[j], dq_ey.v[j], dq_ez.v[j], exb, eyb,
-                                  eb_z.v[j], dk, G, div, charge);
-                    readout_accumulate(d_acc, pi2L, gr2L, L, G, div, charge);
-                }
+                if constexpr (DIAG) d_g2.v[j] = readout_grad2(fr, fi, fxr, fxi, fyr, fyi, fzr, fzi, dk.f_idx2);
                 o_sxy.v[j] = Sxy; o_syz.v[j] = Syz; h_sxz.v[j] = Sxz;
                 // Eq. 7 without the x-1 (j == 0) and y-1 hops
                 float ar = (fxr + fyr) + (fzr + g_bzr.v[j]) - 6.0f * fr;
@@ -615,6 +570,7 @@ tiled_step_kernel(ConstFields<float> in, Fields<float> out, StepCoef<float> k, i
             // roll the z hand-down
             g_bzr = h_bzr; g_bzi = h_bzi; g_sxz = h_sxz; g_syz = o_syz;
             __syncthreads();
+            if (DIAG && n + 2 <= nplanes + 1) produce();
             // add what row y-1 (and, lane 0, site x0-1) hands over, finish Eqs. 7-10, store
             const float4 a = sm.row[buf][w][0][lane], b = sm.row[buf][w][1][lane];
             const float4 c = sm.row[buf][w][2][lane], d = sm.row[buf][w][3][lane];
@@ -632,7 +588,6 @@ tiled_step_kernel(ConstFields<float> in, Fields<float> out, StepCoef<float> k, i
             const V4 q_r = lds4(&sm.qe[w][0][4 * lane]), q_i = lds4(&sm.qe[w][1][4 * lane]);
             const V4 e_x = lds4(&sm.qe[w][2][4 * lane]), e_y = lds4(&sm.qe[w][3][4 * lane]);
             const V4 e_z = lds4(&sm.qe[w][4][4 * lane]);
-            if constexpr (DIAG) eb_z = e_z;   // the plane below the next one
             V4 f_r, f_i, t_x, t_y, t_z;
 #pragma unroll
             for (int j = 0; j < 4; ++j) {
@@ -648,9 +603,9 @@ tiled_step_kernel(ConstFields<float> in, Fields<float> out, StepCoef<float> k, i
                 t_z.v[j] = c_tz.v[j] + k.dt * E_z.v[j];
             }
             // the staged Pi, ep row has been consumed (its values went through the arithmetic above): refill it
-            // with the next plane's row, which then has almost a whole iteration to land
+            // with the next plane's row, which then has almost a whole iteration to land (DIAG: after the read-outs)
             __syncwarp();
-            if (n + 1 <= nplanes) produce_q();
+            if (!DIAG && n + 1 <= nplanes) produce_q();
             st4(out.f[PI_RE] + oc, P_r);
             st4(out.f[PI_IM] + oc, P_i);
             st4(out.f[EP_X] + oc, E_x);
@@ -661,6 +616,62 @@ tiled_step_kernel(ConstFields<float> in, Fields<float> out, StepCoef<float> k, i
             st4(out.f[TH_X] + oc, t_x);
             st4(out.f[TH_Y] + oc, t_y);
             st4(out.f[TH_Z] + oc, t_z);
+            if constexpr (DIAG) {
+                // ---- read-outs D1-D3 of the entry snapshot of this plane: lane l takes the sites l + 32 j of the row
+                // scratch: this warp's hand-over row, consumed above and free until iteration n + 2: 4 x 128 floats
+                float *scr = reinterpret_cast<float *>(&sm.row[buf][w][0][0]);
+                st4(scr + 4 * lane, d_g2);
+                *reinterpret_cast<float4 *>(scr + TILE_X + 4 * lane) = d_eby;
+                *reinterpret_cast<float4 *>(scr + 2 * TILE_X + 4 * lane) = d_ebz;
+                const float ex_left = d_exl;
+                __syncwarp();
+                int cnt[DS_NINT];
+                double acc[DS_NFLT];
+#pragma unroll
+                for (int a = 0; a < DS_NINT; ++a) cnt[a] = sm.dcnt[a][threadIdx.x];
+#pragma unroll
+                for (int a = 0; a < DS_NFLT; ++a) acc[a] = sm.dacc[a][threadIdx.x];
+#pragma unroll 1
+                for (int j = 0; j < 4; ++j) {
+                    const int cq = lane + 32 * j, c = HALO + cq;
+                    const float eby = scr[TILE_X + cq], ebz = scr[2 * TILE_X + cq];
+                    // D1: winding of the three plaquettes the site owns (Eq. 16 right)
+                    const float t0x = sm.raw[so][2][r_own][c], t0y = sm.raw[so][3][r_own][c], t0z = sm.raw[so][4][r_own][c];
+                    const float ty_xp = sm.raw[so][3][r_own][c + 1], tz_xp = sm.raw[so][4][r_own][c + 1];
+                    const float tx_yp = sm.raw[so][2][r_own + 1][c], tz_yp = sm.raw[so][4][r_own + 1][c];
+                    const float tx_zp = sm.raw[sf][2][r_own][c], ty_zp = sm.raw[sf][3][r_own][c];
+                    const float Pxy = plaq_angle_f32(t0x, ty_xp, tx_yp, t0y), Pxz = plaq_angle_f32(t0x, tz_xp, tx_zp, t0z);
+                    const float Pyz = plaq_angle_f32(t0y, tz_yp, ty_zp, t0z);
+                    const SiteWinding sw = readout_winding(
+                        sm.alpha[so][w][c], sm.alpha[so][w][c + 1], sm.alpha[so][w + 1][c], sm.alpha[sf][w][c],
+                        sm.alpha[so][w + 1][c + 1], sm.alpha[sf][w][c + 1], sm.alpha[sf][w + 1][c], t0x, t0y, t0z, ty_xp,
+                        tz_xp, tx_yp, tz_yp, tx_zp, ty_zp, Pxy, Pxz, Pyz);
+#pragma unroll
+                    for (int pq = 0; pq < 3; ++pq) {
+                        cnt[pq] += abs(sw.w[pq]);
+                        cnt[DS_NEAR] += sw.nearf[pq];
+                        cnt[DS_BIG] += sw.big[pq];
+                    }
+                    // D2, D3 (Eqs. 17-18, Eq. 5) from the staged phi, Pi, ep and the step's gradient energy
+                    const float fr = sm.raw[so][0][r_own][c], fi = sm.raw[so][1][r_own][c];
+                    const float pir = sm.qe[w][0][cq], pii = sm.qe[w][1][cq];
+                    const float ex = sm.qe[w][2][cq], ey = sm.qe[w][3][cq], ez = sm.qe[w][4][cq];
+                    const float exl = sm.qe[w][2][cq > 0 ? cq - 1 : 0];
+                    const float exb = (cq == 0) ? ex_left : exl;
+                    float pi2L, gr2L, L;
+                    readout_lagrangian(fr, fi, scr[cq], readout_plaq_energy(Pxy, Pxz, Pyz, COMPACT ? 1 : 0, dk.f_idx4), pir,
+                                       pii, ex, ey, ez, dk, pi2L, gr2L, L);
+                    double G, div, charge;
+                    readout_gauss(fr, fi, pir, pii, ex, ey, ez, exb, eby, ebz, dk, G, div, charge);
+                    readout_accumulate(acc, pi2L, gr2L, L, G, div, charge);
+                }
+#pragma unroll
+                for (int a = 0; a < DS_NINT; ++a) sm.dcnt[a][threadIdx.x] = cnt[a];
+#pragma unroll
+                for (int a = 0; a < DS_NFLT; ++a) sm.dacc[a][threadIdx.x] = acc[a];
+                __syncwarp();   // every lane is done with the staged Pi, ep row
+                if (n + 1 <= nplanes) produce_q();
+            }
             // the forward plane becomes the own plane
             c_pr = lds4(&sm.raw[sf][0][r_own][cofs]); c_pi = lds4(&sm.raw[sf][1][r_own][cofs]);
             c_tx = lds4(&sm.raw[sf][2][r_own][cofs]); c_ty = lds4(&sm.raw[sf][3][r_own][cofs]);
@@ -677,6 +688,14 @@ tiled_step_kernel(ConstFields<float> in, Fields<float> out, StepCoef<float> k, i
 
     if constexpr (DIAG) {
         // CTA reduction: warp shuffles, then the warps through shared memory (the hand-over rows are free now)
+        int d_cnt[DS_NINT] = {0, 0, 0, 0, 0};
+        double d_acc[DS_NFLT] = {0, 0, 0, 0, 0, 0, 0};
+        if (is_main) {
+#pragma unroll
+            for (int a = 0; a < DS_NINT; ++a) d_cnt[a] = sm.dcnt[a][threadIdx.x];
+#pragma unroll
+            for (int a = 0; a < DS_NFLT; ++a) d_acc[a] = sm.dacc[a][threadIdx.x];
+        }
         __syncthreads();
         double *s_f = reinterpret_cast<double *>(&sm.row[0][0][0][0]);       // [TY + 1][DS_NFLT]
         long long *s_i = reinterpret_cast<long long *>(s_f + (TY + 1) * DS_NFLT);   // [TY + 1][DS_NINT]
@@ -714,26 +733,27 @@ tiled_step_kernel(ConstFields<float> in, Fields<float> out, StepCoef<float> k, i
 
 // --------------------------------------------------------------------------------- launch
 
-constexpr int TILE_Y = 6;    // 6 main warps + 1 helper = 224 threads, 2 CTAs per SM (106 KB shared memory each)
+constexpr int TILE_Y = 6;        // plain step: 6 main warps + 1 helper = 224 threads, 2 CTAs per SM (106 KB shared memory each)
+constexpr int TILE_Y_DIAG = 5;   // fused read-outs: the site-phase ring and the parked partial sums take the room of one row
 
 bool tiled_supported(int nx, int ny, int nz) { return nx >= TILE_X && nx % TILE_X == 0 && ny >= 1 && nz >= 1; }
 
-template <bool COMPACT, bool DIAG>
+template <int TY, bool COMPACT, bool DIAG>
 static cudaError_t setup_one()
 {
-    cudaError_t e = cudaFuncSetAttribute(tiled_step_kernel<TILE_Y, COMPACT, DIAG>,
-                                         cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Smem<TILE_Y, DIAG>));
+    cudaError_t e = cudaFuncSetAttribute(tiled_step_kernel<TY, COMPACT, DIAG>,
+                                         cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Smem<TY, DIAG>));
     if (e != cudaSuccess) return e;
-    return cudaFuncSetAttribute(tiled_step_kernel<TILE_Y, COMPACT, DIAG>,
+    return cudaFuncSetAttribute(tiled_step_kernel<TY, COMPACT, DIAG>,
                                 cudaFuncAttributePreferredSharedMemoryCarveout, 100);
 }
 
 cudaError_t tiled_setup()
 {
-    cudaError_t e = setup_one<true, false>();
-    if (e == cudaSuccess) e = setup_one<false, false>();
-    if (e == cudaSuccess) e = setup_one<true, true>();
-    if (e == cudaSuccess) e = setup_one<false, true>();
+    cudaError_t e = setup_one<TILE_Y, true, false>();
+    if (e == cudaSuccess) e = setup_one<TILE_Y, false, false>();
+    if (e == cudaSuccess) e = setup_one<TILE_Y_DIAG, true, true>();
+    if (e == cudaSuccess) e = setup_one<TILE_Y_DIAG, false, true>();
     return e;
 }
 
@@ -748,9 +768,9 @@ cudaError_t tiled_setup()
 #ifndef AH_ZC_MAX
 #define AH_ZC_MAX 64
 #endif
-int tiled_chunk(int nx, int ny, int nz)
+static int chunk_for(int nx, int ny, int nz, int ty)
 {
-    const long long cols = (long long)(nx / TILE_X) * ((ny + TILE_Y - 1) / TILE_Y);
+    const long long cols = (long long)(nx / TILE_X) * ((ny + ty - 1) / ty);
     const long long resident = 148LL * 2;
     int best = nz < 8 ? nz : 8;
     double best_cost = 1e300;
@@ -770,39 +790,43 @@ int tiled_chunk(int nx, int ny, int nz)
     return best;
 }
 
-int tiled_num_blocks(int nx, int ny, int nz)
+int tiled_chunk(int nx, int ny, int nz, bool diag) { return chunk_for(nx, ny, nz, diag ? TILE_Y_DIAG : TILE_Y); }
+
+int tiled_num_blocks(int nx, int ny, int nz, bool diag)
 {
     if (!tiled_supported(nx, ny, nz)) return 0;
-    const int zc = tiled_chunk(nx, ny, nz);
-    return (nx / TILE_X) * ((ny + TILE_Y - 1) / TILE_Y) * ((nz + zc - 1) / zc);
+    const int ty = diag ? TILE_Y_DIAG : TILE_Y;
+    const int zc = chunk_for(nx, ny, nz, ty);
+    return (nx / TILE_X) * ((ny + ty - 1) / ty) * ((nz + zc - 1) / zc);
+}
+
+template <int TY, bool COMPACT, bool DIAG>
+static cudaError_t launch_one(const ConstFields<float> &in, const Fields<float> &out, const StepCoef<float> &k, int nx,
+                              int ny, int nz, int *overflow, cudaStream_t st, const DiagCoef &d, DiagPartial *partials)
+{
+    const int zc = chunk_for(nx, ny, nz, TY);
+    dim3 grid(nx / TILE_X, (ny + TY - 1) / TY, (nz + zc - 1) / zc);
+    dim3 block((TY + 1) * 32);
+    if (grid.y > 65535u || grid.z > 65535u) return cudaErrorInvalidConfiguration;
+    tiled_step_kernel<TY, COMPACT, DIAG><<<grid, block, sizeof(Smem<TY, DIAG>), st>>>(in, out, k, nx, ny, nz, zc, overflow,
+                                                                                    d, partials);
+    return cudaGetLastError();
 }
 
 // partials == nullptr: plain step.  Otherwise the DIAG instantiation, which also writes one DiagPartial per
-// CTA (tiled_num_blocks of them) holding the read-outs of the entry snapshot.
+// CTA (tiled_num_blocks(.., true) of them) holding the read-outs of the entry snapshot.
 cudaError_t launch_tiled_step(const ConstFields<float> &in, const Fields<float> &out,
                               const StepCoef<float> &k, int nx, int ny, int nz, int *overflow, cudaStream_t st,
                               const DiagCoef *dk, DiagPartial *partials)
 {
     if (!tiled_supported(nx, ny, nz)) return cudaErrorInvalidValue;
-    const int zc = tiled_chunk(nx, ny, nz);
-    dim3 grid(nx / TILE_X, (ny + TILE_Y - 1) / TILE_Y, (nz + zc - 1) / zc);
-    dim3 block((TILE_Y + 1) * 32);
-    if (grid.y > 65535u || grid.z > 65535u) return cudaErrorInvalidConfiguration;
     const bool diag = partials != nullptr && dk != nullptr;
-    const size_t smem = diag ? sizeof(Smem<TILE_Y, true>) : sizeof(Smem<TILE_Y, false>);
     const DiagCoef d = diag ? *dk : DiagCoef{};
-    if (k.compact) {
-        if (diag)
-            tiled_step_kernel<TILE_Y, true, true><<<grid, block, smem, st>>>(in, out, k, nx, ny, nz, zc, overflow, d, partials);
-        else
-            tiled_step_kernel<TILE_Y, true, false><<<grid, block, smem, st>>>(in, out, k, nx, ny, nz, zc, overflow, d, nullptr);
-    } else {
-        if (diag)
-            tiled_step_kernel<TILE_Y, false, true><<<grid, block, smem, st>>>(in, out, k, nx, ny, nz, zc, overflow, d, partials);
-        else
-            tiled_step_kernel<TILE_Y, false, false><<<grid, block, smem, st>>>(in, out, k, nx, ny, nz, zc, overflow, d, nullptr);
-    }
-    return cudaGetLastError();
+    if (k.compact)
+        return diag ? launch_one<TILE_Y_DIAG, true, true>(in, out, k, nx, ny, nz, overflow, st, d, partials)
+                    : launch_one<TILE_Y, true, false>(in, out, k, nx, ny, nz, overflow, st, d, nullptr);
+    return diag ? launch_one<TILE_Y_DIAG, false, true>(in, out, k, nx, ny, nz, overflow, st, d, partials)
+                : launch_one<TILE_Y, false, false>(in, out, k, nx, ny, nz, overflow, st, d, nullptr);
 }
 
 }  // namespace ah
