@@ -227,19 +227,40 @@ __device__ __forceinline__ float wrap_2pi_fix(float y)
     const float r = __fmaf_rn(k, -6.2831854820251465f, y);    // fl32(2 pi)
     return __fmaf_rn(k, 1.7484555314695172e-07f, r);          // fl32(2 pi - fl32(2 pi)) (negative)
 }
-// d = principal value of alpha_head - alpha_tail - th; 0 when either end has no phase.  |th| < 2^16.
-__device__ __forceinline__ float link_phase_fix(float a_tail, float a_head, float th)
+// d = principal value of alpha_head - alpha_tail - th (|th| < 2^16); NaN when either end has no phase
+__device__ __forceinline__ float link_phase_raw(float a_tail, float a_head, float th)
 {
-    const float y = __fadd_rn(__fadd_rn(a_head, -a_tail), -wrap_2pi_fix(th));
-    const float d = wrap_2pi_fix(y);
-    return (y == y) ? d : 0.0f;
+    return wrap_2pi_fix(__fadd_rn(__fadd_rn(a_head, -a_tail), -wrap_2pi_fix(th)));
 }
 
 struct SiteWinding {
-    int w[3];       // W_xy, W_xz, W_yz
+    float absw[3];  // |W_xy|, |W_xz|, |W_yz| as exact small integers in fp32
+    int w[3];       // the signed integers (dead code unless the caller uses them)
     int nearf[3];   // any of the four link phases within 1e-5 of +-pi
     int big[3];     // |Phi_ij| > pi - 1e-5
 };
+
+// one plaquette: W = rint{[d1 + d2 - d3 - d4 + Phi] / 2 pi} (Eq. 16 right, reading #13).  A link that touches a
+// site without a phase (phi == 0 exactly) has d = NaN here and counts as d = 0 (the oracle's atan2(0,0) := 0):
+// fmaxf drops NaNs from the near-branch test by itself, and the sum is redone with zeros only when it is NaN.
+__device__ __forceinline__ void plaquette_winding(float d1, float d2, float d3, float d4, float Phi, float &absw, int &w,
+                                                  int &nearf, int &big)
+{
+    const float lim = 3.14159274101257324f - 1e-5f;
+    const float inv2pi = 0.15915494309189533577f;
+    const float magic = 12582912.0f;   // 1.5 * 2^23
+    float sum = __fadd_rn(__fadd_rn(__fadd_rn(__fadd_rn(d1, d2), -d3), -d4), Phi);
+    if (sum != sum) {
+        d1 = (d1 == d1) ? d1 : 0.0f; d2 = (d2 == d2) ? d2 : 0.0f;
+        d3 = (d3 == d3) ? d3 : 0.0f; d4 = (d4 == d4) ? d4 : 0.0f;
+        sum = __fadd_rn(__fadd_rn(__fadd_rn(__fadd_rn(d1, d2), -d3), -d4), Phi);
+    }
+    const float wf = __fadd_rn(__fmaf_rn(sum, inv2pi, magic), -magic);   // rint(sum / 2 pi), |.| < 2^22
+    absw = fabsf(wf);
+    w = (int)wf;
+    nearf = fmaxf(fmaxf(fabsf(d1), fabsf(d2)), fmaxf(fabsf(d3), fabsf(d4))) >= lim;
+    big = fabsf(Phi) > lim;
+}
 
 // D1 of one site.  a0 = alpha(x); ax, ay, az = alpha(x+i); axy, axz, ayz = alpha(x+i+j);
 // t0* = th_*(x); t{j}_{i}p = th_j(x+i); P* = Phi_ij(x) (plaq_angle_f32).
@@ -248,31 +269,17 @@ __device__ __forceinline__ SiteWinding readout_winding(float a0, float ax, float
                                                        float tz_xp, float tx_yp, float tz_yp, float tx_zp,
                                                        float ty_zp, float Pxy, float Pxz, float Pyz)
 {
-    const float lim = 3.14159274101257324f - 1e-5f;
-    const float inv2pi = 0.15915494309189533577f;
-    const float dx0 = link_phase_fix(a0, ax, t0x), dy0 = link_phase_fix(a0, ay, t0y), dz0 = link_phase_fix(a0, az, t0z);
+    const float dx0 = link_phase_raw(a0, ax, t0x), dy0 = link_phase_raw(a0, ay, t0y), dz0 = link_phase_raw(a0, az, t0z);
     SiteWinding r;
-    {   // xy: d_x(x) + d_y(x+x) - d_x(x+y) - d_y(x)
-        const float d2 = link_phase_fix(ax, axy, ty_xp), d3 = link_phase_fix(ay, axy, tx_yp);
-        const float sum = __fadd_rn(__fadd_rn(__fadd_rn(__fadd_rn(dx0, d2), -d3), -dy0), Pxy);
-        r.w[0] = __float2int_rn(__fmul_rn(sum, inv2pi));
-        r.nearf[0] = fmaxf(fmaxf(fabsf(dx0), fabsf(d2)), fmaxf(fabsf(d3), fabsf(dy0))) >= lim;
-        r.big[0] = fabsf(Pxy) > lim;
-    }
-    {   // xz: d_x(x) + d_z(x+x) - d_x(x+z) - d_z(x)
-        const float d2 = link_phase_fix(ax, axz, tz_xp), d3 = link_phase_fix(az, axz, tx_zp);
-        const float sum = __fadd_rn(__fadd_rn(__fadd_rn(__fadd_rn(dx0, d2), -d3), -dz0), Pxz);
-        r.w[1] = __float2int_rn(__fmul_rn(sum, inv2pi));
-        r.nearf[1] = fmaxf(fmaxf(fabsf(dx0), fabsf(d2)), fmaxf(fabsf(d3), fabsf(dz0))) >= lim;
-        r.big[1] = fabsf(Pxz) > lim;
-    }
-    {   // yz: d_y(x) + d_z(x+y) - d_y(x+z) - d_z(x)
-        const float d2 = link_phase_fix(ay, ayz, tz_yp), d3 = link_phase_fix(az, ayz, ty_zp);
-        const float sum = __fadd_rn(__fadd_rn(__fadd_rn(__fadd_rn(dy0, d2), -d3), -dz0), Pyz);
-        r.w[2] = __float2int_rn(__fmul_rn(sum, inv2pi));
-        r.nearf[2] = fmaxf(fmaxf(fabsf(dy0), fabsf(d2)), fmaxf(fabsf(d3), fabsf(dz0))) >= lim;
-        r.big[2] = fabsf(Pyz) > lim;
-    }
+    // xy: d_x(x) + d_y(x+x) - d_x(x+y) - d_y(x)
+    plaquette_winding(dx0, link_phase_raw(ax, axy, ty_xp), link_phase_raw(ay, axy, tx_yp), dy0, Pxy, r.absw[0], r.w[0],
+                      r.nearf[0], r.big[0]);
+    // xz: d_x(x) + d_z(x+x) - d_x(x+z) - d_z(x)
+    plaquette_winding(dx0, link_phase_raw(ax, axz, tz_xp), link_phase_raw(az, axz, tx_zp), dz0, Pxz, r.absw[1], r.w[1],
+                      r.nearf[1], r.big[1]);
+    // yz: d_y(x) + d_z(x+y) - d_y(x+z) - d_z(x)
+    plaquette_winding(dy0, link_phase_raw(ay, ayz, tz_yp), link_phase_raw(az, ayz, ty_zp), dz0, Pyz, r.absw[2], r.w[2],
+                      r.nearf[2], r.big[2]);
     return r;
 }
 

@@ -145,7 +145,8 @@ struct Smem {
     // DIAG: per-thread partial sums of the main warps, parked here between read-out loops so that they do not
     // occupy registers during the step's arithmetic
     double dacc[DIAG ? DS_NFLT : 1][DIAG ? TY * 32 : 1];
-    int dcnt[DIAG ? DS_NINT : 1][DIAG ? TY * 32 : 1];
+    float dwnd[DIAG ? 3 : 1][DIAG ? TY * 32 : 1];   // |W| sums: exact integers in fp32 (<= 64 planes x 4 sites x |W|)
+    int dflg[DIAG ? 2 : 1][DIAG ? TY * 32 : 1];     // near-branch and big-plaquette counts
     float4 col[2][TY];                    // x hand-over of the site x0-1: (b_x.re, b_x.im, S_xy, S_xz)
     unsigned long long full[NST];         // a staged phi, th plane has landed
     unsigned long long qfull[TY];         // a warp's Pi, ep row has landed
@@ -352,7 +353,8 @@ tiled_step_kernel(ConstFields<float> in, Fields<float> out, StepCoef<float> k, i
 #pragma unroll
             for (int a = 0; a < DS_NFLT; ++a) sm.dacc[a][threadIdx.x] = 0.0;
 #pragma unroll
-            for (int a = 0; a < DS_NINT; ++a) sm.dcnt[a][threadIdx.x] = 0;
+            for (int a = 0; a < 3; ++a) sm.dwnd[a][threadIdx.x] = 0.0f;
+            sm.dflg[0][threadIdx.x] = sm.dflg[1][threadIdx.x] = 0;
         }
     }
 
@@ -625,10 +627,11 @@ tiled_step_kernel(ConstFields<float> in, Fields<float> out, StepCoef<float> k, i
                 *reinterpret_cast<float4 *>(scr + 2 * TILE_X + 4 * lane) = d_ebz;
                 const float ex_left = d_exl;
                 __syncwarp();
-                int cnt[DS_NINT];
+                float wnd[3];
+                int n_near = sm.dflg[0][threadIdx.x], n_big = sm.dflg[1][threadIdx.x];
                 double acc[DS_NFLT];
 #pragma unroll
-                for (int a = 0; a < DS_NINT; ++a) cnt[a] = sm.dcnt[a][threadIdx.x];
+                for (int a = 0; a < 3; ++a) wnd[a] = sm.dwnd[a][threadIdx.x];
 #pragma unroll
                 for (int a = 0; a < DS_NFLT; ++a) acc[a] = sm.dacc[a][threadIdx.x];
 #pragma unroll 1
@@ -648,9 +651,9 @@ tiled_step_kernel(ConstFields<float> in, Fields<float> out, StepCoef<float> k, i
                         tz_xp, tx_yp, tz_yp, tx_zp, ty_zp, Pxy, Pxz, Pyz);
 #pragma unroll
                     for (int pq = 0; pq < 3; ++pq) {
-                        cnt[pq] += abs(sw.w[pq]);
-                        cnt[DS_NEAR] += sw.nearf[pq];
-                        cnt[DS_BIG] += sw.big[pq];
+                        wnd[pq] += sw.absw[pq];
+                        n_near += sw.nearf[pq];
+                        n_big += sw.big[pq];
                     }
                     // D2, D3 (Eqs. 17-18, Eq. 5) from the staged phi, Pi, ep and the step's gradient energy
                     const float fr = sm.raw[so][0][r_own][c], fi = sm.raw[so][1][r_own][c];
@@ -666,7 +669,9 @@ tiled_step_kernel(ConstFields<float> in, Fields<float> out, StepCoef<float> k, i
                     readout_accumulate(acc, pi2L, gr2L, L, G, div, charge);
                 }
 #pragma unroll
-                for (int a = 0; a < DS_NINT; ++a) sm.dcnt[a][threadIdx.x] = cnt[a];
+                for (int a = 0; a < 3; ++a) sm.dwnd[a][threadIdx.x] = wnd[a];
+                sm.dflg[0][threadIdx.x] = n_near;
+                sm.dflg[1][threadIdx.x] = n_big;
 #pragma unroll
                 for (int a = 0; a < DS_NFLT; ++a) sm.dacc[a][threadIdx.x] = acc[a];
                 __syncwarp();   // every lane is done with the staged Pi, ep row
@@ -692,7 +697,9 @@ tiled_step_kernel(ConstFields<float> in, Fields<float> out, StepCoef<float> k, i
         double d_acc[DS_NFLT] = {0, 0, 0, 0, 0, 0, 0};
         if (is_main) {
 #pragma unroll
-            for (int a = 0; a < DS_NINT; ++a) d_cnt[a] = sm.dcnt[a][threadIdx.x];
+            for (int a = 0; a < 3; ++a) d_cnt[a] = (int)sm.dwnd[a][threadIdx.x];
+            d_cnt[DS_NEAR] = sm.dflg[0][threadIdx.x];
+            d_cnt[DS_BIG] = sm.dflg[1][threadIdx.x];
 #pragma unroll
             for (int a = 0; a < DS_NFLT; ++a) d_acc[a] = sm.dacc[a][threadIdx.x];
         }
