@@ -2,13 +2,15 @@
 """bench.py — site-updates/s of the fused Abelian-Higgs leapfrog step on B200.
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--size 1024] [--impl ours|reference]
+                    [--diag-every M] [--pre-steps P] [--sustained-steps S]
 
 One "step" = one pass of the whole hot path over the lattice.  Workload at
 N=1: BASELINE.json configs[3] — 1024^3 periodic lattice, dx=0.5, dt=0.1, fp32 SoA with ping-pong
 buffers (85.9 GB), lambda=2, e=1, sigma=1, radiation era, s=1, seeded random-phase IC, no
 diagnostics.  The path does not shard: with --gpus N each
 rank evolves its own replica of the same lattice (a different seed), value = all ranks' site-updates
-divided by the slowest rank's device time, scaling "weak".
+divided by the slowest rank's device time, scaling "weak".  Started without a torchrun environment,
+`--gpus N` (N > 1) re-executes itself under `python -m torch.distributed.run` with N ranks on 127.0.0.1.
 
 Prints ONE JSON line on rank 0.  `--impl reference` times the fp64 CPU oracle (oracle/) on the host
 cores on a bounded sample of the same workload.
@@ -18,6 +20,7 @@ from __future__ import annotations
 import argparse
 import json
 import os
+import socket
 import subprocess
 import sys
 import threading
@@ -46,13 +49,20 @@ def parse():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--diag-every", type=int, default=0, help="fused diagnostics every n steps (0 = none)")
+    ap.add_argument("--pre-steps", type=int, default=0,
+                    help="untimed steps before the warm-up (starts the timed window at a later epoch tau)")
+    ap.add_argument("--sustained-steps", type=int, default=200,
+                    help="after the K timed steps, time a further window of this many steps (0 = skip) and report it "
+                         "as roofline.sustained: the number the board holds under its power cap")
+    ap.add_argument("--selftest-launcher", action="store_true",
+                    help="CPU-only check of the multi-rank launch path (gloo): no kernels, synthetic per-rank timings")
     return ap.parse_args()
 
 
-def workload_params(n, steps, warmup):
+def workload_params(n, total_steps):
     # configs[3]: radiation era (p=1), s=1; a(tau) normalised to 1 at the end of the run (reading #6)
     return dict(dx=DX, lambda0=2.0, e0=1.0, sigma=1.0, s=1.0, p=1.0,
-                tau_ref=TAU0 + DT * (warmup + steps), alpha=2.0, compact=1)
+                tau_ref=TAU0 + DT * total_steps, alpha=2.0, compact=1)
 
 
 def measured_peak():
@@ -66,19 +76,22 @@ def measured_peak():
 
 
 def recorded_traffic(n, kernel_name):
-    """DRAM bytes per launch of the dominant kernel from the committed ncu --set full capture, or None."""
+    """(DRAM bytes per launch, source) of the dominant kernel from the committed ncu --set full captures, or (None, None).
+
+    The figure is NOT measured in this run (a number taken under a profiler is never a bench value, and the bench
+    does not run under one): it is read from profiles/traffic.csv, which names the capture each row came from."""
     p = ROOT / "profiles" / "traffic.csv"
     if not p.exists():
-        return None
+        return None, None
     try:
         import csv
         with open(p, newline="") as fh:
             for rec in csv.DictReader(fh):
                 if int(rec["size"]) == n and rec["kernel"] == kernel_name:
-                    return float(rec["dram_bytes_per_launch"])
+                    return float(rec["dram_bytes_per_launch"]), f"profiles/traffic.csv (ncu --set full, builder-run): {rec['source']}"
     except Exception:
-        return None
-    return None
+        return None, None
+    return None, None
 
 
 class ClockSampler:
@@ -164,7 +177,7 @@ def run_reference(args):
     if rank != 0:
         return 0
     n = args.size
-    params = workload_params(n, args.steps, args.warmup)
+    params = workload_params(n, args.steps + args.warmup)
     from oracle import ah_oracle as o
     rate64, _, threads = oracle_rate(params, 64, 2)
     budget_s = 150.0
@@ -197,24 +210,27 @@ def run_reference(args):
 
 # ------------------------------------------------------------------------------- CUDA arm
 
+def total_steps(args):
+    return args.pre_steps + max(args.warmup, 3) + args.steps + args.sustained_steps
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
 
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    rank = int(os.environ.get("RANK", "0"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
+    from paper_2005_14454_b200 import replicas
+    rank, local, world = replicas.rank_world()
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
     torch.cuda.set_device(local)
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
 
-    from paper_2005_14454_b200 import build, binding, replicas
+    from paper_2005_14454_b200 import build, binding
     build.build()
 
-    n, K, W = args.size, args.steps, args.warmup
-    params = workload_params(n, K, W)
+    n, K, W = args.size, args.steps, max(args.warmup, 3)
+    params = workload_params(n, total_steps(args))
     sim = binding.Simulation(params=binding.make_params(n, **params), device=f"cuda:{local}")
     if args.kernel != "auto":
         sim.set_kernel({"site": binding.KERNEL_SITE, "tiled": binding.KERNEL_TILED}[args.kernel])
@@ -234,24 +250,44 @@ def run_ours(args):
         sim.step(nsteps, tau, DT)
         return 0
 
+    def timed_window(nsteps, tau):
+        """(max-over-ranks ms, whole-job units, launches, clocks) of nsteps steps from tau, device-timed."""
+        barrier()
+        sampler = ClockSampler(local)
+        if rank == 0:
+            sampler.start()
+        l0 = sim.launch_count()
+        ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        ev0.record(stream)
+        advance(nsteps, tau)
+        ev1.record(stream)
+        barrier()
+        ms_local = ev0.elapsed_time(ev1)
+        launches = sim.launch_count() - l0
+        clocks = sampler.stop() if rank == 0 else None
+        ms, units = replicas.aggregate(ms_local, sites * nsteps, dist if world > 1 else None, device="cuda")
+        return ms, units, launches, clocks
+
     # ---- device-resident throughput
     sim.init_fields(replicas.replica_seed(1, rank))
-    advance(max(W, 3), TAU0)
-    barrier()
-    sampler = ClockSampler(local)
-    if rank == 0:
-        sampler.start()
-    l0 = sim.launch_count()
-    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    ev0.record(stream)
-    advance(K, TAU0 + W * DT)
-    ev1.record(stream)
-    barrier()
-    ms = ev0.elapsed_time(ev1)
-    launches = sim.launch_count() - l0
-    clocks = sampler.stop() if rank == 0 else None
-    ms, units = replicas.aggregate(ms, sites * K, dist if world > 1 else None, device="cuda")   # max time, sum of work
+    tau = TAU0
+    if args.pre_steps > 0:
+        sim.step(args.pre_steps, tau, DT)
+        tau += args.pre_steps * DT
+    advance(W, tau)
+    tau += W * DT
+    tau_timed = tau
+    ms, units, launches, clocks = timed_window(K, tau)
+    tau += K * DT
     value = replicas.throughput(ms, units)
+
+    # ---- the same measurement over a longer window: what the board sustains under its power cap
+    sustained = None
+    if args.sustained_steps > 0:
+        ms_s, units_s, _, clocks_s = timed_window(args.sustained_steps, tau)
+        tau += args.sustained_steps * DT
+        sustained = {"steps": args.sustained_steps, "ms_per_step": ms_s / args.sustained_steps,
+                     "value": replicas.throughput(ms_s, units_s), "unit": UNIT, "clocks": clocks_s}
 
     # ---- end to end through the C ABI with HOST buffers: upload, K steps, download
     e2e = None
@@ -267,40 +303,49 @@ def run_ours(args):
         barrier()
         t0 = time.perf_counter()
         sim.set_fields_ptr(host.data_ptr())          # H2D inside the timed region
-        sim.step(K, TAU0 + W * DT, DT)
+        sim.step(K, tau_timed, DT)
         sim.get_fields_ptr(host.data_ptr())          # D2H (synchronises)
         torch.cuda.synchronize()
         el = time.perf_counter() - t0
-        el_ms, units = replicas.aggregate(el * 1e3, sites * K, dist if world > 1 else None, device="cuda")
+        el_ms, units_e = replicas.aggregate(el * 1e3, sites * K, dist if world > 1 else None, device="cuda")
         el = el_ms * 1e-3
-        e2e = {"value": units / el, "unit": UNIT, "h2d_bytes_per_step": nbytes / K,
+        e2e = {"value": units_e / el, "unit": UNIT, "h2d_bytes_per_step": nbytes / K,
                "d2h_bytes_per_step": nbytes / K, "pinned_host": pinned, "seconds": el,
                "what": f"ah_set_fields(host) + ah_step({K}) + ah_get_fields(host), wall clock"}
         del host
 
     if rank == 0:
         peak, peak_src = measured_peak()
+        diag = args.diag_every > 0
         kernel_name = kernel_used
-        step_launches = K
-        avg_launch_ms = ms / step_launches            # one step-kernel launch per step
+        # one step-kernel launch per step; on diagnostic steps the launch is the DIAG instantiation of the same kernel
+        avg_launch_ms = ms / K
         achieved = BYTES_PER_SITE * sites / (avg_launch_ms * 1e-3) / 1e9
+        traffic, traffic_src = recorded_traffic(n, kernel_name + ("<DIAG>" if diag else ""))
         roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                    "traffic": recorded_traffic(n, kernel_name), "peak_source": peak_src, "kernel": kernel_name,
+                    "traffic": traffic, "traffic_source": traffic_src, "peak_source": peak_src, "kernel": kernel_name,
                     "algorithmic_bytes_per_launch": BYTES_PER_SITE * sites,
                     "frac_of_nominal_8TBs": achieved / NOMINAL_HBM_GBS,
                     "timing": "CUDA events on the launching stream around the K timed steps; avg = elapsed/K "
                               "(each step = 1 tiled_step_kernel launch + 1 conditional-redo launch that exits "
                               "at once, ~2 us; see profiles/ launch list)"
-                              + (" (includes diagnostic launches)" if args.diag_every else "")}
+                              + (f" (every {args.diag_every}th step is the DIAG instantiation + 2 small launches; "
+                                 "the average is over all steps)" if diag else "")}
+        if sustained is not None:
+            ach_s = BYTES_PER_SITE * sites * world / (sustained["ms_per_step"] * 1e-3) / 1e9 / world
+            sustained.update(achieved=ach_s, frac=ach_s / peak, frac_of_nominal_8TBs=ach_s / NOMINAL_HBM_GBS)
+            roofline["sustained"] = sustained
         line = {
-            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": max(W, 3),
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
             "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f32", "data": "synthetic",
             "config": {"workload": f"{n}^3 periodic lattice, dx=0.5, dt=0.1, fp32 SoA ping-pong ({20 * 4 * sites / 1e9:.1f} GB), "
                                    f"lambda=2, e=1, sigma=1, radiation era, s=1, seeded random-phase IC, "
-                                   f"{'no diagnostics' if not args.diag_every else 'diagnostics every %d steps' % args.diag_every}"
-                                   f"{' (BASELINE configs[3])' if n == 1024 and not args.diag_every else ''}",
+                                   f"{'no diagnostics' if not diag else 'fused diagnostics every %d steps' % args.diag_every}"
+                                   f"{' (BASELINE configs[3])' if n == 1024 and not diag else ''}"
+                                   f"{' (BASELINE configs[4] row)' if diag and args.diag_every == 10 else ''}",
                        "kernel": kernel_name, "parallelism": "replicas only" if world > 1 else "single GPU",
+                       "tau_at_timed_window": tau_timed,
                        "l2": "working set (80 B/site x N^3) exceeds the 126 MB L2 for N >= 128; no flush needed"
                              if n >= 128 else "working set fits in L2 (small-lattice case)"},
             "pct_of_8TBs_roofline": 100.0 * value / world * BYTES_PER_SITE / (NOMINAL_HBM_GBS * 1e9),
@@ -317,8 +362,51 @@ def run_ours(args):
     return 0
 
 
+# ------------------------------------------------------------------------------- launcher
+
+def free_port():
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        return sk.getsockname()[1]
+
+
+def relaunch_under_torchrun(args):
+    """`python bench.py --gpus N` without a torchrun environment: start N ranks (one per GPU) of this same command."""
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+           "--master-addr", "127.0.0.1", "--master-port", str(free_port()), str(Path(__file__).resolve())] + sys.argv[1:]
+    return subprocess.call(cmd)
+
+
+def run_selftest_launcher(args):
+    """The multi-rank path without a GPU (tests/test_replicas_gloo.py): every rank reports a synthetic device time and
+    unit count through the same replicas.aggregate / JSON code as the CUDA arm, over gloo."""
+    import torch.distributed as dist
+    from paper_2005_14454_b200 import replicas
+    rank, local, world = replicas.rank_world()
+    if world > 1:
+        dist.init_process_group("gloo")
+    ms_local, units_local = 10.0 * (rank + 1), 1000.0 * args.steps
+    ms, units = replicas.aggregate(ms_local, units_local, dist if world > 1 else None, device="cpu")
+    if rank == 0:
+        print(json.dumps({"selftest": "launcher", "n_gpus": world, "steps": args.steps, "ms": ms, "units": units,
+                          "value": replicas.throughput(ms, units), "seed_of_last_rank": replicas.replica_seed(1, world - 1)}),
+              flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
 def main():
     args = parse()
+    if args.gpus < 1:
+        raise SystemExit("--gpus must be >= 1")
+    in_torchrun = "WORLD_SIZE" in os.environ and "RANK" in os.environ
+    if in_torchrun and int(os.environ["WORLD_SIZE"]) != args.gpus:
+        raise SystemExit(f"--gpus {args.gpus} but WORLD_SIZE={os.environ['WORLD_SIZE']}")
+    if args.gpus > 1 and not in_torchrun and (args.impl == "ours" or args.selftest_launcher):
+        return relaunch_under_torchrun(args)
+    if args.selftest_launcher:
+        return run_selftest_launcher(args)
     if args.impl == "reference":
         return run_reference(args)
     return run_ours(args)

@@ -64,3 +64,30 @@ def test_single_process_and_validation():
         replicas.throughput(0.0, 1.0)
     with pytest.raises(ValueError):
         replicas.replica_seed(-1, 0)
+
+
+def test_bench_gpus_n_starts_n_ranks():
+    """`python bench.py --gpus 2` started WITHOUT a torchrun environment must itself start 2 ranks (the way the driver
+    runs it at N = 1 is the same command line).  The launcher self-test runs that path on CPU over gloo: same re-exec,
+    same replicas.aggregate (max of the times, sum of the units), same JSON printing by rank 0 only."""
+    import json
+    import os
+    import subprocess
+    import sys
+    from pathlib import Path
+
+    root = Path(__file__).resolve().parent.parent
+    env = {k: v for k, v in os.environ.items() if k not in ("RANK", "WORLD_SIZE", "LOCAL_RANK", "MASTER_ADDR", "MASTER_PORT")}
+    out = subprocess.run([sys.executable, str(root / "bench.py"), "--gpus", "2", "--steps", "3", "--selftest-launcher"],
+                         capture_output=True, text=True, timeout=300, env=env, cwd=str(root))
+    assert out.returncode == 0, out.stderr[-2000:]
+    lines = [json.loads(ln) for ln in out.stdout.splitlines() if ln.startswith("{")]
+    assert len(lines) == 1, out.stdout                      # rank 0 alone prints
+    rec = lines[0]
+    assert rec["n_gpus"] == 2 and rec["ms"] == 20.0 and rec["units"] == 6000.0
+    assert rec["value"] == 6000.0 / 20e-3 and rec["seed_of_last_rank"] == 2
+    # a WORLD_SIZE that contradicts --gpus is refused instead of silently timing one GPU
+    env2 = dict(env, WORLD_SIZE="1", RANK="0", LOCAL_RANK="0")
+    bad = subprocess.run([sys.executable, str(root / "bench.py"), "--gpus", "2", "--selftest-launcher"],
+                         capture_output=True, text=True, timeout=120, env=env2, cwd=str(root))
+    assert bad.returncode != 0 and "WORLD_SIZE" in (bad.stderr + bad.stdout)
