@@ -15,7 +15,7 @@ extern "C" {
 /* kernel selection for ah_set_kernel */
 #define AH_KERNEL_AUTO 0  /* fused tiled kernel when the lattice allows it, else the site kernel */
 #define AH_KERNEL_SITE 1  /* one thread per site, neighbours through L1/L2 (any nx,ny,nz >= 1) */
-#define AH_KERNEL_TILED 2 /* z-marching register/shared-memory tiled kernel (needs nx % 128 == 0) */
+#define AH_KERNEL_TILED 2 /* z-marching register/shared-memory tiled kernel (needs nx % 64 == 0) */
 
 /* Choose the step kernel (AH_KERNEL_*).  AH_EINVAL if the lattice does not allow it. */
 int ah_set_kernel(ah_ctx *ctx, int kernel);

@@ -387,7 +387,7 @@ int ah_set_kernel(ah_ctx *c, int kernel)
     const bool can_tile = !c->P.fp64 && ah::tiled_supported(c->P.nx, c->P.ny, c->P.nz);
     if (kernel == AH_KERNEL_AUTO) kernel = can_tile ? AH_KERNEL_TILED : AH_KERNEL_SITE;
     if (kernel == AH_KERNEL_TILED) {
-        if (!can_tile) return fail(AH_EINVAL, "ah_set_kernel: tiled kernel needs fp32 and nx %% 128 == 0");
+        if (!can_tile) return fail(AH_EINVAL, "ah_set_kernel: tiled kernel needs fp32 and nx %% 64 == 0");
         AH_CUDA(ah::tiled_setup());
     } else if (kernel != AH_KERNEL_SITE) {
         return fail(AH_EINVAL, "ah_set_kernel: unknown kernel %d", kernel);
@@ -405,7 +405,7 @@ int ah_get_kernel(const ah_ctx *c)
 int ah_tiled_launch_info(int nx, int ny, int nz, int *planes_per_cta, int *n_ctas)
 {
     if (!planes_per_cta || !n_ctas) return fail(AH_EINVAL, "ah_tiled_launch_info: null pointer");
-    if (!ah::tiled_supported(nx, ny, nz)) return fail(AH_EINVAL, "ah_tiled_launch_info: tiled kernel needs nx %% 128 == 0");
+    if (!ah::tiled_supported(nx, ny, nz)) return fail(AH_EINVAL, "ah_tiled_launch_info: tiled kernel needs nx %% 64 == 0");
     *planes_per_cta = ah::tiled_chunk(nx, ny, nz);
     *n_ctas = ah::tiled_num_blocks(nx, ny, nz);
     return AH_OK;

@@ -267,6 +267,31 @@ __device__ __forceinline__ float plaq_angle_f32(float th_i, float th_j_xi, float
     return __fadd_rn(__fadd_rn(__fadd_rn(th_i, th_j_xi), -th_i_xj), -th_j);
 }
 
+// ---- programmatic dependent launch (PTX griddepcontrol; sm_90+): the step kernels of consecutive steps are launched
+// with cudaLaunchAttributeProgrammaticStreamSerialization, so the launch of kernel k+1 is processed while kernel k
+// still runs.  pdl_wait() blocks until the preceding kernel of the stream has completed and its writes are visible;
+// it precedes EVERY global access of a kernel launched that way (also on early-exit paths, so that completion of a
+// kernel always implies completion of its predecessors).  pdl_launch_dependents() lets the next kernel's CTAs be
+// scheduled as soon as there is room for them.
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+
+template <typename... KArgs, typename... Args>
+cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, Args... args)
+{
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid;
+    cfg.blockDim = block;
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, kernel, KArgs(args)...);
+}
+
 // ------------------------------------------------------------------------- block reduction
 
 __device__ __forceinline__ double warp_sum(double v)

@@ -15,7 +15,8 @@ template <typename real>
 cudaError_t launch_init(const Fields<real> &out, uint64_t seed, double sigma, size_t n,
                         cudaStream_t st);
 
-// z-marching tiled fp32 step (ah_tiled_kernel.cu); needs nx % 128 == 0
+// z-marching tiled fp32 step (ah_tiled_kernel.cu); needs nx % 64 == 0 (128-site warp rows when nx % 128 == 0,
+// 64-site rows otherwise)
 bool tiled_supported(int nx, int ny, int nz);
 //   overflow: device int, set to 1 when a link angle is outside the kernel's domain (|th| >= 2^16 rad);
 //             the outputs of that step must then be recomputed with the site kernel

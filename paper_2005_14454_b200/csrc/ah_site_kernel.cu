@@ -2,7 +2,7 @@
 //
 // This is the general kernel: it evaluates Eqs. 7-10 at one site per thread with
 // every neighbour read straight from global memory through L1/L2.  It serves lattices the tiled
-// kernel does not cover (nx not a multiple of 128, fp64 state) and is the algebra check of the
+// kernel does not cover (nx not a multiple of 64, fp64 state) and is the algebra check of the
 // tiled kernel (tests compare the two bit-for-bit-independent paths against the oracle).
 #include "ah_kernels.h"
 
@@ -122,6 +122,8 @@ __global__ void __launch_bounds__(256)
 site_redo_kernel(const int *flag, int *clear, ConstFields<float> in, Fields<float> out, StepCoef<float> k,
                  int nx, int ny, int nz)
 {
+    pdl_launch_dependents();
+    pdl_wait();   // before the flag is read, and before the early exit (ah_common.cuh)
     if (blockIdx.x == 0 && threadIdx.x == 0) *clear = 0;
     if (*flag == 0) return;
     const size_t n = (size_t)nx * ny * nz;
@@ -134,8 +136,7 @@ site_redo_kernel(const int *flag, int *clear, ConstFields<float> in, Fields<floa
 cudaError_t launch_site_redo(const int *flag, int *clear, const ConstFields<float> &in, const Fields<float> &out,
                              const StepCoef<float> &k, int nx, int ny, int nz, cudaStream_t st)
 {
-    site_redo_kernel<<<148 * 4, 256, 0, st>>>(flag, clear, in, out, k, nx, ny, nz);
-    return cudaGetLastError();
+    return launch_pdl(site_redo_kernel, dim3(148 * 4), dim3(256), 0, st, flag, clear, in, out, k, nx, ny, nz);
 }
 
 template <typename real>

@@ -32,29 +32,57 @@ namespace ah {
 
 namespace {
 
-constexpr int TILE_X = 128;            // sites per warp row segment (32 lanes x 4)
 constexpr int HALO = 4;                // staged halo columns on each side (16 bytes)
-constexpr int ROWF = TILE_X + 2 * HALO;   // floats per staged row
 constexpr int NST = 3;                 // ring slots
 constexpr int NRAW = 5;                // staged fields: phi_re, phi_im, th_x, th_y, th_z
 constexpr unsigned FULL = 0xffffffffu;
 
-struct V4 {
-    float v[4];
+// SPT consecutive x sites of one thread (4: 128-bit accesses, 128-site warp rows; 2: 64-bit, 64-site rows)
+template <int SPT>
+struct VN {
+    float v[SPT];
 };
 
-__device__ __forceinline__ V4 lds4(const float *p)
+template <int SPT>
+__device__ __forceinline__ VN<SPT> ldsN(const float *p)
 {
-    const float4 t = *reinterpret_cast<const float4 *>(p);
-    V4 r;
-    r.v[0] = t.x; r.v[1] = t.y; r.v[2] = t.z; r.v[3] = t.w;
+    VN<SPT> r;
+    if constexpr (SPT == 4) {
+        const float4 t = *reinterpret_cast<const float4 *>(p);
+        r.v[0] = t.x; r.v[1] = t.y; r.v[2] = t.z; r.v[3] = t.w;
+    } else {
+        const float2 t = *reinterpret_cast<const float2 *>(p);
+        r.v[0] = t.x; r.v[1] = t.y;
+    }
     return r;
 }
-__device__ __forceinline__ void st4(float *__restrict__ p, const V4 &a)
+template <int SPT>
+__device__ __forceinline__ VN<SPT> ldgN(const float *p)
 {
-    *reinterpret_cast<float4 *>(p) = make_float4(a.v[0], a.v[1], a.v[2], a.v[3]);
+    VN<SPT> r;
+    if constexpr (SPT == 4) {
+        const float4 t = __ldg(reinterpret_cast<const float4 *>(p));
+        r.v[0] = t.x; r.v[1] = t.y; r.v[2] = t.z; r.v[3] = t.w;
+    } else {
+        const float2 t = __ldg(reinterpret_cast<const float2 *>(p));
+        r.v[0] = t.x; r.v[1] = t.y;
+    }
+    return r;
 }
-__device__ __forceinline__ float4 f4(const V4 &a) { return make_float4(a.v[0], a.v[1], a.v[2], a.v[3]); }
+template <int SPT>
+__device__ __forceinline__ void stN(float *__restrict__ p, const VN<SPT> &a)
+{
+    if constexpr (SPT == 4) *reinterpret_cast<float4 *>(p) = make_float4(a.v[0], a.v[1], a.v[2], a.v[3]);
+    else *reinterpret_cast<float2 *>(p) = make_float2(a.v[0], a.v[1]);
+}
+template <int SPT>
+__device__ __forceinline__ float vmaxabs(const VN<SPT> &a)
+{
+    float m = fabsf(a.v[0]);
+#pragma unroll
+    for (int j = 1; j < SPT; ++j) m = fmaxf(m, fabsf(a.v[j]));
+    return m;
+}
 
 // ---- mbarrier / bulk-copy primitives (PTX; SASS: SYNCS.*, UBLKCP)
 __device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
@@ -131,17 +159,19 @@ __device__ __forceinline__ float plaq_f(float phi)
     return COMPACT ? sin_poly_f32(phi) : phi;   // reading #10; range check by the caller
 }
 
-template <int TY, bool DIAG>
+template <int SPT, int TY, bool DIAG>
 struct Smem {
-    float raw[NST][NRAW][TY + 2][ROWF];   // staged planes; row r <-> y0 - 1 + r, column c <-> x0 - HALO + c
-    float qe[TY][NRAW][TILE_X];           // staged old Pi, ep of the own rows (one plane): pi_re, pi_im, ep_x, ep_y, ep_z
+    static constexpr int TX = 32 * SPT;        // sites per warp row segment
+    static constexpr int RF = TX + 2 * HALO;   // floats per staged row
+    float raw[NST][NRAW][TY + 2][RF];     // staged planes; row r <-> y0 - 1 + r, column c <-> x0 - HALO + c
+    float qe[TY][NRAW][TX];               // staged old Pi, ep of the own rows (one plane): pi_re, pi_im, ep_x, ep_y, ep_z
     // y hand-over: (b_y.re, b_y.im, S_xy, S_yz); row 0 = halo row y0-1, row w+1 from warp w.  Double buffered
     // (one barrier per plane).  DIAG: after warp w has consumed row w of a buffer it re-uses the first 128 floats
     // of that row as scratch (the sites' gradient energies, handed from the step to the read-out loop)
-    float4 row[2][TY][4][32];
+    float row[2][TY][4][TX];
     // DIAG: alpha = Arg(phi) (ah_diag_site.cuh) of the staged rows 1 .. TY+1 (columns HALO .. HALO+128) of the
     // plane held by the ring slot of the same index
-    float alpha[DIAG ? NST : 1][DIAG ? TY + 1 : 1][DIAG ? ROWF : 4];
+    float alpha[DIAG ? NST : 1][DIAG ? TY + 1 : 1][DIAG ? RF : 4];
     // DIAG: per-thread partial sums of the main warps, parked here between read-out loops so that they do not
     // occupy registers during the step's arithmetic
     double dacc[DIAG ? DS_NFLT : 1][DIAG ? TY * 32 : 1];
@@ -180,17 +210,19 @@ namespace {
 //     and one ep_x per row.
 // Per-thread partial sums (int32 counts, fp64 sums) live in shared memory between loops, are reduced per CTA
 // into partials[linear CTA index]; diag_final_kernel adds them in a fixed order.
-template <int TY, bool COMPACT, bool DIAG>
+template <int SPT, int TY, bool COMPACT, bool DIAG>
 __global__ void __launch_bounds__((TY + 1) * 32, ((TY + 1) * 32 <= 256) ? 2 : 1)
 tiled_step_kernel(ConstFields<float> in, Fields<float> out, StepCoef<float> k, int nx, int ny, int nz, int zc,
                   int *overflow, DiagCoef dk, DiagPartial *partials)
 {
     extern __shared__ __align__(128) unsigned char smem_bytes[];
-    Smem<TY, DIAG> &sm = *reinterpret_cast<Smem<TY, DIAG> *>(smem_bytes);
+    Smem<SPT, TY, DIAG> &sm = *reinterpret_cast<Smem<SPT, TY, DIAG> *>(smem_bytes);
+    constexpr int TX = 32 * SPT, RF = TX + 2 * HALO;
+    using VS = VN<SPT>;
 
     const int lane = threadIdx.x & 31;
     const int w = __shfl_sync(FULL, (int)(threadIdx.x >> 5), 0);   // warp-uniform by construction
-    const int x0 = blockIdx.x * TILE_X, y0 = blockIdx.y * TY, z0 = blockIdx.z * zc;
+    const int x0 = blockIdx.x * TX, y0 = blockIdx.y * TY, z0 = blockIdx.z * zc;
     const int z1 = min(nz, z0 + zc);
     const int nplanes = z1 - z0;           // planes this CTA updates; loads n = 0 .. nplanes + 1
     const size_t sxy = (size_t)nx * ny;
@@ -200,7 +232,7 @@ tiled_step_kernel(ConstFields<float> in, Fields<float> out, StepCoef<float> k, i
     // load n  <->  plane z0 - 1 + n (periodic), slot n % NST.  Every main warp copies its own staged row (one
     // copy per field), the helper warp the two halo rows 0 and TY+1, and it arms the slot's mbarrier with the
     // byte count of the whole plane.  One elected lane per warp issues them, with warp-uniform operands.
-    const bool interior = (x0 > 0) && (x0 + TILE_X < nx);
+    const bool interior = (x0 > 0) && (x0 + TX < nx);
     auto wrap_y = [&](int yy) {
         yy %= ny;
         return yy < 0 ? yy + ny : yy;
@@ -222,13 +254,13 @@ tiled_step_kernel(ConstFields<float> in, Fields<float> out, StepCoef<float> k, i
             const float *srow = in.f[FLD[f]] + src_off;
             float *dst = &sm.raw[slot][f][r][0];
             if (interior) {
-                copy1(dst, srow + x0 - HALO, ROWF * sizeof(float), &sm.full[slot]);
+                copy1(dst, srow + x0 - HALO, RF * sizeof(float), &sm.full[slot]);
             } else {
                 const int xl = (x0 == 0) ? nx - HALO : x0 - HALO;
-                const int xr = (x0 + TILE_X == nx) ? 0 : x0 + TILE_X;
-                copy1(dst + HALO, srow + x0, TILE_X * sizeof(float), &sm.full[slot]);
+                const int xr = (x0 + TX == nx) ? 0 : x0 + TX;
+                copy1(dst + HALO, srow + x0, TX * sizeof(float), &sm.full[slot]);
                 copy1(dst, srow + xl, HALO * sizeof(float), &sm.full[slot]);
-                copy1(dst + HALO + TILE_X, srow + xr, HALO * sizeof(float), &sm.full[slot]);
+                copy1(dst + HALO + TX, srow + xr, HALO * sizeof(float), &sm.full[slot]);
             }
         }
     };
@@ -240,7 +272,7 @@ tiled_step_kernel(ConstFields<float> in, Fields<float> out, StepCoef<float> k, i
             if (is_main) {
                 copy_row(ld_slot, w + 1, ld_plane + p_row0);
             } else {
-                mbar_expect_tx(&sm.full[ld_slot], (unsigned)(NRAW * (TY + 2) * ROWF * sizeof(float)));
+                mbar_expect_tx(&sm.full[ld_slot], (unsigned)(NRAW * (TY + 2) * RF * sizeof(float)));
                 copy_row(ld_slot, 0, ld_plane + p_row0);
                 copy_row(ld_slot, TY + 1, ld_plane + p_row1);
             }
@@ -258,15 +290,16 @@ tiled_step_kernel(ConstFields<float> in, Fields<float> out, StepCoef<float> k, i
     auto produce_q = [&]() {
         if (elect_one()) {
             constexpr int FLD[NRAW] = {PI_RE, PI_IM, EP_X, EP_Y, EP_Z};
-            mbar_expect_tx(&sm.qfull[w], (unsigned)(NRAW * TILE_X * sizeof(float)));
+            mbar_expect_tx(&sm.qfull[w], (unsigned)(NRAW * TX * sizeof(float)));
 #pragma unroll
             for (int f = 0; f < NRAW; ++f)
-                if (AH_L2_HINTS) bulk_g2s_hint(&sm.qe[w][f][0], in.f[FLD[f]] + q_off, TILE_X * sizeof(float), &sm.qfull[w], pol_stream);
-                else bulk_g2s(&sm.qe[w][f][0], in.f[FLD[f]] + q_off, TILE_X * sizeof(float), &sm.qfull[w]);
+                if (AH_L2_HINTS) bulk_g2s_hint(&sm.qe[w][f][0], in.f[FLD[f]] + q_off, TX * sizeof(float), &sm.qfull[w], pol_stream);
+                else bulk_g2s(&sm.qe[w][f][0], in.f[FLD[f]] + q_off, TX * sizeof(float), &sm.qfull[w]);
         }
         q_off += sxy;
     };
 
+    pdl_launch_dependents();
     if (threadIdx.x == 0) {
 #pragma unroll
         for (int s = 0; s < NST; ++s) mbar_init(&sm.full[s], 1);
@@ -276,6 +309,7 @@ tiled_step_kernel(ConstFields<float> in, Fields<float> out, StepCoef<float> k, i
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
     }
     __syncthreads();
+    pdl_wait();   // the previous step's kernels have completed: its outputs are this step's inputs
     produce();   // loads 0, 1, 2
     produce();
     produce();
@@ -289,8 +323,8 @@ tiled_step_kernel(ConstFields<float> in, Fields<float> out, StepCoef<float> k, i
     const int y = y0 + w;
     const bool act = is_main && y < ny;
     const int r_own = w + 1;
-    const int cofs = HALO + 4 * lane;                    // staged column of this thread's first site
-    const size_t ro = (size_t)(act ? y : 0) * nx + x0 + 4 * lane;
+    const int cofs = HALO + SPT * lane;                    // staged column of this thread's first site
+    const size_t ro = (size_t)(act ? y : 0) * nx + x0 + SPT * lane;
     // ---- helper-warp geometry: halo row (staged row 0) and halo column x0-1 (staged column HALO-1)
     const bool col_act = !is_main && lane < TY;
 
@@ -300,40 +334,37 @@ tiled_step_kernel(ConstFields<float> in, Fields<float> out, StepCoef<float> k, i
         if constexpr (DIAG) {
             const int r = is_main ? w + 1 : TY + 1;
 #pragma unroll
-            for (int j = 0; j < 4; ++j) {
+            for (int j = 0; j < SPT; ++j) {
                 const int c = HALO + lane + 32 * j;
                 sm.alpha[slot][r - 1][c] = site_phase_fast(sm.raw[slot][0][r][c], sm.raw[slot][1][r][c]);
             }
             if (!is_main && lane <= TY)
-                sm.alpha[slot][lane][HALO + TILE_X] =
-                    site_phase_fast(sm.raw[slot][0][lane + 1][HALO + TILE_X], sm.raw[slot][1][lane + 1][HALO + TILE_X]);
+                sm.alpha[slot][lane][HALO + TX] =
+                    site_phase_fast(sm.raw[slot][0][lane + 1][HALO + TX], sm.raw[slot][1][lane + 1][HALO + TX]);
         }
     };
 
     // ---- prologue: hand-down of the plane below the chunk (needs loads 0 and 1)
-    V4 c_pr, c_pi, c_tx, c_ty, c_tz;        // own old phi, th of the current plane
-    V4 g_bzr, g_bzi, g_sxz, g_syz;          // b_z, S_xz, S_yz of the site below (z-1)
+    VS c_pr, c_pi, c_tx, c_ty, c_tz;        // own old phi, th of the current plane
+    VS g_bzr, g_bzi, g_sxz, g_syz;          // b_z, S_xz, S_yz of the site below (z-1)
     mbar_wait(&sm.full[0], 0);
     mbar_wait(&sm.full[1], 0);
     if (act) {
-        c_pr = lds4(&sm.raw[1][0][r_own][cofs]); c_pi = lds4(&sm.raw[1][1][r_own][cofs]);
-        c_tx = lds4(&sm.raw[1][2][r_own][cofs]); c_ty = lds4(&sm.raw[1][3][r_own][cofs]);
-        c_tz = lds4(&sm.raw[1][4][r_own][cofs]);
-        if (!(fmaxf(fmaxf(fmaxf(fabsf(c_tx.v[0]), fabsf(c_tx.v[1])), fmaxf(fabsf(c_tx.v[2]), fabsf(c_tx.v[3]))),
-                    fmaxf(fmaxf(fmaxf(fabsf(c_ty.v[0]), fabsf(c_ty.v[1])), fmaxf(fabsf(c_ty.v[2]), fabsf(c_ty.v[3]))),
-                          fmaxf(fmaxf(fabsf(c_tz.v[0]), fabsf(c_tz.v[1])), fmaxf(fabsf(c_tz.v[2]), fabsf(c_tz.v[3]))))) <
-              AH_TILED_TH_LIMIT))
+        c_pr = ldsN<SPT>(&sm.raw[1][0][r_own][cofs]); c_pi = ldsN<SPT>(&sm.raw[1][1][r_own][cofs]);
+        c_tx = ldsN<SPT>(&sm.raw[1][2][r_own][cofs]); c_ty = ldsN<SPT>(&sm.raw[1][3][r_own][cofs]);
+        c_tz = ldsN<SPT>(&sm.raw[1][4][r_own][cofs]);
+        if (!(fmaxf(vmaxabs<SPT>(c_tx), fmaxf(vmaxabs<SPT>(c_ty), vmaxabs<SPT>(c_tz))) < AH_TILED_TH_LIMIT))
             *overflow = 1;
-        const V4 m_pr = lds4(&sm.raw[0][0][r_own][cofs]), m_pi = lds4(&sm.raw[0][1][r_own][cofs]);
-        const V4 m_tx = lds4(&sm.raw[0][2][r_own][cofs]), m_ty = lds4(&sm.raw[0][3][r_own][cofs]);
-        const V4 m_tz = lds4(&sm.raw[0][4][r_own][cofs]);
-        const V4 my_tz = lds4(&sm.raw[0][4][r_own + 1][cofs]);
-        const float me_tz = sm.raw[0][4][r_own][cofs + 4];
+        const VS m_pr = ldsN<SPT>(&sm.raw[0][0][r_own][cofs]), m_pi = ldsN<SPT>(&sm.raw[0][1][r_own][cofs]);
+        const VS m_tx = ldsN<SPT>(&sm.raw[0][2][r_own][cofs]), m_ty = ldsN<SPT>(&sm.raw[0][3][r_own][cofs]);
+        const VS m_tz = ldsN<SPT>(&sm.raw[0][4][r_own][cofs]);
+        const VS my_tz = ldsN<SPT>(&sm.raw[0][4][r_own + 1][cofs]);
+        const float me_tz = sm.raw[0][4][r_own][cofs + SPT];
 #pragma unroll
-        for (int j = 0; j < 4; ++j) {
+        for (int j = 0; j < SPT; ++j) {
             float s, c;
             sincos_pi_f32(m_tz.v[j], s, c);
-            const float tz_xp = (j < 3) ? m_tz.v[j < 3 ? j + 1 : 3] : me_tz;
+            const float tz_xp = (j < SPT - 1) ? m_tz.v[j < SPT - 1 ? j + 1 : SPT - 1] : me_tz;
             const float a_xz = m_tx.v[j] + tz_xp - c_tx.v[j] - m_tz.v[j];
             const float a_yz = m_ty.v[j] + my_tz.v[j] - c_ty.v[j] - m_tz.v[j];
             const float sxz = plaq_f<COMPACT>(a_xz), syz = plaq_f<COMPACT>(a_yz);
@@ -376,19 +407,19 @@ tiled_step_kernel(ConstFields<float> in, Fields<float> out, StepCoef<float> k, i
             mbar_wait(&sm.full[sf], sf_par);
             stage_alpha(sf);
             // helper: shared quantities of the halo row y0-1 (staged row 0) at this plane
-            const V4 h_pr = lds4(&sm.raw[so][0][0][cofs]), h_pi = lds4(&sm.raw[so][1][0][cofs]);
-            const V4 h_tx = lds4(&sm.raw[so][2][0][cofs]), h_ty = lds4(&sm.raw[so][3][0][cofs]);
-            const V4 h_tz = lds4(&sm.raw[so][4][0][cofs]);
-            const V4 hn_ty = lds4(&sm.raw[sf][3][0][cofs]);
-            const V4 hy_tx = lds4(&sm.raw[so][2][1][cofs]), hy_tz = lds4(&sm.raw[so][4][1][cofs]);
+            const VS h_pr = ldsN<SPT>(&sm.raw[so][0][0][cofs]), h_pi = ldsN<SPT>(&sm.raw[so][1][0][cofs]);
+            const VS h_tx = ldsN<SPT>(&sm.raw[so][2][0][cofs]), h_ty = ldsN<SPT>(&sm.raw[so][3][0][cofs]);
+            const VS h_tz = ldsN<SPT>(&sm.raw[so][4][0][cofs]);
+            const VS hn_ty = ldsN<SPT>(&sm.raw[sf][3][0][cofs]);
+            const VS hy_tx = ldsN<SPT>(&sm.raw[so][2][1][cofs]), hy_tz = ldsN<SPT>(&sm.raw[so][4][1][cofs]);
             float hr_ty = __shfl_down_sync(FULL, h_ty.v[0], 1);
-            if (lane == 31) hr_ty = sm.raw[so][3][0][cofs + 4];
-            V4 o_byr, o_byi, o_sxy, o_syz;
+            if (lane == 31) hr_ty = sm.raw[so][3][0][cofs + SPT];
+            VS o_byr, o_byi, o_sxy, o_syz;
 #pragma unroll
-            for (int j = 0; j < 4; ++j) {
+            for (int j = 0; j < SPT; ++j) {
                 float s, c;
                 sincos_pi_f32(h_ty.v[j], s, c);
-                const float ty_xp = (j < 3) ? h_ty.v[j < 3 ? j + 1 : 3] : hr_ty;
+                const float ty_xp = (j < SPT - 1) ? h_ty.v[j < SPT - 1 ? j + 1 : SPT - 1] : hr_ty;
                 const float a_xy = h_tx.v[j] + ty_xp - hy_tx.v[j] - h_ty.v[j];
                 const float a_yz = h_ty.v[j] + hy_tz.v[j] - hn_ty.v[j] - h_tz.v[j];
                 const float sxy_ = plaq_f<COMPACT>(a_xy), syz_ = plaq_f<COMPACT>(a_yz);
@@ -397,10 +428,10 @@ tiled_step_kernel(ConstFields<float> in, Fields<float> out, StepCoef<float> k, i
                 o_sxy.v[j] = sxy_;
                 o_syz.v[j] = syz_;
             }
-            sm.row[buf][0][0][lane] = f4(o_byr);
-            sm.row[buf][0][1][lane] = f4(o_byi);
-            sm.row[buf][0][2][lane] = f4(o_sxy);
-            sm.row[buf][0][3][lane] = f4(o_syz);
+            stN<SPT>(&sm.row[buf][0][0][SPT * lane], o_byr);
+            stN<SPT>(&sm.row[buf][0][1][SPT * lane], o_byi);
+            stN<SPT>(&sm.row[buf][0][2][SPT * lane], o_sxy);
+            stN<SPT>(&sm.row[buf][0][3][SPT * lane], o_syz);
             // halo column x0-1 (staged column HALO-1) of tile row `lane`
             if (col_act) {
                 const int r = lane + 1, cw = HALO - 1;
@@ -437,43 +468,43 @@ tiled_step_kernel(ConstFields<float> in, Fields<float> out, StepCoef<float> k, i
             const int so = sf;
             if (++sf == NST) { sf = 0; sf_par ^= 1; }
             oc += sxy;
-            V4 P_r, P_i, E_x, E_y, E_z;   // Pi+, ep+ still lacking the old Pi, ep and the terms from row y-1 / site x0-1
+            VS P_r, P_i, E_x, E_y, E_z;   // Pi+, ep+ still lacking the old Pi, ep and the terms from row y-1 / site x0-1
             if (!DIAG && n + 2 <= nplanes + 1) produce();
             // DIAG: the backward ep neighbours that are not on chip (row y-1 of this plane, this row of the plane
             // below, and - lane 0 - the site x0-1), requested a whole phase before the read-out loop needs them
-            float4 d_eby = make_float4(0.f, 0.f, 0.f, 0.f), d_ebz = d_eby;
+            VS d_eby, d_ebz;
             float d_exl = 0.f;
             if constexpr (DIAG) {
                 const int z = z0 + n - 1, zm = (z == 0) ? nz - 1 : z - 1, ym = (y == 0) ? ny - 1 : y - 1;
-                d_eby = __ldg(reinterpret_cast<const float4 *>(in.f[EP_Y] + (size_t)z * sxy + (size_t)ym * nx + x0 + 4 * lane));
-                d_ebz = __ldg(reinterpret_cast<const float4 *>(in.f[EP_Z] + (size_t)zm * sxy + ro));
+                d_eby = ldgN<SPT>(in.f[EP_Y] + (size_t)z * sxy + (size_t)ym * nx + x0 + SPT * lane);
+                d_ebz = ldgN<SPT>(in.f[EP_Z] + (size_t)zm * sxy + ro);
                 if (lane == 0) d_exl = __ldg(in.f[EP_X] + (size_t)z * sxy + (size_t)y * nx + ((x0 == 0) ? nx - 1 : x0 - 1));
             }
             mbar_wait(&sm.full[sf], sf_par);
             stage_alpha(sf);   // DIAG: site phases of the forward plane
-            V4 o_byr, o_byi, o_sxy, o_syz;   // for row y+1, through shared memory
-            V4 h_bzr, h_bzi, h_sxz;          // this plane's hand-down to z+1 (with S_yz in o_syz)
+            VS o_byr, o_byi, o_sxy, o_syz;   // for row y+1, through shared memory
+            VS h_bzr, h_bzi, h_sxz;          // this plane's hand-down to z+1 (with S_yz in o_syz)
             float l_bxr = 0.f, l_bxi = 0.f, l_sxy = 0.f, l_sxz = 0.f;   // from the site to the left
-            const V4 y_pr = lds4(&sm.raw[so][0][r_own + 1][cofs]), y_pi = lds4(&sm.raw[so][1][r_own + 1][cofs]);
-            const V4 y_tx = lds4(&sm.raw[so][2][r_own + 1][cofs]), y_tz = lds4(&sm.raw[so][4][r_own + 1][cofs]);
-            const V4 n_pr = lds4(&sm.raw[sf][0][r_own][cofs]), n_pi = lds4(&sm.raw[sf][1][r_own][cofs]);
-            const V4 n_tx = lds4(&sm.raw[sf][2][r_own][cofs]), n_ty = lds4(&sm.raw[sf][3][r_own][cofs]);
+            const VS y_pr = ldsN<SPT>(&sm.raw[so][0][r_own + 1][cofs]), y_pi = ldsN<SPT>(&sm.raw[so][1][r_own + 1][cofs]);
+            const VS y_tx = ldsN<SPT>(&sm.raw[so][2][r_own + 1][cofs]), y_tz = ldsN<SPT>(&sm.raw[so][4][r_own + 1][cofs]);
+            const VS n_pr = ldsN<SPT>(&sm.raw[sf][0][r_own][cofs]), n_pi = ldsN<SPT>(&sm.raw[sf][1][r_own][cofs]);
+            const VS n_tx = ldsN<SPT>(&sm.raw[sf][2][r_own][cofs]), n_ty = ldsN<SPT>(&sm.raw[sf][3][r_own][cofs]);
             // right neighbours of the 4th site: lane+1's first site, or (lane 31) the staged halo column
             float r_pr = __shfl_down_sync(FULL, c_pr.v[0], 1), r_pi = __shfl_down_sync(FULL, c_pi.v[0], 1);
             float r_ty = __shfl_down_sync(FULL, c_ty.v[0], 1), r_tz = __shfl_down_sync(FULL, c_tz.v[0], 1);
             if (lane == 31) {
-                r_pr = sm.raw[so][0][r_own][cofs + 4]; r_pi = sm.raw[so][1][r_own][cofs + 4];
-                r_ty = sm.raw[so][3][r_own][cofs + 4]; r_tz = sm.raw[so][4][r_own][cofs + 4];
+                r_pr = sm.raw[so][0][r_own][cofs + SPT]; r_pi = sm.raw[so][1][r_own][cofs + SPT];
+                r_ty = sm.raw[so][3][r_own][cofs + SPT]; r_tz = sm.raw[so][4][r_own][cofs + SPT];
             }
 
             // plaquette angles owned by the 4 sites (Eqs. 14-15), then their sines: when every angle of the
             // warp is small (the physical regime) a Taylor polynomial without range reduction is exact to fp32
-            V4 S_xy, S_xz, S_yz;
+            VS S_xy, S_xz, S_yz;
             float amax = 0.f;
 #pragma unroll
-            for (int j = 0; j < 4; ++j) {
-                const int jn = (j < 3) ? j + 1 : 3;
-                const float ty_xp = (j < 3) ? c_ty.v[jn] : r_ty, tz_xp = (j < 3) ? c_tz.v[jn] : r_tz;
+            for (int j = 0; j < SPT; ++j) {
+                const int jn = (j < SPT - 1) ? j + 1 : SPT - 1;
+                const float ty_xp = (j < SPT - 1) ? c_ty.v[jn] : r_ty, tz_xp = (j < SPT - 1) ? c_tz.v[jn] : r_tz;
                 S_xy.v[j] = plaq_angle_f32(c_tx.v[j], ty_xp, y_tx.v[j], c_ty.v[j]);
                 S_xz.v[j] = plaq_angle_f32(c_tx.v[j], tz_xp, n_tx.v[j], c_tz.v[j]);
                 S_yz.v[j] = plaq_angle_f32(c_ty.v[j], y_tz.v[j], n_ty.v[j], c_tz.v[j]);
@@ -481,9 +512,9 @@ tiled_step_kernel(ConstFields<float> in, Fields<float> out, StepCoef<float> k, i
             }
             if (COMPACT) {
                 // two angles per issued instruction (FFMA2); bit-identical to the scalar polynomials
-                auto sines = [&](V4 &a, bool small) {
+                auto sines = [&](VS &a, bool small) {
 #pragma unroll
-                    for (int h = 0; h < 4; h += 2) {
+                    for (int h = 0; h < SPT; h += 2) {
                         const f32x2 x = pack2(a.v[h], a.v[h + 1]);
                         unpack2(small ? sin_small_f32x2(x) : sin_poly_f32x2(x), a.v[h], a.v[h + 1]);
                     }
@@ -496,11 +527,11 @@ tiled_step_kernel(ConstFields<float> in, Fields<float> out, StepCoef<float> k, i
             }
 
             // link variables of the 4 sites (Eq. 12), two angles per issued instruction
-            V4 s_x, c_x, s_y, c_y, s_z, c_z;
+            VS s_x, c_x, s_y, c_y, s_z, c_z;
             {
-                auto sincos4 = [&](const V4 &t, V4 &sn, V4 &cs) {
+                auto sincos4 = [&](const VS &t, VS &sn, VS &cs) {
 #pragma unroll
-                    for (int h = 0; h < 4; h += 2) {
+                    for (int h = 0; h < SPT; h += 2) {
                         f32x2 s2, c2;
                         sincos_pi_f32x2(pack2(t.v[h], t.v[h + 1]), s2, c2);
                         unpack2(s2, sn.v[h], sn.v[h + 1]);
@@ -511,13 +542,13 @@ tiled_step_kernel(ConstFields<float> in, Fields<float> out, StepCoef<float> k, i
                 sincos4(c_ty, s_y, c_y);
                 sincos4(c_tz, s_z, c_z);
             }
-            V4 d_g2;   // DIAG: gradient energy of the 4 sites, for the read-out loop
+            VS d_g2;   // DIAG: gradient energy of the 4 sites, for the read-out loop
 #pragma unroll
-            for (int j = 0; j < 4; ++j) {
+            for (int j = 0; j < SPT; ++j) {
                 const float fr = c_pr.v[j], fi = c_pi.v[j];
                 const float tx = c_tx.v[j], ty = c_ty.v[j], tz = c_tz.v[j];
-                const int jn = (j < 3) ? j + 1 : 3;
-                const float xr = (j < 3) ? c_pr.v[jn] : r_pr, xi = (j < 3) ? c_pi.v[jn] : r_pi;
+                const int jn = (j < SPT - 1) ? j + 1 : SPT - 1;
+                const float xr = (j < SPT - 1) ? c_pr.v[jn] : r_pr, xi = (j < SPT - 1) ? c_pi.v[jn] : r_pi;
                 const float Sxy = S_xy.v[j], Sxz = S_xz.v[j], Syz = S_yz.v[j];
                 const float sx = s_x.v[j], cx = c_x.v[j], sy = s_y.v[j], cy = c_y.v[j], sz = s_z.v[j], cz = c_z.v[j];
                 // forward hops U_i(s) phi(s+i)                                   (Eq. 13)
@@ -553,10 +584,10 @@ tiled_step_kernel(ConstFields<float> in, Fields<float> out, StepCoef<float> k, i
             }
             // y-1 hand-over for the row above
             if (w + 1 < TY) {
-                sm.row[buf][w + 1][0][lane] = f4(o_byr);
-                sm.row[buf][w + 1][1][lane] = f4(o_byi);
-                sm.row[buf][w + 1][2][lane] = f4(o_sxy);
-                sm.row[buf][w + 1][3][lane] = f4(o_syz);
+                stN<SPT>(&sm.row[buf][w + 1][0][SPT * lane], o_byr);
+                stN<SPT>(&sm.row[buf][w + 1][1][SPT * lane], o_byi);
+                stN<SPT>(&sm.row[buf][w + 1][2][SPT * lane], o_sxy);
+                stN<SPT>(&sm.row[buf][w + 1][3][SPT * lane], o_syz);
             }
             // x-1 terms of the first site: lane-1's last site (lane 0: the helper's column entry, after the barrier)
             l_bxr = __shfl_up_sync(FULL, l_bxr, 1);
@@ -574,10 +605,8 @@ tiled_step_kernel(ConstFields<float> in, Fields<float> out, StepCoef<float> k, i
             __syncthreads();
             if (DIAG && n + 2 <= nplanes + 1) produce();
             // add what row y-1 (and, lane 0, site x0-1) hands over, finish Eqs. 7-10, store
-            const float4 a = sm.row[buf][w][0][lane], b = sm.row[buf][w][1][lane];
-            const float4 c = sm.row[buf][w][2][lane], d = sm.row[buf][w][3][lane];
-            const float av[4] = {a.x, a.y, a.z, a.w}, bv[4] = {b.x, b.y, b.z, b.w};
-            const float cv[4] = {c.x, c.y, c.z, c.w}, dv[4] = {d.x, d.y, d.z, d.w};
+            const VS av = ldsN<SPT>(&sm.row[buf][w][0][SPT * lane]), bv = ldsN<SPT>(&sm.row[buf][w][1][SPT * lane]);
+            const VS cv = ldsN<SPT>(&sm.row[buf][w][2][SPT * lane]), dv = ldsN<SPT>(&sm.row[buf][w][3][SPT * lane]);
             if (lane == 0) {
                 const float4 cdat = sm.col[buf][w];
                 P_r.v[0] += kA * cdat.x;
@@ -587,17 +616,17 @@ tiled_step_kernel(ConstFields<float> in, Fields<float> out, StepCoef<float> k, i
             }
             // old Pi, ep of the own sites: staged one plane ahead by this warp
             mbar_wait(&sm.qfull[w], (n - 1) & 1);
-            const V4 q_r = lds4(&sm.qe[w][0][4 * lane]), q_i = lds4(&sm.qe[w][1][4 * lane]);
-            const V4 e_x = lds4(&sm.qe[w][2][4 * lane]), e_y = lds4(&sm.qe[w][3][4 * lane]);
-            const V4 e_z = lds4(&sm.qe[w][4][4 * lane]);
-            V4 f_r, f_i, t_x, t_y, t_z;
+            const VS q_r = ldsN<SPT>(&sm.qe[w][0][SPT * lane]), q_i = ldsN<SPT>(&sm.qe[w][1][SPT * lane]);
+            const VS e_x = ldsN<SPT>(&sm.qe[w][2][SPT * lane]), e_y = ldsN<SPT>(&sm.qe[w][3][SPT * lane]);
+            const VS e_z = ldsN<SPT>(&sm.qe[w][4][SPT * lane]);
+            VS f_r, f_i, t_x, t_y, t_z;
 #pragma unroll
-            for (int j = 0; j < 4; ++j) {
-                P_r.v[j] = k.c1 * q_r.v[j] + (P_r.v[j] + kA * av[j]);
-                P_i.v[j] = k.c1 * q_i.v[j] + (P_i.v[j] + kA * bv[j]);
-                E_x.v[j] = k.w1 * e_x.v[j] + (E_x.v[j] + kB * cv[j]);
+            for (int j = 0; j < SPT; ++j) {
+                P_r.v[j] = k.c1 * q_r.v[j] + (P_r.v[j] + kA * av.v[j]);
+                P_i.v[j] = k.c1 * q_i.v[j] + (P_i.v[j] + kA * bv.v[j]);
+                E_x.v[j] = k.w1 * e_x.v[j] + (E_x.v[j] + kB * cv.v[j]);
                 E_y.v[j] = k.w1 * e_y.v[j] + E_y.v[j];
-                E_z.v[j] = k.w1 * e_z.v[j] + (E_z.v[j] - kB * dv[j]);
+                E_z.v[j] = k.w1 * e_z.v[j] + (E_z.v[j] - kB * dv.v[j]);
                 f_r.v[j] = c_pr.v[j] + k.dt * P_r.v[j];   // Eq. 9
                 f_i.v[j] = c_pi.v[j] + k.dt * P_i.v[j];
                 t_x.v[j] = c_tx.v[j] + k.dt * E_x.v[j];   // Eq. 10
@@ -608,23 +637,23 @@ tiled_step_kernel(ConstFields<float> in, Fields<float> out, StepCoef<float> k, i
             // with the next plane's row, which then has almost a whole iteration to land (DIAG: after the read-outs)
             __syncwarp();
             if (!DIAG && n + 1 <= nplanes) produce_q();
-            st4(out.f[PI_RE] + oc, P_r);
-            st4(out.f[PI_IM] + oc, P_i);
-            st4(out.f[EP_X] + oc, E_x);
-            st4(out.f[EP_Y] + oc, E_y);
-            st4(out.f[EP_Z] + oc, E_z);
-            st4(out.f[PHI_RE] + oc, f_r);
-            st4(out.f[PHI_IM] + oc, f_i);
-            st4(out.f[TH_X] + oc, t_x);
-            st4(out.f[TH_Y] + oc, t_y);
-            st4(out.f[TH_Z] + oc, t_z);
+            stN<SPT>(out.f[PI_RE] + oc, P_r);
+            stN<SPT>(out.f[PI_IM] + oc, P_i);
+            stN<SPT>(out.f[EP_X] + oc, E_x);
+            stN<SPT>(out.f[EP_Y] + oc, E_y);
+            stN<SPT>(out.f[EP_Z] + oc, E_z);
+            stN<SPT>(out.f[PHI_RE] + oc, f_r);
+            stN<SPT>(out.f[PHI_IM] + oc, f_i);
+            stN<SPT>(out.f[TH_X] + oc, t_x);
+            stN<SPT>(out.f[TH_Y] + oc, t_y);
+            stN<SPT>(out.f[TH_Z] + oc, t_z);
             if constexpr (DIAG) {
                 // ---- read-outs D1-D3 of the entry snapshot of this plane: lane l takes the sites l + 32 j of the row
                 // scratch: this warp's hand-over row, consumed above and free until iteration n + 2: 4 x 128 floats
                 float *scr = reinterpret_cast<float *>(&sm.row[buf][w][0][0]);
-                st4(scr + 4 * lane, d_g2);
-                *reinterpret_cast<float4 *>(scr + TILE_X + 4 * lane) = d_eby;
-                *reinterpret_cast<float4 *>(scr + 2 * TILE_X + 4 * lane) = d_ebz;
+                stN<SPT>(scr + SPT * lane, d_g2);
+                stN<SPT>(scr + TX + SPT * lane, d_eby);
+                stN<SPT>(scr + 2 * TX + SPT * lane, d_ebz);
                 const float ex_left = d_exl;
                 __syncwarp();
                 float wnd[3];
@@ -635,9 +664,9 @@ tiled_step_kernel(ConstFields<float> in, Fields<float> out, StepCoef<float> k, i
 #pragma unroll
                 for (int a = 0; a < DS_NFLT; ++a) acc[a] = sm.dacc[a][threadIdx.x];
 #pragma unroll 1
-                for (int j = 0; j < 4; ++j) {
+                for (int j = 0; j < SPT; ++j) {
                     const int cq = lane + 32 * j, c = HALO + cq;
-                    const float eby = scr[TILE_X + cq], ebz = scr[2 * TILE_X + cq];
+                    const float eby = scr[TX + cq], ebz = scr[2 * TX + cq];
                     // D1: winding of the three plaquettes the site owns (Eq. 16 right)
                     const float t0x = sm.raw[so][2][r_own][c], t0y = sm.raw[so][3][r_own][c], t0z = sm.raw[so][4][r_own][c];
                     const float ty_xp = sm.raw[so][3][r_own][c + 1], tz_xp = sm.raw[so][4][r_own][c + 1];
@@ -678,14 +707,11 @@ tiled_step_kernel(ConstFields<float> in, Fields<float> out, StepCoef<float> k, i
                 if (n + 1 <= nplanes) produce_q();
             }
             // the forward plane becomes the own plane
-            c_pr = lds4(&sm.raw[sf][0][r_own][cofs]); c_pi = lds4(&sm.raw[sf][1][r_own][cofs]);
-            c_tx = lds4(&sm.raw[sf][2][r_own][cofs]); c_ty = lds4(&sm.raw[sf][3][r_own][cofs]);
-            c_tz = lds4(&sm.raw[sf][4][r_own][cofs]);
+            c_pr = ldsN<SPT>(&sm.raw[sf][0][r_own][cofs]); c_pi = ldsN<SPT>(&sm.raw[sf][1][r_own][cofs]);
+            c_tx = ldsN<SPT>(&sm.raw[sf][2][r_own][cofs]); c_ty = ldsN<SPT>(&sm.raw[sf][3][r_own][cofs]);
+            c_tz = ldsN<SPT>(&sm.raw[sf][4][r_own][cofs]);
             if (n < nplanes) {
-                if (!(fmaxf(fmaxf(fmaxf(fabsf(c_tx.v[0]), fabsf(c_tx.v[1])), fmaxf(fabsf(c_tx.v[2]), fabsf(c_tx.v[3]))),
-                            fmaxf(fmaxf(fmaxf(fabsf(c_ty.v[0]), fabsf(c_ty.v[1])), fmaxf(fabsf(c_ty.v[2]), fabsf(c_ty.v[3]))),
-                                  fmaxf(fmaxf(fabsf(c_tz.v[0]), fabsf(c_tz.v[1])), fmaxf(fabsf(c_tz.v[2]), fabsf(c_tz.v[3]))))) <
-                      AH_TILED_TH_LIMIT))
+                if (!(fmaxf(vmaxabs<SPT>(c_tx), fmaxf(vmaxabs<SPT>(c_ty), vmaxabs<SPT>(c_tz))) < AH_TILED_TH_LIMIT))
                     *overflow = 1;
             }
         }
@@ -743,24 +769,35 @@ tiled_step_kernel(ConstFields<float> in, Fields<float> out, StepCoef<float> k, i
 constexpr int TILE_Y = 6;        // plain step: 6 main warps + 1 helper = 224 threads, 2 CTAs per SM (106 KB shared memory each)
 constexpr int TILE_Y_DIAG = 5;   // fused read-outs: the site-phase ring and the parked partial sums take the room of one row
 
-bool tiled_supported(int nx, int ny, int nz) { return nx >= TILE_X && nx % TILE_X == 0 && ny >= 1 && nz >= 1; }
+// sites per thread: 4 (128-site warp rows, 128-bit accesses) when nx allows it, else 2 (64-site rows, 64-bit accesses)
+static int spt_for(int nx) { return nx % 128 == 0 ? 4 : 2; }
 
-template <int TY, bool COMPACT, bool DIAG>
+bool tiled_supported(int nx, int ny, int nz) { return nx >= 64 && nx % 64 == 0 && ny >= 1 && nz >= 1; }
+
+template <int SPT, int TY, bool COMPACT, bool DIAG>
 static cudaError_t setup_one()
 {
-    cudaError_t e = cudaFuncSetAttribute(tiled_step_kernel<TY, COMPACT, DIAG>,
-                                         cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Smem<TY, DIAG>));
+    cudaError_t e = cudaFuncSetAttribute(tiled_step_kernel<SPT, TY, COMPACT, DIAG>,
+                                         cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Smem<SPT, TY, DIAG>));
     if (e != cudaSuccess) return e;
-    return cudaFuncSetAttribute(tiled_step_kernel<TY, COMPACT, DIAG>,
+    return cudaFuncSetAttribute(tiled_step_kernel<SPT, TY, COMPACT, DIAG>,
                                 cudaFuncAttributePreferredSharedMemoryCarveout, 100);
+}
+
+template <int SPT>
+static cudaError_t setup_spt()
+{
+    cudaError_t e = setup_one<SPT, TILE_Y, true, false>();
+    if (e == cudaSuccess) e = setup_one<SPT, TILE_Y, false, false>();
+    if (e == cudaSuccess) e = setup_one<SPT, TILE_Y_DIAG, true, true>();
+    if (e == cudaSuccess) e = setup_one<SPT, TILE_Y_DIAG, false, true>();
+    return e;
 }
 
 cudaError_t tiled_setup()
 {
-    cudaError_t e = setup_one<TILE_Y, true, false>();
-    if (e == cudaSuccess) e = setup_one<TILE_Y, false, false>();
-    if (e == cudaSuccess) e = setup_one<TILE_Y_DIAG, true, true>();
-    if (e == cudaSuccess) e = setup_one<TILE_Y_DIAG, false, true>();
+    cudaError_t e = setup_spt<4>();
+    if (e == cudaSuccess) e = setup_spt<2>();
     return e;
 }
 
@@ -777,7 +814,7 @@ cudaError_t tiled_setup()
 #endif
 static int chunk_for(int nx, int ny, int nz, int ty)
 {
-    const long long cols = (long long)(nx / TILE_X) * ((ny + ty - 1) / ty);
+    const long long cols = (long long)(nx / (32 * spt_for(nx))) * ((ny + ty - 1) / ty);
     const long long resident = 148LL * 2;
     int best = nz < 8 ? nz : 8;
     double best_cost = 1e300;
@@ -804,20 +841,31 @@ int tiled_num_blocks(int nx, int ny, int nz, bool diag)
     if (!tiled_supported(nx, ny, nz)) return 0;
     const int ty = diag ? TILE_Y_DIAG : TILE_Y;
     const int zc = chunk_for(nx, ny, nz, ty);
-    return (nx / TILE_X) * ((ny + ty - 1) / ty) * ((nz + zc - 1) / zc);
+    return (nx / (32 * spt_for(nx))) * ((ny + ty - 1) / ty) * ((nz + zc - 1) / zc);
 }
 
-template <int TY, bool COMPACT, bool DIAG>
+template <int SPT, int TY, bool COMPACT, bool DIAG>
 static cudaError_t launch_one(const ConstFields<float> &in, const Fields<float> &out, const StepCoef<float> &k, int nx,
                               int ny, int nz, int *overflow, cudaStream_t st, const DiagCoef &d, DiagPartial *partials)
 {
     const int zc = chunk_for(nx, ny, nz, TY);
-    dim3 grid(nx / TILE_X, (ny + TY - 1) / TY, (nz + zc - 1) / zc);
+    dim3 grid(nx / (32 * SPT), (ny + TY - 1) / TY, (nz + zc - 1) / zc);
     dim3 block((TY + 1) * 32);
     if (grid.y > 65535u || grid.z > 65535u) return cudaErrorInvalidConfiguration;
-    tiled_step_kernel<TY, COMPACT, DIAG><<<grid, block, sizeof(Smem<TY, DIAG>), st>>>(in, out, k, nx, ny, nz, zc, overflow,
-                                                                                    d, partials);
-    return cudaGetLastError();
+    return launch_pdl(tiled_step_kernel<SPT, TY, COMPACT, DIAG>, grid, block, sizeof(Smem<SPT, TY, DIAG>), st, in, out, k, nx,
+                      ny, nz, zc, overflow, d, partials);
+}
+
+template <int SPT>
+static cudaError_t launch_spt(const ConstFields<float> &in, const Fields<float> &out, const StepCoef<float> &k, int nx,
+                              int ny, int nz, int *overflow, cudaStream_t st, bool diag, const DiagCoef &d,
+                              DiagPartial *partials)
+{
+    if (k.compact)
+        return diag ? launch_one<SPT, TILE_Y_DIAG, true, true>(in, out, k, nx, ny, nz, overflow, st, d, partials)
+                    : launch_one<SPT, TILE_Y, true, false>(in, out, k, nx, ny, nz, overflow, st, d, nullptr);
+    return diag ? launch_one<SPT, TILE_Y_DIAG, false, true>(in, out, k, nx, ny, nz, overflow, st, d, partials)
+                : launch_one<SPT, TILE_Y, false, false>(in, out, k, nx, ny, nz, overflow, st, d, nullptr);
 }
 
 // partials == nullptr: plain step.  Otherwise the DIAG instantiation, which also writes one DiagPartial per
@@ -829,11 +877,8 @@ cudaError_t launch_tiled_step(const ConstFields<float> &in, const Fields<float> 
     if (!tiled_supported(nx, ny, nz)) return cudaErrorInvalidValue;
     const bool diag = partials != nullptr && dk != nullptr;
     const DiagCoef d = diag ? *dk : DiagCoef{};
-    if (k.compact)
-        return diag ? launch_one<TILE_Y_DIAG, true, true>(in, out, k, nx, ny, nz, overflow, st, d, partials)
-                    : launch_one<TILE_Y, true, false>(in, out, k, nx, ny, nz, overflow, st, d, nullptr);
-    return diag ? launch_one<TILE_Y_DIAG, false, true>(in, out, k, nx, ny, nz, overflow, st, d, partials)
-                : launch_one<TILE_Y, false, false>(in, out, k, nx, ny, nz, overflow, st, d, nullptr);
+    return spt_for(nx) == 4 ? launch_spt<4>(in, out, k, nx, ny, nz, overflow, st, diag, d, partials)
+                            : launch_spt<2>(in, out, k, nx, ny, nz, overflow, st, diag, d, partials);
 }
 
 }  // namespace ah

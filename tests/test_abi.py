@@ -71,8 +71,13 @@ def test_tiled_launch_geometry(ahlib):
     assert (zc, ctas) == (1, 1)
     zc, ctas = ahlib.tiled_launch_info(256, 16, 11)
     assert zc * -(-11 // zc) >= 11 and ctas == 2 * 3 * -(-11 // zc)
+    # 64-site warp rows when nx is a multiple of 64 but not of 128: one x tile per 64 sites
+    zc, ctas = ahlib.tiled_launch_info(64, 64, 64)
+    assert ctas == 1 * 11 * -(-64 // zc) and 4 <= zc <= 64
+    zc, ctas = ahlib.tiled_launch_info(192, 6, 4)
+    assert ctas == 3 * 1 * -(-4 // zc)
     with pytest.raises(ahlib.AhError):
-        ahlib.tiled_launch_info(64, 64, 64)
+        ahlib.tiled_launch_info(32, 64, 64)
     with pytest.raises(ahlib.AhError):
         ahlib.tiled_launch_info(200, 8, 8)
 

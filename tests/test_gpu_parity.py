@@ -50,7 +50,7 @@ def rel_max(a, b):
 
 def kernels_for(ah, nx):
     ks = [ah.KERNEL_SITE]
-    if nx % 128 == 0:
+    if nx % 64 == 0:
         ks.append(ah.KERNEL_TILED)
     return ks
 
@@ -137,7 +137,8 @@ def test_one_step_fp64_site_kernel(ah, oracle, case, shape):
 
 
 @pytest.mark.parametrize("case", ONE_STEP_CASES)
-@pytest.mark.parametrize("shape", [(20, 12, 7), (128, 9, 6), (256, 16, 11), (128, 8, 1), (128, 1, 5), (384, 3, 2)])
+@pytest.mark.parametrize("shape", [(20, 12, 7), (128, 9, 6), (256, 16, 11), (128, 8, 1), (128, 1, 5), (384, 3, 2),
+                                   (64, 9, 6), (192, 7, 5), (64, 1, 1)])    # the last three: 64-site warp rows
 def test_one_step_fp32(ah, oracle, case, shape):
     f0 = inputs.random_state(*shape, seed=7)
     for kern in kernels_for(ah, shape[0]):
@@ -217,6 +218,7 @@ def test_parity_config1_64cubed_100_and_160_steps(ah, oracle):
     north_star: max rel |d phi|, |d ep| <= 1e-4 after 100 steps."""
     n, dt, tau0 = 64, 0.1, 1.0
     sim, Po = both(ah, oracle, (n, n, n), p=1.0, s=0.0)
+    assert sim.get_kernel() == ah.KERNEL_TILED            # the product kernel (64-site warp rows), not the site kernel
     f = oracle.init_fields(Po, 1)
     sim.set_fields(f)                      # identical ICs: cos/sin values rounded once to fp32
     f = sim.get_fields().astype(np.float64)
