@@ -43,6 +43,16 @@ extern "C" {
 
 #define AH_NFIELDS 10
 
+/* ah_params.fp64 */
+#define AH_PRECISION_FP32 0
+#define AH_PRECISION_FP64 1
+#define AH_PRECISION_MIXED 2 /* fp32 storage, fp64 arithmetic; results rounded once, on the store */
+
+/* z slabs (below): fields whose boundary planes neighbours exchange, and the raw partial sums of a slab's read-outs */
+#define AH_NHALO 6      /* phi_re, phi_im, th_x, th_y, th_z, ep_z */
+#define AH_NDIAG_INT 5  /* |W| sums xy, xz, yz; near-branch count; big-plaquette count            */
+#define AH_NDIAG_FLT 7  /* sum |Pi|^2 L, sum grad2 L, sum L, sum G^2, sum div^2, sum charge^2, max |G| */
+
 typedef struct ah_ctx ah_ctx; /* opaque */
 
 /* Model and lattice parameters.  Plain data, host side. */
@@ -55,7 +65,8 @@ typedef struct {
     double tau_ref;     /* a(tau) = (tau/tau_ref)^p (reading #6); ignored when p == 0 or s == 0      */
     double alpha;       /* damping constant of PAPER.md:78; 2 = physical Hubble damping              */
     int32_t compact;    /* 1: sin(plaquette) force, 2(1-cos) energy (reading #10); 0: non-compact     */
-    int32_t fp64;       /* 0: fp32 state and arithmetic (the product); 1: fp64 state, site kernel only */
+    int32_t fp64;       /* AH_PRECISION_*: 0 fp32 state and arithmetic (the product); 1 fp64 state and arithmetic
+                           (site kernel); 2 fp32 state, every operation of the step in fp64 (site kernel)   */
 } ah_params;
 
 /* Diagnostics of one snapshot. */
@@ -137,6 +148,53 @@ int ah_step_diag(ah_ctx *ctx, int n, double tau, double dt, int every, ah_diag *
 /* Per-plaquette winding integers of the current snapshot: host_w3 receives 3 arrays (xy, xz, yz)
  * of nx*ny*nz int8; host_near3 (may be NULL) the near-branch flags as uint8.  Synchronous. */
 int ah_winding_field(ah_ctx *ctx, int8_t *host_w3, uint8_t *host_near3);
+
+/*
+ * ---- z slabs: one periodic lattice cut along z over several GPUs (the paper's domain decomposition, PAPER.md:122-142,
+ * in its natural single-node form: 1-D slabs, one exchange of boundary planes per step, overlapped with the update of
+ * the interior).  BASELINE's north_star keeps the measured build on ONE GPU; these calls are the correct-by-
+ * construction multi-GPU path (tests cut a lattice into slabs on one GPU and require bit-identical fields).
+ *
+ * A slab context owns nz_own consecutive planes z_first .. z_first+nz_own-1 of the global lattice params->nz and
+ * stores nz_own + 2 planes per array: plane 0 is the ghost copy of global plane z_first-1, planes 1 .. nz_own the
+ * own planes, plane nz_own+1 the ghost copy of global plane z_first+nz_own (indices modulo nz).  dev_bufs are 20
+ * caller-owned arrays of nx*ny*(nz_own+2) elements.  ah_init_fields fills own AND ghost planes (the generator is
+ * counter-based on the global site index); ah_set_fields / ah_get_fields move all nz_own+2 planes.
+ *
+ * Per step:   ah_slab_step(ctx, tau, dt, want_diag, comm_stream)
+ *             copy the planes ah_slab_halo_ptrs names, on comm_stream (NCCL send/recv between ranks, or plain
+ *               device copies between slabs of one process):  my send_lo -> lower neighbour's recv_hi,
+ *                                                              my send_hi -> upper neighbour's recv_lo
+ *             ah_slab_exchange_done(ctx, comm_stream)
+ * ah_slab_step updates the two boundary planes first, makes comm_stream wait for exactly those launches, then
+ * updates the interior on the context's stream, so the copies overlap the interior.  ah_slab_exchange_done makes the
+ * context's stream wait for what has been enqueued on comm_stream.  comm_stream may be the context's own stream
+ * (no overlap, no events).  ah_step / ah_step_diag / ah_diagnostics return AH_ESTATE on a slab context.
+ */
+int ah_create_slab(ah_ctx **out, const ah_params *global_params, int nz_own, int z_first, void *const dev_bufs[],
+                   int nbufs, size_t bytes_each, void *cuda_stream);
+
+/* One step of the slab's own planes.  want_diag != 0: also the read-outs D1-D3 of the ENTRY snapshot of the own
+ * planes (fused on the tiled kernel), left on the device for ah_slab_diag_partial. */
+int ah_slab_step(ah_ctx *ctx, double tau, double dt, int want_diag, void *comm_stream);
+
+/* Device pointers of the boundary / ghost planes of the CURRENT state, per exchanged field (AH_NHALO of them, order
+ * above), each plane_bytes = nx*ny*sizeof(element) long. */
+int ah_slab_halo_ptrs(ah_ctx *ctx, void *dev_send_lo[AH_NHALO], void *dev_send_hi[AH_NHALO], void *dev_recv_lo[AH_NHALO],
+                      void *dev_recv_hi[AH_NHALO], size_t *plane_bytes);
+
+int ah_slab_exchange_done(ah_ctx *ctx, void *comm_stream);
+
+/* Read-outs of the own planes of the current snapshot (standalone kernel), left on the device. */
+int ah_slab_diagnostics(ah_ctx *ctx, double tau, double dt);
+
+/* The slab's raw partial sums of the last requested read-out (synchronises the stream).  Slabs combine them by
+ * adding counts and sums[0..5] and taking the maximum of sums[6] (an all-reduce of 12 numbers), then ah_diag_finish. */
+int ah_slab_diag_partial(ah_ctx *ctx, int64_t host_counts[AH_NDIAG_INT], double host_sums[AH_NDIAG_FLT]);
+
+/* Totals of a whole lattice -> the ah_diag record; host arithmetic only: xi_W, xi_L, <v^2>_phi, Gauss norms. */
+int ah_diag_finish(const ah_params *global_params, const int64_t host_counts[AH_NDIAG_INT],
+                   const double host_sums[AH_NDIAG_FLT], double tau, ah_diag *host_out);
 
 /* Host-side coefficients as the kernels receive them (for tests): a, q = a^{2s}, delta, omega. */
 int ah_coeffs(const ah_params *params, double tau, double dt, double *a, double *q, double *delta,

@@ -22,12 +22,17 @@ LIB_PATH = _PKG / "libah_b200.so"
 
 AH_OK, AH_EINVAL, AH_ECUDA, AH_ESTATE = 0, -1, -2, -3
 AH_NFIELDS = 10
+AH_NHALO, AH_NDIAG_INT, AH_NDIAG_FLT = 6, 5, 7
+HALO_FIELDS = (0, 1, 4, 5, 6, 9)          # phi_re, phi_im, th_x, th_y, th_z, ep_z (include/ah_b200.h)
 KERNEL_AUTO, KERNEL_SITE, KERNEL_TILED = 0, 1, 2
+PRECISION_FP32, PRECISION_FP64, PRECISION_MIXED = 0, 1, 2
 
 FIELD_NAMES = ("phi_re", "phi_im", "pi_re", "pi_im", "th_x", "th_y", "th_z", "ep_x", "ep_y", "ep_z")
 
-# every symbol include/ah_b200.h declares (checked by tests/test_abi.py)
+# every symbol include/*.h declares (checked by tests/test_abi.py)
 EXPORTS = (
+    "ah_create_slab", "ah_slab_step", "ah_slab_halo_ptrs", "ah_slab_exchange_done", "ah_slab_diagnostics",
+    "ah_slab_diag_partial", "ah_diag_finish",
     "ah_create", "ah_destroy", "ah_init_fields", "ah_set_fields", "ah_get_fields", "ah_current_bufs",
     "ah_step", "ah_step_cooling", "ah_diagnostics", "ah_step_diag", "ah_winding_field", "ah_set_kernel", "ah_get_kernel",
     "ah_launch_count", "ah_tiled_launch_info", "ah_coeffs", "ah_test_trig", "ah_test_trig_fast", "ah_last_error", "ah_version",
@@ -84,6 +89,13 @@ def lib():
     L.ah_last_error.restype = C.c_char_p
     L.ah_version.restype = C.c_char_p
     L.ah_create.argtypes = [C.POINTER(vp), C.POINTER(Params), C.POINTER(vp), ip, C.c_size_t, vp]
+    L.ah_create_slab.argtypes = [C.POINTER(vp), C.POINTER(Params), ip, ip, C.POINTER(vp), ip, C.c_size_t, vp]
+    L.ah_slab_step.argtypes = [vp, dp, dp, ip, vp]
+    L.ah_slab_halo_ptrs.argtypes = [vp] + [C.POINTER(vp)] * 4 + [C.POINTER(C.c_size_t)]
+    L.ah_slab_exchange_done.argtypes = [vp, vp]
+    L.ah_slab_diagnostics.argtypes = [vp, dp, dp]
+    L.ah_slab_diag_partial.argtypes = [vp, C.POINTER(C.c_int64), C.POINTER(dp)]
+    L.ah_diag_finish.argtypes = [C.POINTER(Params), C.POINTER(C.c_int64), C.POINTER(dp), dp, C.POINTER(Diag)]
     L.ah_destroy.argtypes = [vp]
     L.ah_init_fields.argtypes = [vp, C.c_uint64]
     L.ah_set_fields.argtypes = [vp, vp]
@@ -118,8 +130,9 @@ def make_params(nx, ny=None, nz=None, dx=0.5, lambda0=2.0, e0=1.0, sigma=1.0, s=
                 tau_ref=1.0, alpha=2.0, compact=1, fp64=False) -> Params:
     ny = nx if ny is None else ny
     nz = nx if nz is None else nz
+    # fp64: False / True, or one of PRECISION_FP32 / PRECISION_FP64 / PRECISION_MIXED
     return Params(int(nx), int(ny), int(nz), float(dx), float(lambda0), float(e0), float(sigma),
-                  float(s), float(p), float(tau_ref), float(alpha), int(compact), int(bool(fp64)))
+                  float(s), float(p), float(tau_ref), float(alpha), int(compact), int(fp64))
 
 
 def tiled_launch_info(nx, ny, nz):
@@ -147,8 +160,8 @@ class Simulation:
         P = self.P
         self.torch = torch
         self.device = torch.device(device)
-        self.dtype = torch.float64 if P.fp64 else torch.float32
-        self.np_dtype = np.float64 if P.fp64 else np.float32
+        self.dtype = torch.float64 if P.fp64 == PRECISION_FP64 else torch.float32
+        self.np_dtype = np.float64 if P.fp64 == PRECISION_FP64 else np.float32
         self.n = P.nx * P.ny * P.nz
         self.shape = (AH_NFIELDS, P.nz, P.ny, P.nx)
         with torch.cuda.device(self.device):
@@ -263,6 +276,296 @@ class Simulation:
 
     def synchronize(self):
         self.stream.synchronize()
+
+
+def diag_finish(P: Params, counts, sums, tau: float) -> dict:
+    """ah_diag_finish: totals of a whole lattice -> the ah_diag record (host side of the library)."""
+    ci = (C.c_int64 * AH_NDIAG_INT)(*[int(v) for v in counts])
+    cf = (C.c_double * AH_NDIAG_FLT)(*[float(v) for v in sums])
+    d = Diag()
+    _check(lib().ah_diag_finish(C.byref(P), ci, cf, float(tau), C.byref(d)))
+    return d.asdict()
+
+
+def slab_planes(nz: int, nslabs: int, r: int):
+    """(first own plane, number of own planes) of slab r when nz planes are cut into nslabs nearly equal slabs."""
+    if not (1 <= nslabs <= nz and 0 <= r < nslabs):
+        raise ValueError("need 1 <= nslabs <= nz and 0 <= r < nslabs")
+    base, rem = divmod(nz, nslabs)
+    first = r * base + min(r, rem)
+    return first, base + (1 if r < rem else 0)
+
+
+class SlabSimulation:
+    """One z slab of a periodic lattice (ah_create_slab): own planes [z_first, z_first + nz_own) plus one ghost plane
+    on each side, 20 torch-owned buffers of nx*ny*(nz_own+2) elements.  Marshalling and stream plumbing only; the
+    exchange of the boundary planes is done by a SlabGroup (slabs of one process) or a DistributedSlab (one slab per
+    rank, torch.distributed)."""
+
+    def __init__(self, params: Params, nz_own: int, z_first: int, device="cuda:0", stream=None, comm_stream=None):
+        import torch
+
+        if not torch.cuda.is_available():
+            raise RuntimeError("paper_2005_14454_b200 needs a CUDA device (B200); there is no CPU fallback")
+        self.P, self.nz_own, self.z_first = params, int(nz_own), int(z_first)
+        P = params
+        self.torch = torch
+        self.device = torch.device(device)
+        self.dtype = torch.float64 if P.fp64 == PRECISION_FP64 else torch.float32
+        self.np_dtype = np.float64 if P.fp64 == PRECISION_FP64 else np.float32
+        self.nza = self.nz_own + 2
+        self.n = P.nx * P.ny * self.nza
+        self.shape = (AH_NFIELDS, self.nza, P.ny, P.nx)
+        with torch.cuda.device(self.device):
+            self.bufs = [torch.empty(self.n, dtype=self.dtype, device=self.device) for _ in range(2 * AH_NFIELDS)]
+            self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
+            self.comm_stream = comm_stream if comm_stream is not None else self.stream
+            ptrs = (C.c_void_p * (2 * AH_NFIELDS))(*[b.data_ptr() for b in self.bufs])
+            self._ctx = C.c_void_p()
+            _check(lib().ah_create_slab(C.byref(self._ctx), C.byref(P), self.nz_own, self.z_first, ptrs, 2 * AH_NFIELDS,
+                                        self.n * self.bufs[0].element_size(), C.c_void_p(self.stream.cuda_stream)))
+
+    def close(self):
+        if getattr(self, "_ctx", None) is not None and self._ctx.value:
+            lib().ah_destroy(self._ctx)
+            self._ctx = C.c_void_p()
+        self.bufs = []
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def _dev(self):
+        return self.torch.cuda.device(self.device)
+
+    def init_fields(self, seed: int):
+        with self._dev():
+            _check(lib().ah_init_fields(self._ctx, C.c_uint64(seed)))
+
+    def set_fields(self, host):
+        a = np.ascontiguousarray(host, dtype=self.np_dtype)
+        if a.shape != self.shape:
+            raise ValueError(f"fields must have shape {self.shape}, got {a.shape}")
+        with self._dev():
+            _check(lib().ah_set_fields(self._ctx, a.ctypes.data))
+
+    def get_fields(self) -> np.ndarray:
+        out = np.empty(self.shape, dtype=self.np_dtype)
+        with self._dev():
+            _check(lib().ah_get_fields(self._ctx, out.ctypes.data))
+        return out
+
+    def step(self, tau: float, dt: float, want_diag: bool = False):
+        with self._dev():
+            _check(lib().ah_slab_step(self._ctx, float(tau), float(dt), int(bool(want_diag)),
+                                      C.c_void_p(self.comm_stream.cuda_stream)))
+
+    def halo_planes(self):
+        """(send_lo, send_hi, recv_lo, recv_hi): four lists of AH_NHALO torch views (one plane each) into the buffers
+        of the current state, found from the device pointers ah_slab_halo_ptrs returns."""
+        arrs = [(C.c_void_p * AH_NHALO)() for _ in range(4)]
+        nbytes = C.c_size_t(0)
+        _check(lib().ah_slab_halo_ptrs(self._ctx, *arrs, C.byref(nbytes)))
+        by_ptr = {b.data_ptr(): b for b in self.bufs}
+        plane = self.P.nx * self.P.ny
+        es = self.bufs[0].element_size()
+        assert nbytes.value == plane * es
+        out = []
+        for arr in arrs:
+            views = []
+            for p in arr:
+                base = max(q for q in by_ptr if q <= p)          # the buffer this plane lies in
+                off = (p - base) // es
+                views.append(by_ptr[base][off:off + plane])
+            out.append(views)
+        return out
+
+    def exchange_done(self):
+        with self._dev():
+            _check(lib().ah_slab_exchange_done(self._ctx, C.c_void_p(self.comm_stream.cuda_stream)))
+
+    def diagnostics_partial(self, tau: float, dt: float):
+        with self._dev():
+            _check(lib().ah_slab_diagnostics(self._ctx, float(tau), float(dt)))
+        return self.diag_partial()
+
+    def diag_partial(self):
+        ci = (C.c_int64 * AH_NDIAG_INT)()
+        cf = (C.c_double * AH_NDIAG_FLT)()
+        with self._dev():
+            _check(lib().ah_slab_diag_partial(self._ctx, ci, cf))
+        return list(ci), list(cf)
+
+    def launch_count(self) -> int:
+        return int(lib().ah_launch_count(self._ctx))
+
+    def get_kernel(self) -> int:
+        return int(lib().ah_get_kernel(self._ctx))
+
+
+def combine_partials(parts):
+    """Totals of per-slab (counts, sums): counts and sums[0..5] add, sums[6] (max |G|) takes the maximum."""
+    counts = [sum(p[0][a] for p in parts) for a in range(AH_NDIAG_INT)]
+    sums = [sum(p[1][a] for p in parts) for a in range(AH_NDIAG_FLT - 1)] + [max(p[1][AH_NDIAG_FLT - 1] for p in parts)]
+    return counts, sums
+
+
+class SlabGroup:
+    """All slabs of one lattice in ONE process (one GPU, or several GPUs of one process): the boundary planes are
+    exchanged by device-to-device copies on each slab's comm stream.  This is how the multi-GPU path is exercised
+    with a single GPU: the slabs' kernels are launched one after the other and never wait on one another."""
+
+    def __init__(self, params: Params, nslabs: int, devices=None, overlap=True):
+        import torch
+
+        self.P = params
+        devices = devices or ["cuda:0"] * nslabs
+        self.slabs = []
+        for r in range(nslabs):
+            first, own = slab_planes(params.nz, nslabs, r)
+            with torch.cuda.device(devices[r]):
+                comm = torch.cuda.Stream(device=devices[r]) if overlap else None
+            self.slabs.append(SlabSimulation(params, own, first, device=devices[r], comm_stream=comm))
+        self.torch = torch
+
+    def close(self):
+        for s in self.slabs:
+            s.close()
+
+    def init_fields(self, seed: int):
+        for s in self.slabs:
+            s.init_fields(seed)
+
+    def set_fields(self, host):
+        """host: the whole lattice (10, nz, ny, nx); every slab gets its own planes and its two ghost planes."""
+        nz = self.P.nz
+        for s in self.slabs:
+            idx = [(s.z_first - 1 + k) % nz for k in range(s.nza)]
+            s.set_fields(np.ascontiguousarray(np.asarray(host)[:, idx]))
+
+    def get_fields(self) -> np.ndarray:
+        out = np.empty((AH_NFIELDS, self.P.nz, self.P.ny, self.P.nx), dtype=self.slabs[0].np_dtype)
+        for s in self.slabs:
+            out[:, s.z_first:s.z_first + s.nz_own] = s.get_fields()[:, 1:-1]
+        return out
+
+    def _exchange(self):
+        R = len(self.slabs)
+        planes = [s.halo_planes() for s in self.slabs]
+        for r, s in enumerate(self.slabs):
+            lo, hi = (r - 1) % R, (r + 1) % R
+            with self.torch.cuda.stream(s.comm_stream):
+                # the copies run on the SENDER's comm stream (it waits for the sender's boundary planes); the
+                # receiver's compute stream is made to wait for them in exchange_done below
+                for a in range(AH_NHALO):
+                    planes[lo][3][a].copy_(planes[r][0][a], non_blocking=True)     # my first own plane -> lower's upper ghost
+                    planes[hi][2][a].copy_(planes[r][1][a], non_blocking=True)     # my last own plane  -> upper's lower ghost
+        # a slab's next step must see the ghost planes its neighbours wrote: wait on their comm streams too
+        for r, s in enumerate(self.slabs):
+            for nb in {(r - 1) % R, (r + 1) % R, r}:
+                ev = self.torch.cuda.Event()
+                ev.record(self.slabs[nb].comm_stream)
+                s.stream.wait_event(ev)
+            s.exchange_done()
+
+    def step(self, n: int, tau: float, dt: float, diag_every: int = 0):
+        """n steps; diag_every > 0 returns the records of the entry snapshots of steps 0, diag_every, ..."""
+        recs = []
+        for j in range(n):
+            tj = tau + j * dt
+            want = diag_every > 0 and j % diag_every == 0
+            # a slab's step reads its ghost planes, which the neighbours' comm streams wrote: ordering is in _exchange
+            for s in self.slabs:
+                s.step(tj, dt, want)
+            if want:
+                counts, sums = combine_partials([s.diag_partial() for s in self.slabs])
+                recs.append(diag_finish(self.P, counts, sums, tj))
+            self._exchange()
+        return recs
+
+    def diagnostics(self, tau: float, dt: float) -> dict:
+        counts, sums = combine_partials([s.diagnostics_partial(tau, dt) for s in self.slabs])
+        return diag_finish(self.P, counts, sums, tau)
+
+
+def halo_schedule(rank: int, world: int):
+    """Point-to-point operations of one boundary exchange for `rank` of `world` slabs (periodic in z), per exchanged
+    field: (kind, which plane list of SlabSimulation.halo_planes(), peer).  plane lists: 0 send_lo (first own plane),
+    1 send_hi (last own plane), 2 recv_lo (ghost below), 3 recv_hi (ghost above).  My first own plane is my lower
+    neighbour's upper ghost; my last own plane is my upper neighbour's lower ghost.  The order pairs every send with the
+    receive the peer posts at the same position (a rank's "send down / receive from above" meets the neighbour's),
+    so the schedule also works with blocking transports."""
+    if not (world >= 1 and 0 <= rank < world):
+        raise ValueError("need world >= 1 and 0 <= rank < world")
+    lo, hi = (rank - 1) % world, (rank + 1) % world
+    return [("send", 0, lo), ("recv", 3, hi), ("send", 1, hi), ("recv", 2, lo)]
+
+
+class DistributedSlab:
+    """One slab per rank (one process per GPU): boundary planes travel by torch.distributed point-to-point calls
+    (NCCL over NVLink on GPUs) on the comm stream, overlapped with the update of the interior; read-outs are combined
+    by two all-reduces (sum, max).  Host plumbing only."""
+
+    def __init__(self, params: Params, dist, device="cuda:0", overlap=True):
+        import torch
+
+        self.P, self.dist, self.torch = params, dist, torch
+        self.rank, self.world = dist.get_rank(), dist.get_world_size()
+        first, own = slab_planes(params.nz, self.world, self.rank)
+        with torch.cuda.device(device):
+            comm = torch.cuda.Stream(device=device) if overlap else None
+        self.slab = SlabSimulation(params, own, first, device=device, comm_stream=comm)
+
+    def exchange_ops(self, planes):
+        """The 4 * AH_NHALO point-to-point operations of one exchange, as (kind, tensor, peer) tuples; with world == 1
+        the slab is its own neighbour and the list is empty (plain copies are used instead)."""
+        ops = []
+        for a in range(AH_NHALO):
+            ops += [(kind, planes[which][a], peer) for kind, which, peer in halo_schedule(self.rank, self.world)]
+        return ops if self.world > 1 else []
+
+    def _exchange(self):
+        s, dist = self.slab, self.dist
+        planes = s.halo_planes()
+        with self.torch.cuda.stream(s.comm_stream):
+            if self.world == 1:
+                for a in range(AH_NHALO):
+                    planes[3][a].copy_(planes[0][a], non_blocking=True)
+                    planes[2][a].copy_(planes[1][a], non_blocking=True)
+            else:
+                reqs = dist.batch_isend_irecv([dist.P2POp(dist.isend if k == "send" else dist.irecv, t, peer)
+                                               for k, t, peer in self.exchange_ops(planes)])
+                for r in reqs:
+                    r.wait()
+        s.exchange_done()
+
+    def step(self, n: int, tau: float, dt: float, diag_every: int = 0):
+        recs = []
+        for j in range(n):
+            tj = tau + j * dt
+            want = diag_every > 0 and j % diag_every == 0
+            self.slab.step(tj, dt, want)
+            if want:
+                recs.append(self._reduce(self.slab.diag_partial(), tj))
+            self._exchange()
+        return recs
+
+    def _reduce(self, part, tau):
+        torch, dist = self.torch, self.dist
+        counts, sums = part
+        dev = self.slab.device if dist.get_backend() == "nccl" else "cpu"
+        add = torch.tensor([float(c) for c in counts] + sums[:-1], dtype=torch.float64, device=dev)   # counts < 2^53
+        mx = torch.tensor([sums[-1]], dtype=torch.float64, device=dev)
+        if self.world > 1:
+            dist.all_reduce(add, op=dist.ReduceOp.SUM)
+            dist.all_reduce(mx, op=dist.ReduceOp.MAX)
+        add = add.tolist()
+        return diag_finish(self.P, [int(round(v)) for v in add[:AH_NDIAG_INT]], add[AH_NDIAG_INT:] + [float(mx.item())], tau)
+
+    def diagnostics(self, tau: float, dt: float) -> dict:
+        return self._reduce(self.slab.diagnostics_partial(tau, dt), tau)
 
 
 def test_trig(x):

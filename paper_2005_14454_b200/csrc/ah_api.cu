@@ -91,12 +91,19 @@ ah::DiagCoef make_diag_coef(const ah_params &P, double tau, double dt)
 }  // namespace
 
 struct ah_ctx {
-    ah_params P;
+    ah_params P;       // the model; nx, ny, nz are the extents of the GLOBAL periodic lattice
     void *bufs[2 * AH_NFIELDS];
     int cur;           // 0: state in bufs[0..10), 1: in bufs[10..20)
     bool have_fields;
     cudaStream_t st;
-    size_t n;          // sites
+    // storage: nza planes of nx*ny sites per array.  Whole lattice: nza = nz, zr = {0, nz}.  z slab (ah_create_slab):
+    // nza = own planes + 2 ghost planes, zr = {1, nza - 1}, plane zl is global plane z_offset + zl.
+    int nza;
+    ah::ZRange zr;
+    int z_offset;
+    bool slab;
+    cudaEvent_t ev_boundary, ev_exchange;   // slab: boundary planes of the new state are final / ghost planes have landed
+    size_t n;          // sites stored per array (nx*ny*nza)
     size_t elem;       // bytes per element
     int kernel;        // resolved AH_KERNEL_SITE / AH_KERNEL_TILED
     int64_t launches;
@@ -133,6 +140,9 @@ ah::Fields<real> cur_fields_mut(const ah_ctx *c)
     return f;
 }
 
+bool is_fp64(const ah_params &P) { return P.fp64 == AH_PRECISION_FP64; }
+bool is_mixed(const ah_params &P) { return P.fp64 == AH_PRECISION_MIXED; }
+
 int check_time(const ah_ctx *c, double tau, double dt)
 {
     if (!(dt > 0.0) || !std::isfinite(dt) || !std::isfinite(tau))
@@ -142,69 +152,79 @@ int check_time(const ah_ctx *c, double tau, double dt)
     return AH_OK;
 }
 
+// Launches of one step over the planes zr of the current state into the other buffer set; no context state changes
+// here except the launch counter.  Tiled kernel: the fast path, then a conditional redo of the same planes with the
+// libm-based site kernel (runs only if the fast path flagged a link angle beyond its polynomial range).
 // diag_slot >= 0 (tiled fp32 kernel only): the fused DIAG instantiation also leaves the read-outs of the entry
-// snapshot in d_results[diag_slot] (SURVEY 8(a) row D-fuse).
-// Context state (ping-pong parity, flag parity, launch count) changes only after EVERY launch of the step was
+// snapshot of those planes in d_results[diag_slot] (SURVEY 8(a) row D-fuse).
+cudaError_t enqueue_step(ah_ctx *c, const ah_params &P, double tau, double dt, ah::ZRange zr, int diag_slot, int *flag,
+                         int *next_flag)
+{
+    cudaError_t e;
+    const int nx = P.nx, ny = P.ny, nza = c->nza;
+    if (is_fp64(P)) {
+        e = ah::launch_site_step<double>(cur_fields<double>(c), next_fields<double>(c), make_coef<double>(P, tau, dt), nx,
+                                         ny, nza, zr, c->st);
+        if (e == cudaSuccess) c->launches += 1;
+    } else if (is_mixed(P)) {
+        e = ah::launch_site_step_mixed(cur_fields<float>(c), next_fields<float>(c), make_coef<double>(P, tau, dt), nx, ny,
+                                       nza, zr, c->st);
+        if (e == cudaSuccess) c->launches += 1;
+    } else if (c->kernel == AH_KERNEL_TILED) {
+        const ah::StepCoef<float> k = make_coef<float>(P, tau, dt);
+        if (diag_slot >= 0) {
+            const ah::DiagCoef dk = make_diag_coef(P, tau, dt);
+            e = ah::launch_tiled_step(cur_fields<float>(c), next_fields<float>(c), k, nx, ny, nza, zr, flag, c->st, &dk,
+                                      c->d_partials);
+            // a link angle outside the tiled kernel's domain spoils its read-outs as well: the standalone kernel
+            // then re-evaluates the entry snapshot (conditional launch, exits at once when the flag is clear)
+            if (e == cudaSuccess) {
+                c->launches += 1;
+                e = ah::launch_diag_partials<float>(cur_fields<float>(c), dk, nx, ny, nza, zr, c->d_partials, nullptr,
+                                                    nullptr, flag, c->st);
+            }
+            if (e == cudaSuccess) {
+                c->launches += 1;
+                e = ah::launch_diag_final(c->d_partials, ah::tiled_num_blocks(nx, ny, zr.hi - zr.lo, true),
+                                          c->d_results + diag_slot, c->st, ah::diag_num_blocks(nx, ny, zr.hi - zr.lo), flag);
+            }
+        } else {
+            e = ah::launch_tiled_step(cur_fields<float>(c), next_fields<float>(c), k, nx, ny, nza, zr, flag, c->st);
+        }
+        if (e == cudaSuccess) {
+            c->launches += 1;
+            e = ah::launch_site_redo(flag, next_flag, cur_fields<float>(c), next_fields<float>(c), k, nx, ny, nza, zr, c->st);
+        }
+        if (e == cudaSuccess) c->launches += 1;
+    } else {
+        e = ah::launch_site_step<float>(cur_fields<float>(c), next_fields<float>(c), make_coef<float>(P, tau, dt), nx, ny,
+                                        nza, zr, c->st);
+        if (e == cudaSuccess) c->launches += 1;
+    }
+    return e;
+}
+
+// One whole step.  Context state (ping-pong parity, flag parity) changes only after EVERY launch of the step was
 // accepted; a failed launch leaves the context on the entry snapshot with both overflow flags cleared.
 // P: the model the step uses (the context's own, or ah_step_cooling's constant-damping copy of it)
 int one_step(ah_ctx *c, const ah_params &P, double tau, double dt, int diag_slot = -1)
 {
-    cudaError_t e;
-    int n_launched = 0;
-    if (P.fp64) {
-        e = ah::launch_site_step<double>(cur_fields<double>(c), next_fields<double>(c),
-                                         make_coef<double>(P, tau, dt), P.nx, P.ny, P.nz, c->st);
-        n_launched = 1;
-    } else if (c->kernel == AH_KERNEL_TILED) {
-        // fast path, then a conditional redo with the libm-based site kernel (runs only if the fast
-        // path flagged a link angle beyond its polynomial range; two flags alternate between steps)
-        const ah::StepCoef<float> k = make_coef<float>(P, tau, dt);
-        int *flag = c->d_overflow + c->step_parity, *next_flag = c->d_overflow + (1 - c->step_parity);
-        if (diag_slot >= 0) {
-            const ah::DiagCoef dk = make_diag_coef(P, tau, dt);
-            e = ah::launch_tiled_step(cur_fields<float>(c), next_fields<float>(c), k, P.nx, P.ny, P.nz, flag, c->st,
-                                      &dk, c->d_partials);
-            // a link angle outside the tiled kernel's domain spoils its read-outs as well: the standalone kernel
-            // then re-evaluates the entry snapshot (conditional launch, exits at once when the flag is clear)
-            if (e == cudaSuccess) {
-                ++n_launched;
-                e = ah::launch_diag_partials<float>(cur_fields<float>(c), dk, P.nx, P.ny, P.nz, c->d_partials, nullptr,
-                                                    nullptr, flag, c->st);
-            }
-            if (e == cudaSuccess) {
-                ++n_launched;
-                e = ah::launch_diag_final(c->d_partials, ah::tiled_num_blocks(P.nx, P.ny, P.nz, true),
-                                          c->d_results + diag_slot, c->st, ah::diag_num_blocks(P.nx, P.ny, P.nz), flag);
-            }
-        } else {
-            e = ah::launch_tiled_step(cur_fields<float>(c), next_fields<float>(c), k, P.nx, P.ny, P.nz, flag, c->st);
-        }
-        if (e == cudaSuccess) {
-            ++n_launched;
-            e = ah::launch_site_redo(flag, next_flag, cur_fields<float>(c), next_fields<float>(c), k, P.nx, P.ny,
-                                     P.nz, c->st);
-        }
-        if (e == cudaSuccess) {
-            ++n_launched;
-            c->step_parity = 1 - c->step_parity;
-        } else {
-            cudaMemsetAsync(c->d_overflow, 0, 2 * sizeof(int), c->st);   // a half-issued step must not leave a stale flag
-        }
-    } else {
-        e = ah::launch_site_step<float>(cur_fields<float>(c), next_fields<float>(c),
-                                        make_coef<float>(P, tau, dt), P.nx, P.ny, P.nz, c->st);
-        n_launched = 1;
+    int *flag = c->d_overflow + c->step_parity, *next_flag = c->d_overflow + (1 - c->step_parity);
+    const cudaError_t e = enqueue_step(c, P, tau, dt, c->zr, diag_slot, flag, next_flag);
+    if (e != cudaSuccess) {
+        cudaMemsetAsync(c->d_overflow, 0, 2 * sizeof(int), c->st);   // a half-issued step must not leave a stale flag
+        return cuda_fail(e, "step kernel launch");
     }
-    if (e != cudaSuccess) return cuda_fail(e, "step kernel launch");
-    c->launches += n_launched;
+    c->step_parity = 1 - c->step_parity;
     c->cur = 1 - c->cur;
     return AH_OK;
 }
 
 int ensure_diag_scratch(ah_ctx *c, int records)
 {
-    int nb = ah::diag_num_blocks(c->P.nx, c->P.ny, c->P.nz);
-    const int nbt = ah::tiled_num_blocks(c->P.nx, c->P.ny, c->P.nz, true);
+    const int own = c->zr.hi - c->zr.lo;
+    int nb = ah::diag_num_blocks(c->P.nx, c->P.ny, own);
+    const int nbt = ah::tiled_num_blocks(c->P.nx, c->P.ny, own, true);
     if (nbt > nb) nb = nbt;
     if (c->n_partials < nb) {
         if (c->d_partials) cudaFree(c->d_partials);
@@ -239,6 +259,7 @@ int check_diag_time(const ah_ctx *c, double tau, double dt)
     return AH_OK;
 }
 
+// standalone read-outs of the own planes of the current snapshot into d_results[slot]
 // winding_only: coefficients of the static a = 1 model (the winding integers depend on none of them)
 int enqueue_diag(ah_ctx *c, double tau, double dt, int slot, int8_t *w3, uint8_t *near3, bool winding_only = false)
 {
@@ -246,20 +267,20 @@ int enqueue_diag(ah_ctx *c, double tau, double dt, int slot, int8_t *w3, uint8_t
     if (winding_only) P.p = 0.0, P.s = 0.0;
     const ah::DiagCoef k = make_diag_coef(P, tau, dt);
     cudaError_t e;
-    if (P.fp64)
-        e = ah::launch_diag<double>(cur_fields<double>(c), k, P.nx, P.ny, P.nz, c->d_partials,
+    if (is_fp64(P))
+        e = ah::launch_diag<double>(cur_fields<double>(c), k, P.nx, P.ny, c->nza, c->zr, c->d_partials,
                                     c->d_results + slot, w3, near3, c->st);
     else
-        e = ah::launch_diag<float>(cur_fields<float>(c), k, P.nx, P.ny, P.nz, c->d_partials,
+        e = ah::launch_diag<float>(cur_fields<float>(c), k, P.nx, P.ny, c->nza, c->zr, c->d_partials,
                                    c->d_results + slot, w3, near3, c->st);
     if (e != cudaSuccess) return cuda_fail(e, "diagnostics kernel launch");
     c->launches += 2;
     return AH_OK;
 }
 
-void finish_diag(const ah_ctx *c, const ah::DiagPartial &r, double tau, ah_diag *out)
+// totals -> the derived numbers of ah_diag (P: the GLOBAL lattice the totals belong to)
+void finish_diag(const ah_params &P, const ah::DiagPartial &r, double tau, ah_diag *out)
 {
-    const ah_params &P = c->P;
     out->tau = tau;
     out->n_wind_xy = r.i[ah::DS_NW_XY];
     out->n_wind_xz = r.i[ah::DS_NW_XZ];
@@ -293,12 +314,95 @@ void finish_diag(const ah_ctx *c, const ah::DiagPartial &r, double tau, ah_diag 
     out->gauss_rel = den > 0.0 ? out->gauss_l2 / den : 0.0;
 }
 
+int check_params(const ah_params *P, const char *who)
+{
+    if (P->nx < 1 || P->ny < 1 || P->nz < 1)
+        return fail(AH_EINVAL, "%s: extents must be >= 1 (%d,%d,%d)", who, P->nx, P->ny, P->nz);
+    if (!(P->dx > 0.0) || !(P->e0 != 0.0) || !(P->alpha >= 0.0) || !std::isfinite(P->lambda0) ||
+        !std::isfinite(P->sigma) || !std::isfinite(P->s) || !std::isfinite(P->p))
+        return fail(AH_EINVAL, "%s: bad model parameters", who);
+    if (P->p != 0.0 && P->s != 0.0 && !(P->tau_ref > 0.0))
+        return fail(AH_EINVAL, "%s: tau_ref must be > 0 when p != 0 and s != 0", who);
+    if (P->fp64 != AH_PRECISION_FP32 && P->fp64 != AH_PRECISION_FP64 && P->fp64 != AH_PRECISION_MIXED)
+        return fail(AH_EINVAL, "%s: fp64 must be 0 (fp32), 1 (fp64) or 2 (fp32 storage, fp64 arithmetic)", who);
+    return AH_OK;
+}
+
+// nz_own planes starting at global plane z_first; slab: with one ghost plane on each side
+int create_ctx(ah_ctx **out, const ah_params *P, bool slab, int nz_own, int z_first, void *const dev_bufs[], int nbufs,
+               size_t bytes_each, void *cuda_stream, const char *who)
+{
+    if (!out || !P || !dev_bufs) return fail(AH_EINVAL, "%s: null pointer", who);
+    *out = nullptr;
+    int rc = check_params(P, who);
+    if (rc != AH_OK) return rc;
+    if (slab && (nz_own < 1 || z_first < 0 || z_first + nz_own > P->nz))
+        return fail(AH_EINVAL, "%s: slab planes [%d, %d) do not lie inside [0, %d)", who, z_first, z_first + nz_own, P->nz);
+    if (nbufs != 2 * AH_NFIELDS) return fail(AH_EINVAL, "%s: nbufs must be 20 (got %d)", who, nbufs);
+    const int nza = slab ? nz_own + 2 : P->nz;
+    const size_t n = (size_t)P->nx * P->ny * nza;
+    const size_t elem = is_fp64(*P) ? sizeof(double) : sizeof(float);
+    if (bytes_each != n * elem)
+        return fail(AH_EINVAL, "%s: bytes_each=%zu but nx*ny*planes*sizeof(elem)=%zu", who, bytes_each, n * elem);
+    for (int i = 0; i < nbufs; ++i) {
+        if (!dev_bufs[i]) return fail(AH_EINVAL, "%s: dev_bufs[%d] is null", who, i);
+        if (((uintptr_t)dev_bufs[i]) & 15u)
+            return fail(AH_EINVAL, "%s: dev_bufs[%d] is not 16-byte aligned", who, i);
+        for (int j = 0; j < i; ++j)
+            if (dev_bufs[i] == dev_bufs[j]) return fail(AH_EINVAL, "%s: dev_bufs[%d] == dev_bufs[%d]", who, i, j);
+    }
+    int ndev = 0;
+    AH_CUDA(cudaGetDeviceCount(&ndev));
+    if (ndev < 1) return fail(AH_ECUDA, "%s: no CUDA device", who);
+
+    ah_ctx *c = new (std::nothrow) ah_ctx;
+    if (!c) return fail(AH_ECUDA, "%s: out of host memory", who);
+    std::memset(c, 0, sizeof(*c));
+    c->P = *P;
+    for (int i = 0; i < nbufs; ++i) c->bufs[i] = dev_bufs[i];
+    c->st = (cudaStream_t)cuda_stream;
+    c->nza = nza;
+    c->zr = slab ? ah::ZRange{1, nza - 1} : ah::ZRange{0, nza};
+    c->z_offset = slab ? z_first - 1 : 0;
+    c->slab = slab;
+    c->n = n;
+    c->elem = elem;
+    const bool can_tile = P->fp64 == AH_PRECISION_FP32 && ah::tiled_supported(P->nx, P->ny, nza);
+    c->kernel = can_tile ? AH_KERNEL_TILED : AH_KERNEL_SITE;
+    if (c->kernel == AH_KERNEL_TILED) {
+        cudaError_t e = ah::tiled_setup();
+        if (e != cudaSuccess) {
+            delete c;
+            return cuda_fail(e, "tiled kernel setup");
+        }
+    }
+    rc = ensure_diag_scratch(c, 256);
+    if (rc != AH_OK) {
+        ah_destroy(c);
+        return rc;
+    }
+    {
+        cudaError_t e = cudaMalloc(&c->d_overflow, 2 * sizeof(int));
+        if (e == cudaSuccess) e = cudaMemsetAsync(c->d_overflow, 0, 2 * sizeof(int), c->st);
+        if (e == cudaSuccess && slab) e = cudaEventCreateWithFlags(&c->ev_boundary, cudaEventDisableTiming);
+        if (e == cudaSuccess && slab) e = cudaEventCreateWithFlags(&c->ev_exchange, cudaEventDisableTiming);
+        if (e != cudaSuccess) {
+            ah_destroy(c);
+            return cuda_fail(e, "context scratch");
+        }
+    }
+    *out = c;
+    return AH_OK;
+}
+
+const int HALO_FIELDS[AH_NHALO] = {ah::PHI_RE, ah::PHI_IM, ah::TH_X, ah::TH_Y, ah::TH_Z, ah::EP_Z};
+
 }  // namespace
 
 extern "C" {
 
 const char *ah_last_error(void) { return g_err; }
-const char *ah_version(void) { return "ah_b200 0.1 (sm_100a)"; }
+const char *ah_version(void) { return "ah_b200 0.2 (sm_100a)"; }
 
 int ah_coeffs(const ah_params *P, double tau, double dt, double *a, double *q, double *delta,
               double *omega)
@@ -312,62 +416,14 @@ int ah_coeffs(const ah_params *P, double tau, double dt, double *a, double *q, d
 int ah_create(ah_ctx **out, const ah_params *P, void *const dev_bufs[], int nbufs, size_t bytes_each,
               void *cuda_stream)
 {
-    if (!out || !P || !dev_bufs) return fail(AH_EINVAL, "ah_create: null pointer");
-    *out = nullptr;
-    if (P->nx < 1 || P->ny < 1 || P->nz < 1)
-        return fail(AH_EINVAL, "ah_create: extents must be >= 1 (%d,%d,%d)", P->nx, P->ny, P->nz);
-    if (!(P->dx > 0.0) || !(P->e0 != 0.0) || !(P->alpha >= 0.0) || !std::isfinite(P->lambda0) ||
-        !std::isfinite(P->sigma) || !std::isfinite(P->s) || !std::isfinite(P->p))
-        return fail(AH_EINVAL, "ah_create: bad model parameters");
-    if (P->p != 0.0 && P->s != 0.0 && !(P->tau_ref > 0.0))
-        return fail(AH_EINVAL, "ah_create: tau_ref must be > 0 when p != 0 and s != 0");
-    if (nbufs != 2 * AH_NFIELDS) return fail(AH_EINVAL, "ah_create: nbufs must be 20 (got %d)", nbufs);
-    const size_t n = (size_t)P->nx * P->ny * P->nz;
-    const size_t elem = P->fp64 ? sizeof(double) : sizeof(float);
-    if (bytes_each != n * elem)
-        return fail(AH_EINVAL, "ah_create: bytes_each=%zu but nx*ny*nz*sizeof(elem)=%zu", bytes_each, n * elem);
-    for (int i = 0; i < nbufs; ++i) {
-        if (!dev_bufs[i]) return fail(AH_EINVAL, "ah_create: dev_bufs[%d] is null", i);
-        if (((uintptr_t)dev_bufs[i]) & 15u)
-            return fail(AH_EINVAL, "ah_create: dev_bufs[%d] is not 16-byte aligned", i);
-        for (int j = 0; j < i; ++j)
-            if (dev_bufs[i] == dev_bufs[j]) return fail(AH_EINVAL, "ah_create: dev_bufs[%d] == dev_bufs[%d]", i, j);
-    }
-    int ndev = 0;
-    AH_CUDA(cudaGetDeviceCount(&ndev));
-    if (ndev < 1) return fail(AH_ECUDA, "ah_create: no CUDA device");
+    return create_ctx(out, P, false, P ? P->nz : 0, 0, dev_bufs, nbufs, bytes_each, cuda_stream, "ah_create");
+}
 
-    ah_ctx *c = new (std::nothrow) ah_ctx;
-    if (!c) return fail(AH_ECUDA, "ah_create: out of host memory");
-    std::memset(c, 0, sizeof(*c));
-    c->P = *P;
-    for (int i = 0; i < nbufs; ++i) c->bufs[i] = dev_bufs[i];
-    c->st = (cudaStream_t)cuda_stream;
-    c->n = n;
-    c->elem = elem;
-    c->kernel = (!P->fp64 && ah::tiled_supported(P->nx, P->ny, P->nz)) ? AH_KERNEL_TILED : AH_KERNEL_SITE;
-    if (c->kernel == AH_KERNEL_TILED) {
-        cudaError_t e = ah::tiled_setup();
-        if (e != cudaSuccess) {
-            delete c;
-            return cuda_fail(e, "tiled kernel setup");
-        }
-    }
-    int rc = ensure_diag_scratch(c, 256);
-    if (rc != AH_OK) {
-        ah_destroy(c);
-        return rc;
-    }
-    {
-        cudaError_t e = cudaMalloc(&c->d_overflow, 2 * sizeof(int));
-        if (e == cudaSuccess) e = cudaMemsetAsync(c->d_overflow, 0, 2 * sizeof(int), c->st);
-        if (e != cudaSuccess) {
-            ah_destroy(c);
-            return cuda_fail(e, "overflow flags");
-        }
-    }
-    *out = c;
-    return AH_OK;
+int ah_create_slab(ah_ctx **out, const ah_params *global_params, int nz_own, int z_first, void *const dev_bufs[],
+                   int nbufs, size_t bytes_each, void *cuda_stream)
+{
+    return create_ctx(out, global_params, true, nz_own, z_first, dev_bufs, nbufs, bytes_each, cuda_stream,
+                      "ah_create_slab");
 }
 
 int ah_destroy(ah_ctx *c)
@@ -377,6 +433,8 @@ int ah_destroy(ah_ctx *c)
     if (c->d_results) cudaFree(c->d_results);
     if (c->h_results) cudaFreeHost(c->h_results);
     if (c->d_overflow) cudaFree(c->d_overflow);
+    if (c->ev_boundary) cudaEventDestroy(c->ev_boundary);
+    if (c->ev_exchange) cudaEventDestroy(c->ev_exchange);
     delete c;
     return AH_OK;
 }
@@ -384,7 +442,7 @@ int ah_destroy(ah_ctx *c)
 int ah_set_kernel(ah_ctx *c, int kernel)
 {
     if (!c) return fail(AH_EINVAL, "ah_set_kernel: null context");
-    const bool can_tile = !c->P.fp64 && ah::tiled_supported(c->P.nx, c->P.ny, c->P.nz);
+    const bool can_tile = c->P.fp64 == AH_PRECISION_FP32 && ah::tiled_supported(c->P.nx, c->P.ny, c->nza);
     if (kernel == AH_KERNEL_AUTO) kernel = can_tile ? AH_KERNEL_TILED : AH_KERNEL_SITE;
     if (kernel == AH_KERNEL_TILED) {
         if (!can_tile) return fail(AH_EINVAL, "ah_set_kernel: tiled kernel needs fp32 and nx %% 64 == 0");
@@ -399,7 +457,7 @@ int ah_set_kernel(ah_ctx *c, int kernel)
 int ah_get_kernel(const ah_ctx *c)
 {
     if (!c) return fail(AH_EINVAL, "ah_get_kernel: null context");
-    return c->P.fp64 ? AH_KERNEL_SITE : c->kernel;
+    return c->P.fp64 != AH_PRECISION_FP32 ? AH_KERNEL_SITE : c->kernel;
 }
 
 int ah_tiled_launch_info(int nx, int ny, int nz, int *planes_per_cta, int *n_ctas)
@@ -417,8 +475,11 @@ int ah_init_fields(ah_ctx *c, uint64_t seed)
 {
     if (!c) return fail(AH_EINVAL, "ah_init_fields: null context");
     c->cur = 0;
-    cudaError_t e = c->P.fp64 ? ah::launch_init<double>(cur_fields_mut<double>(c), seed, c->P.sigma, c->n, c->st)
-                              : ah::launch_init<float>(cur_fields_mut<float>(c), seed, c->P.sigma, c->n, c->st);
+    const ah_params &P = c->P;
+    cudaError_t e = is_fp64(P) ? ah::launch_init<double>(cur_fields_mut<double>(c), seed, P.sigma, P.nx, P.ny, c->nza, P.nz,
+                                                         c->z_offset, c->st)
+                               : ah::launch_init<float>(cur_fields_mut<float>(c), seed, P.sigma, P.nx, P.ny, c->nza, P.nz,
+                                                        c->z_offset, c->st);
     if (e != cudaSuccess) return cuda_fail(e, "init kernel launch");
     c->launches += 1;
     c->have_fields = true;
@@ -461,6 +522,7 @@ int ah_step(ah_ctx *c, int n, double tau, double dt)
     if (!c) return fail(AH_EINVAL, "ah_step: null context");
     if (n < 0) return fail(AH_EINVAL, "ah_step: n must be >= 0 (got %d)", n);
     if (!c->have_fields) return fail(AH_ESTATE, "ah_step: no fields were set");
+    if (c->slab) return fail(AH_ESTATE, "ah_step: a z-slab context steps with ah_slab_step (ghost planes need an exchange)");
     int rc = check_time(c, tau, dt);
     if (rc != AH_OK) return rc;
     for (int j = 0; j < n; ++j) {
@@ -475,6 +537,7 @@ int ah_step_cooling(ah_ctx *c, int n, double delta, double dt)
     if (!c) return fail(AH_EINVAL, "ah_step_cooling: null context");
     if (n < 0) return fail(AH_EINVAL, "ah_step_cooling: n must be >= 0 (got %d)", n);
     if (!c->have_fields) return fail(AH_ESTATE, "ah_step_cooling: no fields were set");
+    if (c->slab) return fail(AH_ESTATE, "ah_step_cooling: not available on a z-slab context");
     if (!(dt > 0.0) || !std::isfinite(dt) || !(delta > 0.0) || !(delta < 1.0))
         return fail(AH_EINVAL, "ah_step_cooling: need dt > 0 and 0 < delta < 1 (dt=%g, delta=%g)", dt, delta);
     // constant damping = the Hubble term frozen at tau = dt/delta with p = 1, alpha = 2; s = 0 keeps q = 1
@@ -491,6 +554,7 @@ int ah_diagnostics(ah_ctx *c, double tau, double dt, ah_diag *out)
 {
     if (!c || !out) return fail(AH_EINVAL, "ah_diagnostics: null pointer");
     if (!c->have_fields) return fail(AH_ESTATE, "ah_diagnostics: no fields were set");
+    if (c->slab) return fail(AH_ESTATE, "ah_diagnostics: a z-slab context reads out with ah_slab_diag_partial");
     int rc = check_diag_time(c, tau, dt);
     if (rc != AH_OK) return rc;
     rc = ensure_diag_scratch(c, 1);
@@ -499,7 +563,7 @@ int ah_diagnostics(ah_ctx *c, double tau, double dt, ah_diag *out)
     if (rc != AH_OK) return rc;
     AH_CUDA(cudaMemcpyAsync(c->h_results, c->d_results, sizeof(ah::DiagPartial), cudaMemcpyDeviceToHost, c->st));
     AH_CUDA(cudaStreamSynchronize(c->st));
-    finish_diag(c, c->h_results[0], tau, out);
+    finish_diag(c->P, c->h_results[0], tau, out);
     return AH_OK;
 }
 
@@ -509,6 +573,7 @@ int ah_step_diag(ah_ctx *c, int n, double tau, double dt, int every, ah_diag *ou
     *n_written = 0;
     if (n < 0 || every < 1) return fail(AH_EINVAL, "ah_step_diag: need n >= 0 and every >= 1");
     if (!c->have_fields) return fail(AH_ESTATE, "ah_step_diag: no fields were set");
+    if (c->slab) return fail(AH_ESTATE, "ah_step_diag: a z-slab context steps with ah_slab_step");
     int rc = check_time(c, tau, dt);
     for (int j = 0; j < n && rc == AH_OK; j += every) rc = check_diag_time(c, tau + (double)j * dt, dt);
     if (rc != AH_OK) return rc;
@@ -520,7 +585,7 @@ int ah_step_diag(ah_ctx *c, int n, double tau, double dt, int every, ah_diag *ou
     for (int j = 0; j < n; ++j) {
         const double tj = tau + (double)j * dt;
         const bool diag = (j % every == 0);
-        const bool fused = diag && !c->P.fp64 && c->kernel == AH_KERNEL_TILED;
+        const bool fused = diag && c->P.fp64 == AH_PRECISION_FP32 && c->kernel == AH_KERNEL_TILED;
         if (diag && !fused) {   // site / fp64 kernels: read-outs by the standalone kernel, then the step
             rc = enqueue_diag(c, tj, dt, r, nullptr, nullptr);
             if (rc != AH_OK) return rc;
@@ -533,7 +598,7 @@ int ah_step_diag(ah_ctx *c, int n, double tau, double dt, int every, ah_diag *ou
         AH_CUDA(cudaMemcpyAsync(c->h_results, c->d_results, sizeof(ah::DiagPartial) * (size_t)r,
                                 cudaMemcpyDeviceToHost, c->st));
     AH_CUDA(cudaStreamSynchronize(c->st));
-    for (int i = 0; i < r; ++i) finish_diag(c, c->h_results[i], tau + (double)(i * every) * dt, out + i);
+    for (int i = 0; i < r; ++i) finish_diag(c->P, c->h_results[i], tau + (double)(i * every) * dt, out + i);
     *n_written = r;
     return AH_OK;
 }
@@ -547,16 +612,18 @@ int ah_winding_field(ah_ctx *c, int8_t *host_w3, uint8_t *host_near3)
     int8_t *d_w = nullptr;
     uint8_t *d_near = nullptr;
     AH_CUDA(cudaMalloc(&d_w, 3 * c->n));
-    if (host_near3) {
-        cudaError_t e = cudaMalloc(&d_near, 3 * c->n);
-        if (e != cudaSuccess) {
-            cudaFree(d_w);
-            return cuda_fail(e, "cudaMalloc near flags");
-        }
+    cudaError_t e = cudaMemsetAsync(d_w, 0, 3 * c->n, c->st);   // ghost planes of a slab stay 0
+    if (e == cudaSuccess && host_near3) {
+        e = cudaMalloc(&d_near, 3 * c->n);
+        if (e == cudaSuccess) e = cudaMemsetAsync(d_near, 0, 3 * c->n, c->st);
+    }
+    if (e != cudaSuccess) {
+        cudaFree(d_w);
+        if (d_near) cudaFree(d_near);
+        return cuda_fail(e, "winding field scratch");
     }
     // winding does not depend on tau or on the couplings
     rc = enqueue_diag(c, 1.0, 1.0, 0, d_w, d_near, /*winding_only=*/true);
-    cudaError_t e = cudaSuccess;
     if (rc == AH_OK) e = cudaMemcpyAsync(host_w3, d_w, 3 * c->n, cudaMemcpyDeviceToHost, c->st);
     if (rc == AH_OK && e == cudaSuccess && host_near3)
         e = cudaMemcpyAsync(host_near3, d_near, 3 * c->n, cudaMemcpyDeviceToHost, c->st);
@@ -568,6 +635,118 @@ int ah_winding_field(ah_ctx *c, int8_t *host_w3, uint8_t *host_near3)
     if (e2 != cudaSuccess) return cuda_fail(e2, "cudaStreamSynchronize");
     return AH_OK;
 }
+
+// ------------------------------------------------------------------------------------------------ z slabs
+
+int ah_slab_step(ah_ctx *c, double tau, double dt, int want_diag, void *comm_stream)
+{
+    if (!c) return fail(AH_EINVAL, "ah_slab_step: null context");
+    if (!c->slab) return fail(AH_ESTATE, "ah_slab_step: not a z-slab context");
+    if (!c->have_fields) return fail(AH_ESTATE, "ah_slab_step: no fields were set");
+    int rc = want_diag ? check_diag_time(c, tau, dt) : check_time(c, tau, dt);
+    if (rc != AH_OK) return rc;
+    int *flag = c->d_overflow + c->step_parity, *next_flag = c->d_overflow + (1 - c->step_parity);
+    const ah::ZRange own = c->zr;
+    const bool tiled = c->P.fp64 == AH_PRECISION_FP32 && c->kernel == AH_KERNEL_TILED;
+    cudaError_t e = cudaSuccess;
+    if (want_diag) {
+        rc = ensure_diag_scratch(c, 1);
+        if (rc != AH_OK) return rc;
+        if (!tiled) {
+            rc = enqueue_diag(c, tau, dt, 0, nullptr, nullptr);
+            if (rc != AH_OK) return rc;
+        }
+    }
+    if (want_diag && tiled) {
+        // fused read-outs: one launch over all own planes (no boundary / interior split on diagnostic steps)
+        e = enqueue_step(c, c->P, tau, dt, own, 0, flag, next_flag);
+        if (e == cudaSuccess) e = cudaEventRecord(c->ev_boundary, c->st);
+    } else if (own.hi - own.lo <= 2) {
+        e = enqueue_step(c, c->P, tau, dt, own, -1, flag, next_flag);
+        if (e == cudaSuccess) e = cudaEventRecord(c->ev_boundary, c->st);
+    } else {
+        // the paper's order: the planes the neighbours need first, then their exchange can run
+        // while the interior is updated
+        e = enqueue_step(c, c->P, tau, dt, ah::ZRange{own.lo, own.lo + 1}, -1, flag, next_flag);
+        if (e == cudaSuccess) e = enqueue_step(c, c->P, tau, dt, ah::ZRange{own.hi - 1, own.hi}, -1, flag, next_flag);
+        if (e == cudaSuccess) e = cudaEventRecord(c->ev_boundary, c->st);
+        if (e == cudaSuccess) e = enqueue_step(c, c->P, tau, dt, ah::ZRange{own.lo + 1, own.hi - 1}, -1, flag, next_flag);
+    }
+    if (e == cudaSuccess && comm_stream != (void *)c->st)
+        e = cudaStreamWaitEvent((cudaStream_t)comm_stream, c->ev_boundary, 0);
+    if (e != cudaSuccess) {
+        cudaMemsetAsync(c->d_overflow, 0, 2 * sizeof(int), c->st);
+        return cuda_fail(e, "slab step launch");
+    }
+    c->step_parity = 1 - c->step_parity;
+    c->cur = 1 - c->cur;
+    return AH_OK;
+}
+
+int ah_slab_halo_ptrs(ah_ctx *c, void *send_lo[AH_NHALO], void *send_hi[AH_NHALO], void *recv_lo[AH_NHALO],
+                      void *recv_hi[AH_NHALO], size_t *plane_bytes)
+{
+    if (!c || !send_lo || !send_hi || !recv_lo || !recv_hi || !plane_bytes)
+        return fail(AH_EINVAL, "ah_slab_halo_ptrs: null pointer");
+    if (!c->slab) return fail(AH_ESTATE, "ah_slab_halo_ptrs: not a z-slab context");
+    const size_t pb = (size_t)c->P.nx * c->P.ny * c->elem;
+    for (int a = 0; a < AH_NHALO; ++a) {
+        char *base = (char *)c->bufs[c->cur * AH_NFIELDS + HALO_FIELDS[a]];
+        recv_lo[a] = base;                                   // ghost plane below the own planes
+        send_lo[a] = base + pb;                              // first own plane  -> the lower neighbour's recv_hi
+        send_hi[a] = base + pb * (size_t)(c->nza - 2);       // last own plane   -> the upper neighbour's recv_lo
+        recv_hi[a] = base + pb * (size_t)(c->nza - 1);       // ghost plane above
+    }
+    *plane_bytes = pb;
+    return AH_OK;
+}
+
+int ah_slab_exchange_done(ah_ctx *c, void *comm_stream)
+{
+    if (!c) return fail(AH_EINVAL, "ah_slab_exchange_done: null context");
+    if (!c->slab) return fail(AH_ESTATE, "ah_slab_exchange_done: not a z-slab context");
+    if (comm_stream == (void *)c->st) return AH_OK;
+    AH_CUDA(cudaEventRecord(c->ev_exchange, (cudaStream_t)comm_stream));
+    AH_CUDA(cudaStreamWaitEvent(c->st, c->ev_exchange, 0));
+    return AH_OK;
+}
+
+int ah_slab_diagnostics(ah_ctx *c, double tau, double dt)
+{
+    if (!c) return fail(AH_EINVAL, "ah_slab_diagnostics: null context");
+    if (!c->slab) return fail(AH_ESTATE, "ah_slab_diagnostics: not a z-slab context");
+    if (!c->have_fields) return fail(AH_ESTATE, "ah_slab_diagnostics: no fields were set");
+    int rc = check_diag_time(c, tau, dt);
+    if (rc != AH_OK) return rc;
+    rc = ensure_diag_scratch(c, 1);
+    if (rc != AH_OK) return rc;
+    return enqueue_diag(c, tau, dt, 0, nullptr, nullptr);
+}
+
+int ah_slab_diag_partial(ah_ctx *c, int64_t counts[AH_NDIAG_INT], double sums[AH_NDIAG_FLT])
+{
+    if (!c || !counts || !sums) return fail(AH_EINVAL, "ah_slab_diag_partial: null pointer");
+    if (!c->slab) return fail(AH_ESTATE, "ah_slab_diag_partial: not a z-slab context");
+    if (!c->d_results) return fail(AH_ESTATE, "ah_slab_diag_partial: no read-out was requested");
+    AH_CUDA(cudaMemcpyAsync(c->h_results, c->d_results, sizeof(ah::DiagPartial), cudaMemcpyDeviceToHost, c->st));
+    AH_CUDA(cudaStreamSynchronize(c->st));
+    for (int a = 0; a < AH_NDIAG_INT; ++a) counts[a] = c->h_results[0].i[a];
+    for (int a = 0; a < AH_NDIAG_FLT; ++a) sums[a] = c->h_results[0].f[a];
+    return AH_OK;
+}
+
+int ah_diag_finish(const ah_params *global_params, const int64_t counts[AH_NDIAG_INT], const double sums[AH_NDIAG_FLT],
+                   double tau, ah_diag *out)
+{
+    if (!global_params || !counts || !sums || !out) return fail(AH_EINVAL, "ah_diag_finish: null pointer");
+    ah::DiagPartial r;
+    for (int a = 0; a < AH_NDIAG_INT; ++a) r.i[a] = counts[a];
+    for (int a = 0; a < AH_NDIAG_FLT; ++a) r.f[a] = sums[a];
+    finish_diag(*global_params, r, tau, out);
+    return AH_OK;
+}
+
+// ------------------------------------------------------------------------------------------------ test hooks
 
 int ah_test_trig(const float *dev_x, float *dev_sin, float *dev_cos, float *dev_plaq_sin, size_t n,
                  void *cuda_stream)

@@ -50,6 +50,13 @@ struct ConstFields {
 
 enum { PHI_RE = 0, PHI_IM, PI_RE, PI_IM, TH_X, TH_Y, TH_Z, EP_X, EP_Y, EP_Z };
 
+// Planes lo .. hi-1 of the nz allocated ones that a launch updates / reads out.  {0, nz}: the whole periodic lattice.
+// A z slab of a multi-GPU run is allocated with one ghost plane below and above its own
+// planes and uses {1, nz - 1}: the periodic wrap of the plane index is then never taken.
+struct ZRange {
+    int lo, hi;
+};
+
 // Number of partial-sum slots a diagnostics block writes.
 enum {
     DS_NW_XY = 0, DS_NW_XZ, DS_NW_YZ, DS_NEAR, DS_BIG,   // integer counts (stored as double-exact int64)

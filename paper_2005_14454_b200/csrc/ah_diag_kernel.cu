@@ -120,7 +120,7 @@ __device__ __forceinline__ void site_readouts(const ConstFields<float> &in, cons
 // only_if != nullptr: the launch is a conditional re-evaluation (ah_api.cu): nothing happens unless *only_if != 0
 template <typename real>
 __global__ void __launch_bounds__(DBX * DBY)
-diag_kernel(ConstFields<real> in, DiagCoef k, int nx, int ny, int nz, DiagPartial *partials,
+diag_kernel(ConstFields<real> in, DiagCoef k, int nx, int ny, int nz, int z_lo, int z_hi, DiagPartial *partials,
             int8_t *w3, uint8_t *near3, const int *only_if)
 {
     if (only_if != nullptr && *only_if == 0) return;
@@ -131,9 +131,9 @@ diag_kernel(ConstFields<real> in, DiagCoef k, int nx, int ny, int nz, DiagPartia
     long long cnt[DS_NINT] = {0, 0, 0, 0, 0};
     double acc[DS_NFLT] = {0, 0, 0, 0, 0, 0, 0};
 
-    const int z_end = min(nz, ((int)blockIdx.z + 1) * DBZ);
+    const int z_end = min(z_hi, z_lo + ((int)blockIdx.z + 1) * DBZ);
     const size_t n = (size_t)nx * ny * nz;
-    for (int z = blockIdx.z * DBZ; active && z < z_end; ++z) {
+    for (int z = z_lo + blockIdx.z * DBZ; active && z < z_end; ++z) {
         int wi[3], nearf[3];
         site_readouts(in, k, nx, ny, nz, x, y, z, cnt, acc, wi, nearf);
         const size_t c = (size_t)x + (size_t)nx * ((size_t)y + (size_t)ny * (size_t)z);
@@ -237,31 +237,31 @@ cudaError_t launch_diag_final(const DiagPartial *partials, int n, DiagPartial *r
 }
 
 template <typename real>
-cudaError_t launch_diag_partials(const ConstFields<real> &in, const DiagCoef &k, int nx, int ny, int nz,
+cudaError_t launch_diag_partials(const ConstFields<real> &in, const DiagCoef &k, int nx, int ny, int nz, ZRange zr,
                                  DiagPartial *partials, int8_t *w3, uint8_t *near3, const int *only_if,
                                  cudaStream_t st)
 {
     dim3 block(DBX, DBY, 1);
-    dim3 grid((nx + DBX - 1) / DBX, (ny + DBY - 1) / DBY, (nz + DBZ - 1) / DBZ);
-    diag_kernel<real><<<grid, block, 0, st>>>(in, k, nx, ny, nz, partials, w3, near3, only_if);
+    dim3 grid((nx + DBX - 1) / DBX, (ny + DBY - 1) / DBY, (zr.hi - zr.lo + DBZ - 1) / DBZ);
+    diag_kernel<real><<<grid, block, 0, st>>>(in, k, nx, ny, nz, zr.lo, zr.hi, partials, w3, near3, only_if);
     return cudaGetLastError();
 }
 
 template <typename real>
-cudaError_t launch_diag(const ConstFields<real> &in, const DiagCoef &k, int nx, int ny, int nz,
+cudaError_t launch_diag(const ConstFields<real> &in, const DiagCoef &k, int nx, int ny, int nz, ZRange zr,
                         DiagPartial *partials, DiagPartial *result, int8_t *w3, uint8_t *near3,
                         cudaStream_t st)
 {
-    cudaError_t e = launch_diag_partials<real>(in, k, nx, ny, nz, partials, w3, near3, nullptr, st);
+    cudaError_t e = launch_diag_partials<real>(in, k, nx, ny, nz, zr, partials, w3, near3, nullptr, st);
     if (e != cudaSuccess) return e;
-    return launch_diag_final(partials, diag_num_blocks(nx, ny, nz), result, st);
+    return launch_diag_final(partials, diag_num_blocks(nx, ny, zr.hi - zr.lo), result, st);
 }
 
-template cudaError_t launch_diag<float>(const ConstFields<float> &, const DiagCoef &, int, int, int,
+template cudaError_t launch_diag<float>(const ConstFields<float> &, const DiagCoef &, int, int, int, ZRange,
                                         DiagPartial *, DiagPartial *, int8_t *, uint8_t *, cudaStream_t);
-template cudaError_t launch_diag<double>(const ConstFields<double> &, const DiagCoef &, int, int, int,
+template cudaError_t launch_diag<double>(const ConstFields<double> &, const DiagCoef &, int, int, int, ZRange,
                                          DiagPartial *, DiagPartial *, int8_t *, uint8_t *, cudaStream_t);
-template cudaError_t launch_diag_partials<float>(const ConstFields<float> &, const DiagCoef &, int, int, int,
+template cudaError_t launch_diag_partials<float>(const ConstFields<float> &, const DiagCoef &, int, int, int, ZRange,
                                                  DiagPartial *, int8_t *, uint8_t *, const int *, cudaStream_t);
 
 // ------------------------------------------------------------------------- trig test hook

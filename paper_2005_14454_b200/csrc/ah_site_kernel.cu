@@ -9,8 +9,10 @@
 namespace ah {
 
 // Eqs. 7-10 at the single site (x, y, z)
-template <typename real>
-__device__ __forceinline__ void site_update(const ConstFields<real> &in, const Fields<real> &out,
+// S: storage type of the state; real: type of the arithmetic (S = real for the fp32 and fp64 builds; S = float,
+// real = double is the mixed-precision variant: fp32 storage, every operation of the step in fp64)
+template <typename S, typename real>
+__device__ __forceinline__ void site_update(const ConstFields<S> &in, const Fields<S> &out,
                                             const StepCoef<real> &k, int nx, int ny, int nz, int x, int y, int z)
 {
     const int xp = (x + 1 == nx) ? 0 : x + 1, xm = (x == 0) ? nx - 1 : x - 1;
@@ -23,8 +25,12 @@ __device__ __forceinline__ void site_update(const ConstFields<real> &in, const F
     const size_t iyp = at(x, yp, z), iym = at(x, ym, z);
     const size_t izp = at(x, y, zp), izm = at(x, y, zm);
 
-    const real *pr = in.f[PHI_RE], *pi = in.f[PHI_IM];
-    const real *thx = in.f[TH_X], *thy = in.f[TH_Y], *thz = in.f[TH_Z];
+    // reads convert to the arithmetic type
+    struct Rd {
+        const S *p;
+        __device__ __forceinline__ real operator[](size_t i) const { return (real)p[i]; }
+    };
+    const Rd pr{in.f[PHI_RE]}, pi{in.f[PHI_IM]}, thx{in.f[TH_X]}, thy{in.f[TH_Y]}, thz{in.f[TH_Z]};
 
     const real fr = pr[c], fi = pi[c];
     const real tx = thx[c], ty = thy[c], tz = thz[c];
@@ -53,8 +59,8 @@ __device__ __forceinline__ void site_update(const ConstFields<real> &in, const F
 
     // Eq. 7
     const real pot = k.half_lam_q * (fr * fr + fi * fi - k.sig2);
-    const real pr_new = k.c1 * in.f[PI_RE][c] + k.c2 * (lap_r - pot * fr);
-    const real pi_new = k.c1 * in.f[PI_IM][c] + k.c2 * (lap_i - pot * fi);
+    const real pr_new = k.c1 * (real)in.f[PI_RE][c] + k.c2 * (lap_r - pot * fr);
+    const real pi_new = k.c1 * (real)in.f[PI_IM][c] + k.c2 * (lap_i - pot * fi);
 
     // Eqs. 14-15: plaquette angles Phi_ij at x and at the backward neighbours (reading #9)
     auto F = [&](real phi) { return k.compact ? plaq_sin(phi) : phi; };
@@ -87,32 +93,52 @@ __device__ __forceinline__ void site_update(const ConstFields<real> &in, const F
     const real jz = fr * fzi - fi * fzr;
 
     // Eq. 8
-    const real ex_new = k.w1 * in.f[EP_X][c] + k.w2 * (k.two_e2_q * jx - k.idx2 * curl_x);
-    const real ey_new = k.w1 * in.f[EP_Y][c] + k.w2 * (k.two_e2_q * jy - k.idx2 * curl_y);
-    const real ez_new = k.w1 * in.f[EP_Z][c] + k.w2 * (k.two_e2_q * jz - k.idx2 * curl_z);
+    const real ex_new = k.w1 * (real)in.f[EP_X][c] + k.w2 * (k.two_e2_q * jx - k.idx2 * curl_x);
+    const real ey_new = k.w1 * (real)in.f[EP_Y][c] + k.w2 * (k.two_e2_q * jy - k.idx2 * curl_y);
+    const real ez_new = k.w1 * (real)in.f[EP_Z][c] + k.w2 * (k.two_e2_q * jz - k.idx2 * curl_z);
 
-    out.f[PI_RE][c] = pr_new;
-    out.f[PI_IM][c] = pi_new;
-    out.f[EP_X][c] = ex_new;
-    out.f[EP_Y][c] = ey_new;
-    out.f[EP_Z][c] = ez_new;
+    out.f[PI_RE][c] = (S)(pr_new);
+    out.f[PI_IM][c] = (S)(pi_new);
+    out.f[EP_X][c] = (S)(ex_new);
+    out.f[EP_Y][c] = (S)(ey_new);
+    out.f[EP_Z][c] = (S)(ez_new);
     // Eqs. 9-10
-    out.f[PHI_RE][c] = fr + k.dt * pr_new;
-    out.f[PHI_IM][c] = fi + k.dt * pi_new;
-    out.f[TH_X][c] = tx + k.dt * ex_new;
-    out.f[TH_Y][c] = ty + k.dt * ey_new;
-    out.f[TH_Z][c] = tz + k.dt * ez_new;
+    out.f[PHI_RE][c] = (S)(fr + k.dt * pr_new);
+    out.f[PHI_IM][c] = (S)(fi + k.dt * pi_new);
+    out.f[TH_X][c] = (S)(tx + k.dt * ex_new);
+    out.f[TH_Y][c] = (S)(ty + k.dt * ey_new);
+    out.f[TH_Z][c] = (S)(tz + k.dt * ez_new);
 }
 
 template <typename real>
 __global__ void __launch_bounds__(256)
-site_step_kernel(ConstFields<real> in, Fields<real> out, StepCoef<real> k, int nx, int ny, int nz)
+site_step_kernel(ConstFields<real> in, Fields<real> out, StepCoef<real> k, int nx, int ny, int nz, int z_lo)
 {
     const int x = blockIdx.x * blockDim.x + threadIdx.x;
     const int y = blockIdx.y * blockDim.y + threadIdx.y;
-    const int z = blockIdx.z;
+    const int z = z_lo + blockIdx.z;
     if (x >= nx || y >= ny) return;
-    site_update<real>(in, out, k, nx, ny, nz, x, y, z);
+    site_update<real, real>(in, out, k, nx, ny, nz, x, y, z);
+}
+
+// mixed precision: fp32 state, the whole step in fp64; results are rounded once, on the store
+__global__ void __launch_bounds__(256)
+site_step_mixed_kernel(ConstFields<float> in, Fields<float> out, StepCoef<double> k, int nx, int ny, int nz, int z_lo)
+{
+    const int x = blockIdx.x * blockDim.x + threadIdx.x;
+    const int y = blockIdx.y * blockDim.y + threadIdx.y;
+    const int z = z_lo + blockIdx.z;
+    if (x >= nx || y >= ny) return;
+    site_update<float, double>(in, out, k, nx, ny, nz, x, y, z);
+}
+
+cudaError_t launch_site_step_mixed(const ConstFields<float> &in, const Fields<float> &out,
+                                   const StepCoef<double> &k, int nx, int ny, int nz, ZRange zr, cudaStream_t st)
+{
+    dim3 block(nx >= 64 ? 64 : 32, nx >= 64 ? 4 : 8, 1);
+    dim3 grid((nx + block.x - 1) / block.x, (ny + block.y - 1) / block.y, zr.hi - zr.lo);
+    site_step_mixed_kernel<<<grid, block, 0, st>>>(in, out, k, nx, ny, nz, zr.lo);
+    return cudaGetLastError();
 }
 
 // Conditional redo of one step (fixed small grid, grid-stride over sites): does nothing unless the tiled
@@ -120,39 +146,39 @@ site_step_kernel(ConstFields<real> in, Fields<real> out, StepCoef<real> k, int n
 // paths above.  Thread 0 also clears the flag the NEXT step will use.
 __global__ void __launch_bounds__(256)
 site_redo_kernel(const int *flag, int *clear, ConstFields<float> in, Fields<float> out, StepCoef<float> k,
-                 int nx, int ny, int nz)
+                 int nx, int ny, int nz, int z_lo, int z_hi)
 {
     pdl_launch_dependents();
     pdl_wait();   // before the flag is read, and before the early exit (ah_common.cuh)
     if (blockIdx.x == 0 && threadIdx.x == 0) *clear = 0;
     if (*flag == 0) return;
-    const size_t n = (size_t)nx * ny * nz;
+    const size_t n = (size_t)nx * ny * (z_hi - z_lo);
     for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
-        const int x = (int)(i % nx), y = (int)((i / nx) % ny), z = (int)(i / ((size_t)nx * ny));
-        site_update<float>(in, out, k, nx, ny, nz, x, y, z);
+        const int x = (int)(i % nx), y = (int)((i / nx) % ny), z = z_lo + (int)(i / ((size_t)nx * ny));
+        site_update<float, float>(in, out, k, nx, ny, nz, x, y, z);
     }
 }
 
 cudaError_t launch_site_redo(const int *flag, int *clear, const ConstFields<float> &in, const Fields<float> &out,
-                             const StepCoef<float> &k, int nx, int ny, int nz, cudaStream_t st)
+                             const StepCoef<float> &k, int nx, int ny, int nz, ZRange zr, cudaStream_t st)
 {
-    return launch_pdl(site_redo_kernel, dim3(148 * 4), dim3(256), 0, st, flag, clear, in, out, k, nx, ny, nz);
+    return launch_pdl(site_redo_kernel, dim3(148 * 4), dim3(256), 0, st, flag, clear, in, out, k, nx, ny, nz, zr.lo, zr.hi);
 }
 
 template <typename real>
 cudaError_t launch_site_step(const ConstFields<real> &in, const Fields<real> &out,
-                             const StepCoef<real> &k, int nx, int ny, int nz, cudaStream_t st)
+                             const StepCoef<real> &k, int nx, int ny, int nz, ZRange zr, cudaStream_t st)
 {
     dim3 block(nx >= 64 ? 64 : 32, nx >= 64 ? 4 : 8, 1);
-    dim3 grid((nx + block.x - 1) / block.x, (ny + block.y - 1) / block.y, nz);
-    site_step_kernel<real><<<grid, block, 0, st>>>(in, out, k, nx, ny, nz);
+    dim3 grid((nx + block.x - 1) / block.x, (ny + block.y - 1) / block.y, zr.hi - zr.lo);
+    site_step_kernel<real><<<grid, block, 0, st>>>(in, out, k, nx, ny, nz, zr.lo);
     return cudaGetLastError();
 }
 
 template cudaError_t launch_site_step<float>(const ConstFields<float> &, const Fields<float> &,
-                                             const StepCoef<float> &, int, int, int, cudaStream_t);
+                                             const StepCoef<float> &, int, int, int, ZRange, cudaStream_t);
 template cudaError_t launch_site_step<double>(const ConstFields<double> &, const Fields<double> &,
-                                              const StepCoef<double> &, int, int, int, cudaStream_t);
+                                              const StepCoef<double> &, int, int, int, ZRange, cudaStream_t);
 
 // ------------------------------------------------------------------------------------ I0
 
@@ -168,13 +194,18 @@ __device__ __forceinline__ uint32_t u24(uint64_t seed, uint64_t idx)
 
 template <typename real>
 __global__ void __launch_bounds__(256)
-init_kernel(Fields<real> out, uint64_t seed, double sigma, size_t n)
+init_kernel(Fields<real> out, uint64_t seed, double sigma, size_t sxy, size_t n, int nz_global, int z_offset)
 {
     const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
+    // linear index of the site in the GLOBAL lattice (a z slab's ghost planes get their periodic neighbours' values)
+    int zg = (int)(i / sxy) + z_offset;
+    zg %= nz_global;
+    if (zg < 0) zg += nz_global;
+    const uint64_t gi = (uint64_t)zg * sxy + (uint64_t)(i % sxy);
     // vartheta = 2 pi u, u = m / 2^24 exactly; evaluate the phase in fp64 so that fp32 and fp64
     // contexts start from the same point rounded once.
-    const double u = (double)u24(seed, (uint64_t)i) * (1.0 / 16777216.0);
+    const double u = (double)u24(seed, gi) * (1.0 / 16777216.0);
     double s, c;
     sincospi(2.0 * u, &s, &c);
     out.f[PHI_RE][i] = (real)(sigma * c);
@@ -184,14 +215,15 @@ init_kernel(Fields<real> out, uint64_t seed, double sigma, size_t n)
 }
 
 template <typename real>
-cudaError_t launch_init(const Fields<real> &out, uint64_t seed, double sigma, size_t n,
-                        cudaStream_t st)
+cudaError_t launch_init(const Fields<real> &out, uint64_t seed, double sigma, int nx, int ny, int nz_alloc,
+                        int nz_global, int z_offset, cudaStream_t st)
 {
+    const size_t sxy = (size_t)nx * ny, n = sxy * nz_alloc;
     const unsigned blocks = (unsigned)((n + 255) / 256);
-    init_kernel<real><<<blocks, 256, 0, st>>>(out, seed, sigma, n);
+    init_kernel<real><<<blocks, 256, 0, st>>>(out, seed, sigma, sxy, n, nz_global, z_offset);
     return cudaGetLastError();
 }
-template cudaError_t launch_init<float>(const Fields<float> &, uint64_t, double, size_t, cudaStream_t);
-template cudaError_t launch_init<double>(const Fields<double> &, uint64_t, double, size_t, cudaStream_t);
+template cudaError_t launch_init<float>(const Fields<float> &, uint64_t, double, int, int, int, int, int, cudaStream_t);
+template cudaError_t launch_init<double>(const Fields<double> &, uint64_t, double, int, int, int, int, int, cudaStream_t);
 
 }  // namespace ah

@@ -212,8 +212,8 @@ namespace {
 // into partials[linear CTA index]; diag_final_kernel adds them in a fixed order.
 template <int SPT, int TY, bool COMPACT, bool DIAG>
 __global__ void __launch_bounds__((TY + 1) * 32, ((TY + 1) * 32 <= 256) ? 2 : 1)
-tiled_step_kernel(ConstFields<float> in, Fields<float> out, StepCoef<float> k, int nx, int ny, int nz, int zc,
-                  int *overflow, DiagCoef dk, DiagPartial *partials)
+tiled_step_kernel(ConstFields<float> in, Fields<float> out, StepCoef<float> k, int nx, int ny, int nz, int z_lo,
+                  int z_hi, int zc, int *overflow, DiagCoef dk, DiagPartial *partials)
 {
     extern __shared__ __align__(128) unsigned char smem_bytes[];
     Smem<SPT, TY, DIAG> &sm = *reinterpret_cast<Smem<SPT, TY, DIAG> *>(smem_bytes);
@@ -222,8 +222,10 @@ tiled_step_kernel(ConstFields<float> in, Fields<float> out, StepCoef<float> k, i
 
     const int lane = threadIdx.x & 31;
     const int w = __shfl_sync(FULL, (int)(threadIdx.x >> 5), 0);   // warp-uniform by construction
-    const int x0 = blockIdx.x * TX, y0 = blockIdx.y * TY, z0 = blockIdx.z * zc;
-    const int z1 = min(nz, z0 + zc);
+    // planes z_lo .. z_hi - 1 are updated (the whole periodic lattice: 0 .. nz; a z slab with ghost planes: 1 .. nz - 1,
+    // where the wrap of the plane index below never happens)
+    const int x0 = blockIdx.x * TX, y0 = blockIdx.y * TY, z0 = z_lo + blockIdx.z * zc;
+    const int z1 = min(z_hi, z0 + zc);
     const int nplanes = z1 - z0;           // planes this CTA updates; loads n = 0 .. nplanes + 1
     const size_t sxy = (size_t)nx * ny;
     const bool is_main = w < TY;
@@ -358,20 +360,40 @@ tiled_step_kernel(ConstFields<float> in, Fields<float> out, StepCoef<float> k, i
         const VS m_pr = ldsN<SPT>(&sm.raw[0][0][r_own][cofs]), m_pi = ldsN<SPT>(&sm.raw[0][1][r_own][cofs]);
         const VS m_tx = ldsN<SPT>(&sm.raw[0][2][r_own][cofs]), m_ty = ldsN<SPT>(&sm.raw[0][3][r_own][cofs]);
         const VS m_tz = ldsN<SPT>(&sm.raw[0][4][r_own][cofs]);
-        const VS my_tz = ldsN<SPT>(&sm.raw[0][4][r_own + 1][cofs]);
-        const float me_tz = sm.raw[0][4][r_own][cofs + SPT];
+        const VS my_tz = ldsN<SPT>(&sm.raw[0][4][r_own + 1][cofs]), my_tx = ldsN<SPT>(&sm.raw[0][2][r_own + 1][cofs]);
+        float me_tz = __shfl_down_sync(FULL, m_tz.v[0], 1), me_ty = __shfl_down_sync(FULL, m_ty.v[0], 1);
+        if (lane == 31) {
+            me_tz = sm.raw[0][4][r_own][cofs + SPT];
+            me_ty = sm.raw[0][3][r_own][cofs + SPT];
+        }
+        // The hand-down of the plane below is what that plane's own iteration (in the CTA of the chunk below)
+        // computes and carries in registers: the same expressions in the same rounding sequence, including the
+        // warp-wide choice between the two plaquette-sine polynomials, so that a site's result does not depend on
+        // where the z chunks (or the z slabs of a multi-GPU run) are cut.
+        VS a_xz, a_yz;
+        float amax = 0.f;
+#pragma unroll
+        for (int j = 0; j < SPT; ++j) {
+            const int jn = (j < SPT - 1) ? j + 1 : SPT - 1;
+            const float ty_xp = (j < SPT - 1) ? m_ty.v[jn] : me_ty, tz_xp = (j < SPT - 1) ? m_tz.v[jn] : me_tz;
+            const float a_xy = plaq_angle_f32(m_tx.v[j], ty_xp, my_tx.v[j], m_ty.v[j]);
+            a_xz.v[j] = plaq_angle_f32(m_tx.v[j], tz_xp, c_tx.v[j], m_tz.v[j]);
+            a_yz.v[j] = plaq_angle_f32(m_ty.v[j], my_tz.v[j], c_ty.v[j], m_tz.v[j]);
+            amax = fmaxf(amax, fmaxf(fmaxf(fabsf(a_xy), fabsf(a_xz.v[j])), fabsf(a_yz.v[j])));
+        }
+        const bool small = __all_sync(FULL, amax < AH_SMALL_ANGLE);
 #pragma unroll
         for (int j = 0; j < SPT; ++j) {
             float s, c;
             sincos_pi_f32(m_tz.v[j], s, c);
-            const float tz_xp = (j < SPT - 1) ? m_tz.v[j < SPT - 1 ? j + 1 : SPT - 1] : me_tz;
-            const float a_xz = m_tx.v[j] + tz_xp - c_tx.v[j] - m_tz.v[j];
-            const float a_yz = m_ty.v[j] + my_tz.v[j] - c_ty.v[j] - m_tz.v[j];
-            const float sxz = plaq_f<COMPACT>(a_xz), syz = plaq_f<COMPACT>(a_yz);
-            g_bzr.v[j] = c * m_pr.v[j] - s * m_pi.v[j];
-            g_bzi.v[j] = c * m_pi.v[j] + s * m_pr.v[j];
-            g_sxz.v[j] = sxz;
-            g_syz.v[j] = syz;
+            hop_bwd_f32(c, s, m_pr.v[j], m_pi.v[j], g_bzr.v[j], g_bzi.v[j]);
+            if (COMPACT) {
+                g_sxz.v[j] = small ? sin_small_f32(a_xz.v[j]) : sin_poly_f32(a_xz.v[j]);
+                g_syz.v[j] = small ? sin_small_f32(a_yz.v[j]) : sin_poly_f32(a_yz.v[j]);
+            } else {
+                g_sxz.v[j] = a_xz.v[j];
+                g_syz.v[j] = a_yz.v[j];
+            }
         }
     }
     stage_alpha(1);
@@ -410,23 +432,37 @@ tiled_step_kernel(ConstFields<float> in, Fields<float> out, StepCoef<float> k, i
             const VS h_pr = ldsN<SPT>(&sm.raw[so][0][0][cofs]), h_pi = ldsN<SPT>(&sm.raw[so][1][0][cofs]);
             const VS h_tx = ldsN<SPT>(&sm.raw[so][2][0][cofs]), h_ty = ldsN<SPT>(&sm.raw[so][3][0][cofs]);
             const VS h_tz = ldsN<SPT>(&sm.raw[so][4][0][cofs]);
-            const VS hn_ty = ldsN<SPT>(&sm.raw[sf][3][0][cofs]);
+            const VS hn_ty = ldsN<SPT>(&sm.raw[sf][3][0][cofs]), hn_tx = ldsN<SPT>(&sm.raw[sf][2][0][cofs]);
             const VS hy_tx = ldsN<SPT>(&sm.raw[so][2][1][cofs]), hy_tz = ldsN<SPT>(&sm.raw[so][4][1][cofs]);
-            float hr_ty = __shfl_down_sync(FULL, h_ty.v[0], 1);
-            if (lane == 31) hr_ty = sm.raw[so][3][0][cofs + SPT];
+            float hr_ty = __shfl_down_sync(FULL, h_ty.v[0], 1), hr_tz = __shfl_down_sync(FULL, h_tz.v[0], 1);
+            if (lane == 31) {
+                hr_ty = sm.raw[so][3][0][cofs + SPT];
+                hr_tz = sm.raw[so][4][0][cofs + SPT];
+            }
+            // the same expressions, rounding sequence and warp-wide choice of the sine polynomial as the main warp
+            // that owns this row in the tile below: a site's result must not depend on where the y tiles are cut
+            // (the plain and the DIAG instantiation cut them differently)
             VS o_byr, o_byi, o_sxy, o_syz;
+            float amax = 0.f;
+#pragma unroll
+            for (int j = 0; j < SPT; ++j) {
+                const int jn = (j < SPT - 1) ? j + 1 : SPT - 1;
+                const float ty_xp = (j < SPT - 1) ? h_ty.v[jn] : hr_ty, tz_xp = (j < SPT - 1) ? h_tz.v[jn] : hr_tz;
+                o_sxy.v[j] = plaq_angle_f32(h_tx.v[j], ty_xp, hy_tx.v[j], h_ty.v[j]);
+                const float a_xz = plaq_angle_f32(h_tx.v[j], tz_xp, hn_tx.v[j], h_tz.v[j]);
+                o_syz.v[j] = plaq_angle_f32(h_ty.v[j], hy_tz.v[j], hn_ty.v[j], h_tz.v[j]);
+                amax = fmaxf(amax, fmaxf(fmaxf(fabsf(o_sxy.v[j]), fabsf(a_xz)), fabsf(o_syz.v[j])));
+            }
+            const bool small = __all_sync(FULL, amax < AH_SMALL_ANGLE);
 #pragma unroll
             for (int j = 0; j < SPT; ++j) {
                 float s, c;
                 sincos_pi_f32(h_ty.v[j], s, c);
-                const float ty_xp = (j < SPT - 1) ? h_ty.v[j < SPT - 1 ? j + 1 : SPT - 1] : hr_ty;
-                const float a_xy = h_tx.v[j] + ty_xp - hy_tx.v[j] - h_ty.v[j];
-                const float a_yz = h_ty.v[j] + hy_tz.v[j] - hn_ty.v[j] - h_tz.v[j];
-                const float sxy_ = plaq_f<COMPACT>(a_xy), syz_ = plaq_f<COMPACT>(a_yz);
-                o_byr.v[j] = c * h_pr.v[j] - s * h_pi.v[j];
-                o_byi.v[j] = c * h_pi.v[j] + s * h_pr.v[j];
-                o_sxy.v[j] = sxy_;
-                o_syz.v[j] = syz_;
+                hop_bwd_f32(c, s, h_pr.v[j], h_pi.v[j], o_byr.v[j], o_byi.v[j]);
+                if (COMPACT) {
+                    o_sxy.v[j] = small ? sin_small_f32(o_sxy.v[j]) : sin_poly_f32(o_sxy.v[j]);
+                    o_syz.v[j] = small ? sin_small_f32(o_syz.v[j]) : sin_poly_f32(o_syz.v[j]);
+                }
             }
             stN<SPT>(&sm.row[buf][0][0][SPT * lane], o_byr);
             stN<SPT>(&sm.row[buf][0][1][SPT * lane], o_byi);
@@ -836,6 +872,7 @@ static int chunk_for(int nx, int ny, int nz, int ty)
 
 int tiled_chunk(int nx, int ny, int nz, bool diag) { return chunk_for(nx, ny, nz, diag ? TILE_Y_DIAG : TILE_Y); }
 
+// nz: number of planes the launch updates
 int tiled_num_blocks(int nx, int ny, int nz, bool diag)
 {
     if (!tiled_supported(nx, ny, nz)) return 0;
@@ -846,39 +883,41 @@ int tiled_num_blocks(int nx, int ny, int nz, bool diag)
 
 template <int SPT, int TY, bool COMPACT, bool DIAG>
 static cudaError_t launch_one(const ConstFields<float> &in, const Fields<float> &out, const StepCoef<float> &k, int nx,
-                              int ny, int nz, int *overflow, cudaStream_t st, const DiagCoef &d, DiagPartial *partials)
+                              int ny, int nz, ZRange zr, int *overflow, cudaStream_t st, const DiagCoef &d,
+                              DiagPartial *partials)
 {
-    const int zc = chunk_for(nx, ny, nz, TY);
-    dim3 grid(nx / (32 * SPT), (ny + TY - 1) / TY, (nz + zc - 1) / zc);
+    const int zc = chunk_for(nx, ny, zr.hi - zr.lo, TY);
+    dim3 grid(nx / (32 * SPT), (ny + TY - 1) / TY, (zr.hi - zr.lo + zc - 1) / zc);
     dim3 block((TY + 1) * 32);
     if (grid.y > 65535u || grid.z > 65535u) return cudaErrorInvalidConfiguration;
     return launch_pdl(tiled_step_kernel<SPT, TY, COMPACT, DIAG>, grid, block, sizeof(Smem<SPT, TY, DIAG>), st, in, out, k, nx,
-                      ny, nz, zc, overflow, d, partials);
+                      ny, nz, zr.lo, zr.hi, zc, overflow, d, partials);
 }
 
 template <int SPT>
 static cudaError_t launch_spt(const ConstFields<float> &in, const Fields<float> &out, const StepCoef<float> &k, int nx,
-                              int ny, int nz, int *overflow, cudaStream_t st, bool diag, const DiagCoef &d,
+                              int ny, int nz, ZRange zr, int *overflow, cudaStream_t st, bool diag, const DiagCoef &d,
                               DiagPartial *partials)
 {
     if (k.compact)
-        return diag ? launch_one<SPT, TILE_Y_DIAG, true, true>(in, out, k, nx, ny, nz, overflow, st, d, partials)
-                    : launch_one<SPT, TILE_Y, true, false>(in, out, k, nx, ny, nz, overflow, st, d, nullptr);
-    return diag ? launch_one<SPT, TILE_Y_DIAG, false, true>(in, out, k, nx, ny, nz, overflow, st, d, partials)
-                : launch_one<SPT, TILE_Y, false, false>(in, out, k, nx, ny, nz, overflow, st, d, nullptr);
+        return diag ? launch_one<SPT, TILE_Y_DIAG, true, true>(in, out, k, nx, ny, nz, zr, overflow, st, d, partials)
+                    : launch_one<SPT, TILE_Y, true, false>(in, out, k, nx, ny, nz, zr, overflow, st, d, nullptr);
+    return diag ? launch_one<SPT, TILE_Y_DIAG, false, true>(in, out, k, nx, ny, nz, zr, overflow, st, d, partials)
+                : launch_one<SPT, TILE_Y, false, false>(in, out, k, nx, ny, nz, zr, overflow, st, d, nullptr);
 }
 
 // partials == nullptr: plain step.  Otherwise the DIAG instantiation, which also writes one DiagPartial per
-// CTA (tiled_num_blocks(.., true) of them) holding the read-outs of the entry snapshot.
+// CTA (tiled_num_blocks(.., planes updated, true) of them) holding the read-outs of the entry snapshot.
+// zr: the planes to update; {0, nz} is the whole periodic lattice.
 cudaError_t launch_tiled_step(const ConstFields<float> &in, const Fields<float> &out,
-                              const StepCoef<float> &k, int nx, int ny, int nz, int *overflow, cudaStream_t st,
+                              const StepCoef<float> &k, int nx, int ny, int nz, ZRange zr, int *overflow, cudaStream_t st,
                               const DiagCoef *dk, DiagPartial *partials)
 {
-    if (!tiled_supported(nx, ny, nz)) return cudaErrorInvalidValue;
+    if (!tiled_supported(nx, ny, nz) || zr.lo < 0 || zr.hi > nz || zr.lo >= zr.hi) return cudaErrorInvalidValue;
     const bool diag = partials != nullptr && dk != nullptr;
     const DiagCoef d = diag ? *dk : DiagCoef{};
-    return spt_for(nx) == 4 ? launch_spt<4>(in, out, k, nx, ny, nz, overflow, st, diag, d, partials)
-                            : launch_spt<2>(in, out, k, nx, ny, nz, overflow, st, diag, d, partials);
+    return spt_for(nx) == 4 ? launch_spt<4>(in, out, k, nx, ny, nz, zr, overflow, st, diag, d, partials)
+                            : launch_spt<2>(in, out, k, nx, ny, nz, zr, overflow, st, diag, d, partials);
 }
 
 }  // namespace ah

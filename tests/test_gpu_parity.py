@@ -593,6 +593,47 @@ def test_fused_step_diag_tiled_kernel(ah, oracle, shape, model):
     b.close()
 
 
+def test_fused_and_plain_steps_agree_bitwise_in_the_physical_regime(ah):
+    """The DIAG instantiation cuts the lattice into tiles of 5 rows, the plain one into tiles of 6: the fields a
+    diagnostic step leaves must still be those of a plain step bit for bit, also where plaquette angles are small and
+    the warp-wide choice of the sine polynomial comes into play (random-phase IC, th = 0 at the start)."""
+    a = ah.Simulation(nx=128, ny=31, nz=24, p=1.0, s=1.0, tau_ref=4.0)
+    b = ah.Simulation(nx=128, ny=31, nz=24, p=1.0, s=1.0, tau_ref=4.0)
+    a.init_fields(3)
+    b.init_fields(3)
+    a.step_diag(12, 1.0, 0.1, 1)
+    b.step(12, 1.0, 0.1)
+    assert np.array_equal(a.get_fields(), b.get_fields())
+    a.close()
+    b.close()
+
+
+@pytest.mark.parametrize("case", [dict(p=1.0, s=1.0, tau_ref=3.0), dict(p=0.0, s=0.0, compact=0)])
+@pytest.mark.parametrize("shape", [(20, 12, 7), (128, 9, 6)])
+def test_one_step_mixed_precision(ah, oracle, case, shape):
+    """SURVEY 8(f)4, mixed precision: fp32 storage, every operation of the step in fp64.  One step from
+    fp32-representable inputs is the oracle's result rounded once to fp32: half an ulp of each value, i.e. 6e-8 of
+    the field's scale (the fp32 build needs 2e-6)."""
+    f0 = inputs.random_state(*shape, seed=7)
+    sim, Po = both(ah, oracle, shape, fp64=ah.PRECISION_MIXED, **case)
+    assert sim.get_kernel() == ah.KERNEL_SITE and sim.np_dtype == np.float32
+    sim.set_fields(f0)
+    sim.step(1, 1.7, 0.1)
+    g = sim.get_fields()
+    o = oracle.step(Po, f0.copy(), 1, 1.7, 0.1)
+    assert np.array_equal(g, o.astype(np.float32)) or max(rel_max(g, o).values()) <= 6.1e-8, rel_max(g, o)
+    # over 40 steps the only rounding is the one store per value and step
+    sim.set_fields(f0)
+    sim.step(40, 1.7, 0.1)
+    ref = oracle.step(Po, f0.copy(), 40, 1.7, 0.1)
+    r = rel_max(sim.get_fields(), ref)
+    print("mixed precision, 40 steps:", r)
+    assert max(r.values()) <= 1e-5, r
+    d = sim.diagnostics(1.7 + 4.0, 0.1)                     # read-outs run on the fp32 snapshot
+    assert d["n_wind"] >= 0
+    sim.close()
+
+
 def test_diagnostics_deterministic(ah):
     sim = ah.Simulation(nx=48, p=1.0, s=0.0)
     sim.init_fields(8)

@@ -1,0 +1,124 @@
+"""z slabs (-m gpu): SURVEY 8(f)2, the paper's domain decomposition in its single-node form.
+
+Only one GPU is available to the tests, so the multi-GPU path is exercised the way DESIGN.md says: ONE lattice is cut
+into several slab contexts on the same GPU, their kernels are launched one after the other (no kernel waits on
+another), and the boundary planes travel by device-to-device copies on the slabs' communication streams, overlapped
+with the update of the interior exactly as NCCL send/recv would be.  Requirement: the slabs reproduce the single-
+lattice run BIT FOR BIT (a site's arithmetic does not depend on where z is cut), and their combined read-outs equal
+the single-lattice read-outs (integers exactly, fp64 sums to the order of summation).
+"""
+import numpy as np
+import pytest
+
+from paper_2005_14454_b200 import inputs
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def ah():
+    import torch
+    assert torch.cuda.is_available(), "these tests need a CUDA device"
+    from paper_2005_14454_b200 import build
+    build.build()
+    from paper_2005_14454_b200 import binding
+    return binding
+
+
+MODEL = dict(p=1.0, s=1.0, tau_ref=3.0)
+
+
+@pytest.mark.parametrize("shape,nslabs,overlap", [((128, 12, 25), 2, True), ((128, 12, 25), 3, True),
+                                                  ((128, 12, 25), 3, False), ((64, 7, 9), 4, True),
+                                                  ((256, 13, 130), 2, True),      # full 64-plane chunks inside a slab
+                                                  ((20, 12, 9), 3, True),         # site kernel (nx % 64 != 0)
+                                                  ((128, 6, 4), 4, True)])        # one own plane per slab
+def test_slabs_reproduce_the_single_lattice_bit_for_bit(ah, shape, nslabs, overlap):
+    nx, ny, nz = shape
+    P = ah.make_params(nx, ny, nz, **MODEL)
+    f0 = inputs.random_state(nx, ny, nz, seed=5, th_amp=0.05, ep_amp=0.05)    # small plaquette angles: both sine paths occur
+    f0[4:7, nz // 2] *= 12.0                                                   # ... and one plane with large ones
+    one = ah.Simulation(params=P)
+    grp = ah.SlabGroup(P, nslabs, overlap=overlap)
+    one.set_fields(f0)
+    grp.set_fields(f0)
+    nsteps, tau0, dt = 7, 1.3, 0.1
+    one.step(nsteps, tau0, dt)
+    grp.step(nsteps, tau0, dt)
+    a, b = one.get_fields(), grp.get_fields()
+    assert np.array_equal(a, b), float(np.abs(a - b).max())
+    # read-outs of the final snapshot: standalone kernels on both sides
+    d1, d2 = one.diagnostics(tau0 + nsteps * dt, dt), grp.diagnostics(tau0 + nsteps * dt, dt)
+    for key in ("n_wind", "n_wind_xy", "n_wind_xz", "n_wind_yz", "n_near_branch", "n_big_plaq"):
+        assert d1[key] == d2[key], key
+    assert d1["gauss_max"] == d2["gauss_max"]
+    for key in ("sum_pi2_L", "sum_grad2_L", "sum_L", "gauss_l2", "gauss_div_l2", "gauss_charge_l2", "v2_phi", "xi_l", "xi_w"):
+        assert d2[key] == pytest.approx(d1[key], rel=1e-11), key
+    one.close()
+    grp.close()
+
+
+def test_slab_fused_records_equal_single_lattice_records(ah):
+    """Fused read-outs on slabs: the records of the entry snapshots equal those of ah_step_diag on the whole lattice."""
+    nx, ny, nz = 128, 11, 20
+    P = ah.make_params(nx, ny, nz, **MODEL)
+    one = ah.Simulation(params=P)
+    grp = ah.SlabGroup(P, 3)
+    one.init_fields(4)
+    grp.init_fields(4)
+    assert np.array_equal(one.get_fields(), grp.get_fields())       # I0 through the global site index, ghosts included
+    r1 = one.step_diag(9, 1.0, 0.1, 4)
+    r2 = grp.step(9, 1.0, 0.1, diag_every=4)
+    assert len(r1) == len(r2) == 3
+    for a, b in zip(r1, r2):
+        assert a["tau"] == b["tau"]
+        for key in ("n_wind", "n_wind_xy", "n_wind_xz", "n_wind_yz", "n_near_branch", "n_big_plaq"):
+            assert a[key] == b[key], key
+        assert a["gauss_max"] == b["gauss_max"]
+        for key in ("sum_pi2_L", "sum_grad2_L", "sum_L", "gauss_l2", "gauss_div_l2", "gauss_charge_l2"):
+            assert b[key] == pytest.approx(a[key], rel=1e-11, abs=1e-300), key
+    assert r1[0]["n_wind"] > 0
+    assert np.array_equal(one.get_fields(), grp.get_fields())
+    one.close()
+    grp.close()
+
+
+def test_slab_against_the_oracle(ah, oracle):
+    """... and against the oracle itself: 3 slabs, 12 steps, the north_star bound on the fields."""
+    nx, ny, nz = 128, 10, 18
+    model = dict(p=2.0, s=1.0, tau_ref=4.0)
+    P = ah.make_params(nx, ny, nz, **model)
+    Po = oracle.make_params(nx, ny, nz, **model)
+    f0 = inputs.random_state(nx, ny, nz, seed=9, th_amp=0.3)
+    grp = ah.SlabGroup(P, 3)
+    grp.set_fields(f0)
+    grp.step(12, 1.5, 0.1)
+    ref = oracle.step(Po, f0.copy(), 12, 1.5, 0.1)
+    got = grp.get_fields().astype(np.float64)
+    for lo, hi in ((0, 2), (2, 4), (4, 7), (7, 10)):
+        err = np.abs(got[lo:hi] - ref[lo:hi]).max() / np.abs(ref[lo:hi]).max()
+        assert err <= 2e-5, (lo, err)
+    d = grp.diagnostics(2.7, 0.1)
+    od = oracle.diagnostics(Po, got, 2.7, 0.1)
+    assert abs(d["n_wind"] - od["n_wind"]) <= d["n_near_branch"] + od["n_near_branch"]
+    assert d["sum_L"] == pytest.approx(od["sum_L"], rel=1e-5)
+    assert d["gauss_l2"] == pytest.approx(od["gauss_l2"], rel=1e-9)
+    grp.close()
+
+
+def test_slab_api_errors(ah):
+    import ctypes as C
+    P = ah.make_params(64, 8, 12)
+    s = ah.SlabSimulation(P, 4, 4)
+    L = ah.lib()
+    assert L.ah_step(s._ctx, 1, 1.0, 0.1) == ah.AH_ESTATE
+    d = ah.Diag()
+    assert L.ah_diagnostics(s._ctx, 1.0, 0.1, C.byref(d)) == ah.AH_ESTATE
+    with pytest.raises(ah.AhError):
+        s.step(1.0, 0.1)                                   # no fields yet
+    s.close()
+    with pytest.raises(ah.AhError):
+        ah.SlabSimulation(P, 5, 8)                         # planes 8 .. 12 do not fit in nz = 12
+    whole = ah.Simulation(params=P)
+    assert L.ah_slab_step(whole._ctx, 1.0, 0.1, 0, None) == ah.AH_ESTATE
+    whole.close()

@@ -91,3 +91,70 @@ def test_bench_gpus_n_starts_n_ranks():
     bad = subprocess.run([sys.executable, str(root / "bench.py"), "--gpus", "2", "--selftest-launcher"],
                          capture_output=True, text=True, timeout=120, env=env2, cwd=str(root))
     assert bad.returncode != 0 and "WORLD_SIZE" in (bad.stderr + bad.stdout)
+
+
+def _slab_worker(rank, world, port, q):
+    import os
+    import torch
+    import torch.distributed as dist
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        from paper_2005_14454_b200 import binding as ah
+        nfield, plane = ah.AH_NHALO, 5
+        # plane lists as SlabSimulation.halo_planes() returns them: send_lo, send_hi, recv_lo, recv_hi; the value of
+        # an element names (rank, which boundary, field)
+        planes = [[torch.full((plane,), 1000.0 * rank + 100.0 * side + a) for a in range(nfield)] for side in (1, 2)]
+        planes += [[torch.full((plane,), -1.0) for _ in range(nfield)] for _ in range(2)]
+        ops = []
+        for a in range(nfield):
+            for kind, which, peer in ah.halo_schedule(rank, world):
+                ops.append(dist.P2POp(dist.isend if kind == "send" else dist.irecv, planes[which][a], peer))
+        for r in dist.batch_isend_irecv(ops):
+            r.wait()
+        lo, hi = (rank - 1) % world, (rank + 1) % world
+        ok = all(float(planes[2][a][0]) == 1000.0 * lo + 200.0 + a and      # ghost below = lower neighbour's LAST own plane
+                 float(planes[3][a][0]) == 1000.0 * hi + 100.0 + a          # ghost above = upper neighbour's FIRST own plane
+                 for a in range(nfield))
+        # read-outs: counts and sums add, the last sum is a maximum
+        counts, sums = [rank + 1] * ah.AH_NDIAG_INT, [0.5 * (rank + 1)] * ah.AH_NDIAG_FLT
+        add = torch.tensor([float(c) for c in counts] + sums[:-1], dtype=torch.float64)
+        mx = torch.tensor([sums[-1]], dtype=torch.float64)
+        dist.all_reduce(add, op=dist.ReduceOp.SUM)
+        dist.all_reduce(mx, op=dist.ReduceOp.MAX)
+        tot = world * (world + 1) / 2
+        ok = ok and add[:ah.AH_NDIAG_INT].tolist() == [tot] * ah.AH_NDIAG_INT and float(mx) == 0.5 * world
+        q.put((rank, ok))
+    finally:
+        dist.destroy_process_group()
+
+
+@pytest.mark.parametrize("world", [2, 3])
+def test_slab_exchange_schedule_over_gloo(world):
+    """Host logic of the z-slab exchange (binding.halo_schedule, the schedule DistributedSlab posts over NCCL): run
+    with CPU tensors over gloo, every rank must end up with its neighbours' boundary planes in its ghost planes, for
+    2 ranks (both neighbours are the same peer) and 3."""
+    import torch.multiprocessing as mp
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = _free_port()
+    procs = [ctx.Process(target=_slab_worker, args=(r, world, port, q)) for r in range(world)]
+    for p in procs:
+        p.start()
+    res = sorted(q.get(timeout=120) for _ in range(world))
+    for p in procs:
+        p.join(timeout=60)
+    assert res == [(r, True) for r in range(world)]
+
+
+def test_slab_partition_and_schedule_host_logic():
+    from paper_2005_14454_b200 import binding as ah
+    for nz, n in ((25, 3), (1024, 8), (7, 7), (10, 1)):
+        parts = [ah.slab_planes(nz, n, r) for r in range(n)]
+        assert parts[0][0] == 0 and sum(p[1] for p in parts) == nz
+        assert all(parts[r][0] + parts[r][1] == parts[r + 1][0] for r in range(n - 1))
+        assert max(p[1] for p in parts) - min(p[1] for p in parts) <= 1
+    with pytest.raises(ValueError):
+        ah.slab_planes(4, 5, 0)
+    assert ah.halo_schedule(0, 1) == [("send", 0, 0), ("recv", 3, 0), ("send", 1, 0), ("recv", 2, 0)]
+    assert ah.combine_partials([([1] * 5, [1.0] * 6 + [3.0]), ([2] * 5, [0.5] * 6 + [7.0])]) == ([3] * 5, [1.5] * 6 + [7.0])
