@@ -117,23 +117,30 @@ __device__ __forceinline__ void site_readouts(const ConstFields<float> &in, cons
     readout_accumulate(acc, pi2L, gr2L, L, G, div, charge);
 }
 
+// One partial per VIRTUAL block vb = (bx, by, bz) of 64 x 4 x 8 sites; the launched blocks take virtual blocks
+// blockIdx.x, blockIdx.x + gridDim.x, ... so that the grid can be smaller than the number of virtual blocks.
 // only_if != nullptr: the launch is a conditional re-evaluation (ah_api.cu): nothing happens unless *only_if != 0
+// (launched with a small grid, since it normally exits at once).
 template <typename real>
 __global__ void __launch_bounds__(DBX * DBY)
-diag_kernel(ConstFields<real> in, DiagCoef k, int nx, int ny, int nz, int z_lo, int z_hi, DiagPartial *partials,
-            int8_t *w3, uint8_t *near3, const int *only_if)
+diag_kernel(ConstFields<real> in, DiagCoef k, int nx, int ny, int nz, int z_lo, int z_hi, int nbx, int nby, int nvb,
+            DiagPartial *partials, int8_t *w3, uint8_t *near3, const int *only_if)
 {
     if (only_if != nullptr && *only_if == 0) return;
-    const int x = blockIdx.x * DBX + threadIdx.x;
-    const int y = blockIdx.y * DBY + threadIdx.y;
+    __shared__ long long s_i[DBX * DBY / 32][DS_NINT];
+    __shared__ double s_f[DBX * DBY / 32][DS_NFLT];
+    for (int vb = blockIdx.x; vb < nvb; vb += gridDim.x) {
+    const int vbx = vb % nbx, vby = (vb / nbx) % nby, vbz = vb / (nbx * nby);
+    const int x = vbx * DBX + threadIdx.x;
+    const int y = vby * DBY + threadIdx.y;
     const bool active = (x < nx) && (y < ny);
 
     long long cnt[DS_NINT] = {0, 0, 0, 0, 0};
     double acc[DS_NFLT] = {0, 0, 0, 0, 0, 0, 0};
 
-    const int z_end = min(z_hi, z_lo + ((int)blockIdx.z + 1) * DBZ);
+    const int z_end = min(z_hi, z_lo + (vbz + 1) * DBZ);
     const size_t n = (size_t)nx * ny * nz;
-    for (int z = z_lo + blockIdx.z * DBZ; active && z < z_end; ++z) {
+    for (int z = z_lo + vbz * DBZ; active && z < z_end; ++z) {
         int wi[3], nearf[3];
         site_readouts(in, k, nx, ny, nz, x, y, z, cnt, acc, wi, nearf);
         const size_t c = (size_t)x + (size_t)nx * ((size_t)y + (size_t)ny * (size_t)z);
@@ -145,8 +152,6 @@ diag_kernel(ConstFields<real> in, DiagCoef k, int nx, int ny, int nz, int z_lo, 
     }
 
     // ---- block reduction: warp shuffles, then 8 warps through shared memory
-    __shared__ long long s_i[DBX * DBY / 32][DS_NINT];
-    __shared__ double s_f[DBX * DBY / 32][DS_NFLT];
     const int tid = threadIdx.y * DBX + threadIdx.x;
     const int lane = tid & 31, warp = tid >> 5;
 #pragma unroll
@@ -176,8 +181,9 @@ diag_kernel(ConstFields<real> in, DiagCoef k, int nx, int ny, int nz, int z_lo, 
                 v = (a == DF_GMAX) ? fmax(v, s_f[w][a]) : v + s_f[w][a];
             p.f[a] = v;
         }
-        const size_t b = blockIdx.x + (size_t)gridDim.x * (blockIdx.y + (size_t)gridDim.y * blockIdx.z);
-        partials[b] = p;
+        partials[vb] = p;
+    }
+    __syncthreads();   // s_i, s_f are re-used by the next virtual block
     }
 }
 
@@ -242,8 +248,12 @@ cudaError_t launch_diag_partials(const ConstFields<real> &in, const DiagCoef &k,
                                  cudaStream_t st)
 {
     dim3 block(DBX, DBY, 1);
-    dim3 grid((nx + DBX - 1) / DBX, (ny + DBY - 1) / DBY, (zr.hi - zr.lo + DBZ - 1) / DBZ);
-    diag_kernel<real><<<grid, block, 0, st>>>(in, k, nx, ny, nz, zr.lo, zr.hi, partials, w3, near3, only_if);
+    const int nbx = (nx + DBX - 1) / DBX, nby = (ny + DBY - 1) / DBY, nbz = (zr.hi - zr.lo + DBZ - 1) / DBZ;
+    const long long nvb = (long long)nbx * nby * nbz;
+    if (nvb > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
+    const int grid = (only_if != nullptr && nvb > 148 * 8) ? 148 * 8 : (int)nvb;
+    diag_kernel<real><<<grid, block, 0, st>>>(in, k, nx, ny, nz, zr.lo, zr.hi, nbx, nby, (int)nvb, partials, w3, near3,
+                                             only_if);
     return cudaGetLastError();
 }
 
