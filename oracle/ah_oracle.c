@@ -18,7 +18,10 @@
  * un-wrapped plaquette angle decides the integer), closed forms of L_x and
  * <v^2>_phi on uniform states (kinetic, electric, potential, gradient and
  * magnetic terms each fixed by arithmetic) besides the naive numpy <v^2> sums,
- * splitmix known answers.  Parity-unpinned items (stated in DESIGN.md): the
+ * splitmix known answers; <v^2>_omega (Eq. 17 right; the paper leaves its
+ * weight, rho and p undefined: DESIGN.md reading #17) by the same uniform-state
+ * closed forms, by p = -rho/3 on the relaxed (critical-coupling) string pair,
+ * by p = rho/3 for pure gauge radiation, and softly by Table 1.  Parity-unpinned items (stated in DESIGN.md): the
  * normalisation a(tau_ref) = 1 and the tau grid (the paper fixes neither).
  *
  * Conventions:
@@ -61,6 +64,7 @@ typedef struct {
     double gauss_max, gauss_l2, gauss_rel;
     double gauss_div_l2, gauss_charge_l2;
     double xi_l;
+    double sum_p_L, sum_rho_L, v2_omega; /* Eq. 17 right, reading #17 */
 } ahref_diag;
 
 #define AHREF_PI 3.14159265358979323846264338327950288
@@ -344,9 +348,12 @@ int ahref_winding(const ahref_params *P, const double *f10, int8_t *w3, uint8_t 
 /* Lagrangian density of site x (reading #15):
  *  L = |Pi|^2 - sum_i |U_i phi(x+i) - phi|^2/dx^2 - (lambda0 q/4)(|phi|^2-sigma^2)^2
  *      + (1/(2 e0^2 q)) [ sum_i ep_i^2/dx^2 - sum_{i<j} 2(1-cos Phi_ij)/dx^4 ]
- * also returns |Pi|^2 and the gradient sum. */
+ * also returns |Pi|^2, the gradient sum, and the energy density and isotropic pressure of the same five pieces
+ * (reading #17, for the equation-of-state estimator of Eq. 17 right):
+ *  rho = |Pi|^2 + grad2 + V + (E2 + B2),   p = |Pi|^2 - grad2/3 - V + (E2 + B2)/3,
+ * with E2 = sum_i ep_i^2/(2 e0^2 q dx^2), B2 = sum_{i<j} 2(1-cos Phi_ij)/(2 e0^2 q dx^4), V the potential term. */
 static double lagrangian_at(const ahref_params *P, const double *f10, const int c[3], double q,
-                            double *pi2_out, double *grad2_out)
+                            double *pi2_out, double *grad2_out, double *rho_out, double *p_out)
 {
     const size_t n = (size_t)P->nx * P->ny * P->nz;
     const double *pr = f10, *pim = f10 + n, *pir = f10 + 2 * n, *pii = f10 + 3 * n;
@@ -370,6 +377,11 @@ static double lagrangian_at(const ahref_params *P, const double *f10, const int 
     const double pot = 0.25 * P->lambda0 * q * (mod2 - sig2) * (mod2 - sig2);
     *pi2_out = pi2;
     *grad2_out = grad2;
+    {
+        const double E2 = e2 / (2.0 * P->e0 * P->e0 * q), B2 = b2 / (2.0 * P->e0 * P->e0 * q);
+        *rho_out = pi2 + grad2 + pot + (E2 + B2);
+        *p_out = pi2 - grad2 / 3.0 - pot + (E2 + B2) / 3.0;
+    }
     return pi2 - grad2 - pot + (e2 - b2) / (2.0 * P->e0 * P->e0 * q);
 }
 
@@ -390,7 +402,7 @@ int ahref_diagnostics(const ahref_params *P, const double *f10, double tau, doub
     const double kappa = q * (1.0 - delta) / (1.0 - omega);
 
     int64_t nw[3] = {0, 0, 0}, n_near = 0, n_big = 0;
-    double s_pi = 0.0, s_gr = 0.0, s_L = 0.0;
+    double s_pi = 0.0, s_gr = 0.0, s_L = 0.0, s_pL = 0.0, s_rL = 0.0;
     double g_max = 0.0, g_sq = 0.0, div_sq = 0.0, ch_sq = 0.0;
 
     /* serial accumulation in site order: the definition, nothing else */
@@ -408,11 +420,14 @@ int ahref_diagnostics(const ahref_params *P, const double *f10, double tau, doub
                     n_big += big;
                 }
                 /* D2 Lagrangian-weighted sums (Eqs. 17-18) */
-                double pi2, grad2;
-                const double L = lagrangian_at(P, f10, c, q, &pi2, &grad2);
+                double pi2, grad2, rho, prs;
+                const double L = lagrangian_at(P, f10, c, q, &pi2, &grad2, &rho, &prs);
                 s_pi += pi2 * L;
                 s_gr += grad2 * L;
                 s_L += L;
+                /* Eq. 17 right with the weight W_x = L_x (reading #17) */
+                s_pL += prs * L;
+                s_rL += rho * L;
                 /* D3 Gauss residual (Eq. 5) */
                 double div = 0.0;
                 for (int i = 0; i < 3; ++i)
@@ -449,6 +464,9 @@ int ahref_diagnostics(const ahref_params *P, const double *f10, double tau, doub
         const double R = s_pi / s_gr;
         out->v2_phi = (s_gr != 0.0) ? 2.0 * R / (1.0 + R) : 0.0;
     }
+    out->sum_p_L = s_pL;
+    out->sum_rho_L = s_rL;
+    out->v2_omega = (s_rL != 0.0) ? 0.5 * (1.0 + 3.0 * s_pL / s_rL) : 0.0;
     out->gauss_max = g_max;
     out->gauss_l2 = sqrt(g_sq);
     out->gauss_div_l2 = sqrt(div_sq);

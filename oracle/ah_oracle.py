@@ -45,6 +45,7 @@ class Diag(C.Structure):
         ("gauss_max", C.c_double), ("gauss_l2", C.c_double), ("gauss_rel", C.c_double),
         ("gauss_div_l2", C.c_double), ("gauss_charge_l2", C.c_double),
         ("xi_l", C.c_double),
+        ("sum_p_L", C.c_double), ("sum_rho_L", C.c_double), ("v2_omega", C.c_double),
     ]
 
     def asdict(self):

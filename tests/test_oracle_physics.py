@@ -324,6 +324,14 @@ def test_lagrangian_closed_form_uniform_state(oracle, model):
     R = pi2 / grad2
     assert d["v2_phi"] == pytest.approx(2 * R / (1 + R), rel=1e-12)
     assert d["n_wind"] == 0 and d["n_big_plaq"] == 0
+    # Eq. 17 right with reading #17: rho and p of the same five pieces, weight W = L
+    pot = 0.25 * lam * q * (rho**2 - sig**2) ** 2
+    E2 = sum(ei**2 for ei in e) / (2.0 * e0**2 * q * dx**2)
+    rho_x = pi2 + grad2 + pot + E2
+    p_x = pi2 - grad2 / 3.0 - pot + E2 / 3.0
+    assert d["sum_rho_L"] == pytest.approx(N * rho_x * L, rel=1e-12)
+    assert d["sum_p_L"] == pytest.approx(N * p_x * L, rel=1e-12)
+    assert d["v2_omega"] == pytest.approx(0.5 * (1.0 + 3.0 * p_x / rho_x), rel=1e-12)
     # the electric and kinetic terms enter with a PLUS sign: L grows with |c| and with |e|
     g = f.copy()
     g[2:4] *= 2.0
@@ -358,3 +366,46 @@ def test_lagrangian_closed_form_uniform_magnetic_field(oracle, compact):
     assert d["sum_L"] == pytest.approx(nx * nz * L_rows.sum(), rel=1e-12)
     assert d["sum_grad2_L"] == pytest.approx(nx * nz * (g2_rows * L_rows).sum(), rel=1e-12)
     assert d["sum_pi2_L"] == 0.0 and d["v2_phi"] == 0.0
+
+
+# ------------------------------------------------------ <v^2>_omega, the equation-of-state estimator (Eq. 17 right)
+
+def test_v2_omega_limits(oracle):
+    """<v^2>_omega = (1 + 3 sum p W / sum rho W) / 2 on states whose equation of state is known
+    whatever the weight: pure kinetic energy p = rho (v^2 = 2 by the formula), pure potential p = -rho (v^2 = -1),
+    pure electric field p = rho/3 (radiation: v^2 = 1), a uniform magnetic field p = rho/3 as well."""
+    o = oracle
+    P = o.make_params(4, 5, 3, dx=0.5, lambda0=2.0, e0=0.9, sigma=1.0, p=1.0, s=1.0, tau_ref=2.0)
+    tau, dt = 1.4, 0.1
+    vac = o.empty_fields(P)
+    vac[0] = 1.0                               # phi = sigma: no gradient, no potential
+    f = vac.copy(); f[2] = 0.3; f[3] = -0.1    # only |Pi|^2
+    assert o.diagnostics(P, f, tau, dt)["v2_omega"] == pytest.approx(2.0, rel=1e-12)
+    f = vac.copy(); f[0] = 0.6                 # only the potential
+    assert o.diagnostics(P, f, tau, dt)["v2_omega"] == pytest.approx(-1.0, rel=1e-12)
+    f = vac.copy(); f[7] = 0.2; f[9] = -0.3    # only the electric field; phi = sigma, th = 0: no current either
+    assert o.diagnostics(P, f, tau, dt)["v2_omega"] == pytest.approx(1.0, rel=1e-12)
+    f = o.empty_fields(P)                      # phi = 0, th_x = B y: only the magnetic energy (and the constant potential)
+    f[4] = 0.37 * np.arange(P.ny)[None, :, None]
+    d = o.diagnostics(P, f, tau, dt)
+    _, q, _, _ = o.coeffs(P, tau, dt)
+    N = P.nx * P.ny * P.nz
+    b2 = np.array([2 * (1 - np.cos(0.37))] * (P.ny - 1) + [2 * (1 - np.cos(0.37 * (P.ny - 1)))]) / 0.5**4 / (2 * 0.9**2 * q)
+    V = 0.25 * 2.0 * q
+    L, rho, prs = -V - b2, V + b2, -V + b2 / 3.0
+    assert d["sum_rho_L"] == pytest.approx(P.nx * P.nz * (rho * L).sum(), rel=1e-12)
+    assert d["sum_p_L"] == pytest.approx(P.nx * P.nz * (prs * L).sum(), rel=1e-12)
+
+
+def test_v2_omega_vanishes_on_the_static_critical_string(oracle):
+    """At critical coupling (beta = 1) the in-plane stresses of a static straight string vanish point by
+    point (Bogomolnyi), so p = T_zz/3 = -rho/3 everywhere and <v^2>_omega = 0 for ANY weight: the relaxed vortex pair
+    must give 0 up to the lattice's O(dx^2) and the relaxation residual, and <v^2>_phi = 0 with it."""
+    o = oracle
+    _, _, _, d = _pair_energy(o, 32, 0.5, 3000)
+    print("static pair, dx = 0.5 :", d["v2_omega"], d["v2_phi"])
+    assert abs(d["v2_omega"]) < 0.02, d["v2_omega"]
+    assert abs(d["v2_phi"]) < 1e-6
+    _, _, _, d2 = _pair_energy(o, 64, 0.25, 5000)
+    print("static pair, dx = 0.25:", d2["v2_omega"], d2["v2_phi"])
+    assert abs(d2["v2_omega"]) < 0.5 * abs(d["v2_omega"]) + 1e-4, (d["v2_omega"], d2["v2_omega"])   # -> 0 with dx
