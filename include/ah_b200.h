@@ -51,7 +51,7 @@ extern "C" {
 /* z slabs (below): fields whose boundary planes neighbours exchange, and the raw partial sums of a slab's read-outs */
 #define AH_NHALO 6      /* phi_re, phi_im, th_x, th_y, th_z, ep_z */
 #define AH_NDIAG_INT 5  /* |W| sums xy, xz, yz; near-branch count; big-plaquette count            */
-#define AH_NDIAG_FLT 7  /* sum |Pi|^2 L, sum grad2 L, sum L, sum G^2, sum div^2, sum charge^2, max |G| */
+#define AH_NDIAG_FLT 9  /* sums of |Pi|^2 L, grad2 L, L, G^2, div^2, charge^2, p L, rho L; then max |G| (last) */
 
 typedef struct ah_ctx ah_ctx; /* opaque */
 
@@ -81,6 +81,9 @@ typedef struct {
     double gauss_div_l2, gauss_charge_l2;
     double xi_l; /* Lagrangian estimator sqrt(-mu V / sum_x L_x dx^3), mu = 2 pi sigma^2 (Eq. 16 left,
                     PAPER.md:102; reading #16); +inf when the sum is not negative                        */
+    double sum_p_L, sum_rho_L; /* sum_x p_x L_x, sum_x rho_x L_x: isotropic pressure and energy density of the five
+                    pieces of L_x, weighted with L_x (reading #17)                               */
+    double v2_omega; /* equation-of-state estimator (1 + 3 sum p L / sum rho L) / 2 (Eq. 17 right)  */
 } ah_diag;
 
 /*
@@ -189,7 +192,7 @@ int ah_slab_exchange_done(ah_ctx *ctx, void *comm_stream);
 int ah_slab_diagnostics(ah_ctx *ctx, double tau, double dt);
 
 /* The slab's raw partial sums of the last requested read-out (synchronises the stream).  Slabs combine them by
- * adding counts and sums[0..5] and taking the maximum of sums[6] (an all-reduce of 12 numbers), then ah_diag_finish. */
+ * adding counts and sums[0..7] and taking the maximum of sums[8] (an all-reduce of 14 numbers), then ah_diag_finish. */
 int ah_slab_diag_partial(ah_ctx *ctx, int64_t host_counts[AH_NDIAG_INT], double host_sums[AH_NDIAG_FLT]);
 
 /* Totals of a whole lattice -> the ah_diag record; host arithmetic only: xi_W, xi_L, <v^2>_phi, Gauss norms. */

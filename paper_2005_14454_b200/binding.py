@@ -22,7 +22,7 @@ LIB_PATH = _PKG / "libah_b200.so"
 
 AH_OK, AH_EINVAL, AH_ECUDA, AH_ESTATE = 0, -1, -2, -3
 AH_NFIELDS = 10
-AH_NHALO, AH_NDIAG_INT, AH_NDIAG_FLT = 6, 5, 7
+AH_NHALO, AH_NDIAG_INT, AH_NDIAG_FLT = 6, 5, 9
 HALO_FIELDS = (0, 1, 4, 5, 6, 9)          # phi_re, phi_im, th_x, th_y, th_z, ep_z (include/ah_b200.h)
 KERNEL_AUTO, KERNEL_SITE, KERNEL_TILED = 0, 1, 2
 PRECISION_FP32, PRECISION_FP64, PRECISION_MIXED = 0, 1, 2
@@ -66,6 +66,7 @@ class Diag(C.Structure):
         ("gauss_max", C.c_double), ("gauss_l2", C.c_double), ("gauss_rel", C.c_double),
         ("gauss_div_l2", C.c_double), ("gauss_charge_l2", C.c_double),
         ("xi_l", C.c_double),
+        ("sum_p_L", C.c_double), ("sum_rho_L", C.c_double), ("v2_omega", C.c_double),
     ]
 
     def asdict(self):
@@ -406,7 +407,7 @@ class SlabSimulation:
 
 
 def combine_partials(parts):
-    """Totals of per-slab (counts, sums): counts and sums[0..5] add, sums[6] (max |G|) takes the maximum."""
+    """Totals of per-slab (counts, sums): counts and all sums but the last add, the last (max |G|) takes the maximum."""
     counts = [sum(p[0][a] for p in parts) for a in range(AH_NDIAG_INT)]
     sums = [sum(p[1][a] for p in parts) for a in range(AH_NDIAG_FLT - 1)] + [max(p[1][AH_NDIAG_FLT - 1] for p in parts)]
     return counts, sums

@@ -306,6 +306,10 @@ void finish_diag(const ah_params &P, const ah::DiagPartial &r, double tau, ah_di
     } else {
         out->v2_phi = 0.0;
     }
+    out->sum_p_L = r.f[ah::DF_SPL];
+    out->sum_rho_L = r.f[ah::DF_SRL];
+    // Eq. 17 right with reading #17
+    out->v2_omega = out->sum_rho_L != 0.0 ? 0.5 * (1.0 + 3.0 * out->sum_p_L / out->sum_rho_L) : 0.0;
     out->gauss_max = r.f[ah::DF_GMAX];
     out->gauss_l2 = std::sqrt(r.f[ah::DF_GSQ]);
     out->gauss_div_l2 = std::sqrt(r.f[ah::DF_DIVSQ]);

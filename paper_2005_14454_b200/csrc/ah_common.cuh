@@ -61,8 +61,8 @@ struct ZRange {
 enum {
     DS_NW_XY = 0, DS_NW_XZ, DS_NW_YZ, DS_NEAR, DS_BIG,   // integer counts (stored as double-exact int64)
     DS_NINT = 5,
-    DF_SPI = 0, DF_SGR, DF_SL, DF_GSQ, DF_DIVSQ, DF_CHSQ, DF_GMAX,
-    DS_NFLT = 7
+    DF_SPI = 0, DF_SGR, DF_SL, DF_GSQ, DF_DIVSQ, DF_CHSQ, DF_SPL, DF_SRL, DF_GMAX,   // DF_GMAX (a maximum) stays last
+    DS_NFLT = 9
 };
 
 struct DiagPartial {

@@ -108,13 +108,14 @@ __device__ __forceinline__ void site_readouts(const ConstFields<float> &in, cons
     hop_fwd_f32(czv, sz, pr[cz], pi[cz], hzr, hzi);
     const float pir = in.f[PI_RE][c], pii = in.f[PI_IM][c];
     const float ex = in.f[EP_X][c], ey = in.f[EP_Y][c], ez = in.f[EP_Z][c];
-    float pi2L, gr2L, L;
+    float pi2L, gr2L, L, pL, rhoL;
     readout_lagrangian(fr, fi, readout_grad2(fr, fi, hxr, hxi, hyr, hyi, hzr, hzi, k.f_idx2),
-                       readout_plaq_energy(Pxy, Pxz, Pyz, k.compact, k.f_idx4), pir, pii, ex, ey, ez, k, pi2L, gr2L, L);
+                       readout_plaq_energy(Pxy, Pxz, Pyz, k.compact, k.f_idx4), pir, pii, ex, ey, ez, k, pi2L, gr2L, L,
+                       pL, rhoL);
     // D3
     double G, div, charge;
     readout_gauss(fr, fi, pir, pii, ex, ey, ez, a.ep_back(0), a.ep_back(1), a.ep_back(2), k, G, div, charge);
-    readout_accumulate(acc, pi2L, gr2L, L, G, div, charge);
+    readout_accumulate(acc, pi2L, gr2L, L, pL, rhoL, G, div, charge);
 }
 
 // One partial per VIRTUAL block vb = (bx, by, bz) of 64 x 4 x 8 sites; the launched blocks take virtual blocks
@@ -136,7 +137,7 @@ diag_kernel(ConstFields<real> in, DiagCoef k, int nx, int ny, int nz, int z_lo, 
     const bool active = (x < nx) && (y < ny);
 
     long long cnt[DS_NINT] = {0, 0, 0, 0, 0};
-    double acc[DS_NFLT] = {0, 0, 0, 0, 0, 0, 0};
+    double acc[DS_NFLT] = {0, 0, 0, 0, 0, 0, 0, 0, 0};
 
     const int z_end = min(z_hi, z_lo + (vbz + 1) * DBZ);
     const size_t n = (size_t)nx * ny * nz;

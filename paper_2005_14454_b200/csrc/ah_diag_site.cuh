@@ -168,6 +168,12 @@ __device__ __forceinline__ void diag_site(const A &a, const DiagCoef &k, long lo
     acc[DF_SPI] += (double)pi2 * (double)L;
     acc[DF_SGR] += (double)grad2 * (double)L;
     acc[DF_SL] += (double)L;
+    // Eq. 17 right, reading #17: energy density and isotropic pressure of the same five pieces
+    const real eb = (e2 + b2) * (real)k.inv_2e2q;
+    const real rho = pi2 + grad2 + pot + eb;
+    const real prs = pi2 - grad2 * (real)(1.0 / 3.0) - pot + eb * (real)(1.0 / 3.0);
+    acc[DF_SPL] += (double)prs * (double)L;
+    acc[DF_SRL] += (double)rho * (double)L;
 
     // ---- D3: Gauss residual, fp64 from the stored values
     double div = 0.0;
@@ -315,10 +321,11 @@ __device__ __forceinline__ float readout_grad2(float fr, float fi, float hxr, fl
     return __fmul_rn(g, idx2);
 }
 
-// D2 of one site (reading #15): L and its two weighted companions |Pi|^2 L, grad2 L (fp32 terms, summed in fp64)
+// D2 of one site (reading #15): L and its weighted companions |Pi|^2 L, grad2 L, and p L, rho L of the
+// equation-of-state estimator (Eq. 17 right, reading #17) (fp32 terms, summed in fp64)
 __device__ __forceinline__ void readout_lagrangian(float fr, float fi, float grad2, float b2, float pir, float pii,
                                                    float ex, float ey, float ez, const DiagCoef &k, float &pi2L,
-                                                   float &gr2L, float &L)
+                                                   float &gr2L, float &L, float &pL, float &rhoL)
 {
     const float pi2 = __fmaf_rn(pir, pir, __fmul_rn(pii, pii));
     const float e2 = __fmul_rn(__fmaf_rn(ez, ez, __fmaf_rn(ey, ey, __fmul_rn(ex, ex))), k.f_idx2);
@@ -327,6 +334,11 @@ __device__ __forceinline__ void readout_lagrangian(float fr, float fi, float gra
     L = __fmaf_rn(__fadd_rn(e2, -b2), k.f_inv_2e2q, __fadd_rn(__fadd_rn(pi2, -grad2), -pot));
     pi2L = __fmul_rn(pi2, L);
     gr2L = __fmul_rn(grad2, L);
+    const float eb = __fmul_rn(__fadd_rn(e2, b2), k.f_inv_2e2q);
+    const float rho = __fadd_rn(__fadd_rn(__fadd_rn(pi2, grad2), pot), eb);
+    const float prs = __fmaf_rn(eb, 0.333333343267440796f, __fadd_rn(__fmaf_rn(grad2, -0.333333343267440796f, pi2), -pot));
+    pL = __fmul_rn(prs, L);
+    rhoL = __fmul_rn(rho, L);
 }
 
 // D3 of one site, in fp64 from the stored fp32 values (a difference of nearly equal numbers)
@@ -342,12 +354,14 @@ __device__ __forceinline__ void readout_gauss(float fr, float fi, float pir, flo
 }
 
 // adds one site's D2 + D3 terms to the fp64 accumulators
-__device__ __forceinline__ void readout_accumulate(double *acc, float pi2L, float gr2L, float L, double G, double div,
-                                                   double charge)
+__device__ __forceinline__ void readout_accumulate(double *acc, float pi2L, float gr2L, float L, float pL, float rhoL,
+                                                   double G, double div, double charge)
 {
     acc[DF_SPI] += (double)pi2L;
     acc[DF_SGR] += (double)gr2L;
     acc[DF_SL] += (double)L;
+    acc[DF_SPL] += (double)pL;
+    acc[DF_SRL] += (double)rhoL;
     acc[DF_GSQ] = __fma_rn(G, G, acc[DF_GSQ]);
     acc[DF_DIVSQ] = __fma_rn(div, div, acc[DF_DIVSQ]);
     acc[DF_CHSQ] = __fma_rn(charge, charge, acc[DF_CHSQ]);

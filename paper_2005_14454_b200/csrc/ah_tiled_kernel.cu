@@ -726,12 +726,12 @@ tiled_step_kernel(ConstFields<float> in, Fields<float> out, StepCoef<float> k, i
                     const float ex = sm.qe[w][2][cq], ey = sm.qe[w][3][cq], ez = sm.qe[w][4][cq];
                     const float exl = sm.qe[w][2][cq > 0 ? cq - 1 : 0];
                     const float exb = (cq == 0) ? ex_left : exl;
-                    float pi2L, gr2L, L;
+                    float pi2L, gr2L, L, pL, rhoL;
                     readout_lagrangian(fr, fi, scr[cq], readout_plaq_energy(Pxy, Pxz, Pyz, COMPACT ? 1 : 0, dk.f_idx4), pir,
-                                       pii, ex, ey, ez, dk, pi2L, gr2L, L);
+                                       pii, ex, ey, ez, dk, pi2L, gr2L, L, pL, rhoL);
                     double G, div, charge;
                     readout_gauss(fr, fi, pir, pii, ex, ey, ez, exb, eby, ebz, dk, G, div, charge);
-                    readout_accumulate(acc, pi2L, gr2L, L, G, div, charge);
+                    readout_accumulate(acc, pi2L, gr2L, L, pL, rhoL, G, div, charge);
                 }
 #pragma unroll
                 for (int a = 0; a < 3; ++a) sm.dwnd[a][threadIdx.x] = wnd[a];
@@ -756,7 +756,7 @@ tiled_step_kernel(ConstFields<float> in, Fields<float> out, StepCoef<float> k, i
     if constexpr (DIAG) {
         // CTA reduction: warp shuffles, then the warps through shared memory (the hand-over rows are free now)
         int d_cnt[DS_NINT] = {0, 0, 0, 0, 0};
-        double d_acc[DS_NFLT] = {0, 0, 0, 0, 0, 0, 0};
+        double d_acc[DS_NFLT] = {0, 0, 0, 0, 0, 0, 0, 0, 0};
         if (is_main) {
 #pragma unroll
             for (int a = 0; a < 3; ++a) d_cnt[a] = (int)sm.dwnd[a][threadIdx.x];

@@ -16,7 +16,7 @@ import sys
 import numpy as np
 
 
-KEYS = ("tau", "n_wind", "xi_w", "xi_l", "v2_phi", "gauss_rel", "sum_L")
+KEYS = ("tau", "n_wind", "xi_w", "xi_l", "v2_phi", "v2_omega", "gauss_rel", "sum_L")
 
 
 def main(argv=None):
@@ -58,6 +58,7 @@ def main(argv=None):
     tau = np.array([r["tau"] for r in recs])
     xi = np.array([r["xi_w"] for r in recs])
     v2 = np.array([r["v2_phi"] for r in recs])
+    vw = np.array([r["v2_omega"] for r in recs])
     xl = np.array([r["xi_l"] for r in recs])
     lo = args.fit_from if args.fit_from is not None else tau0 + 0.4 * (tau_end - tau0)
     m = (tau >= lo) & np.isfinite(xi)
@@ -72,7 +73,8 @@ def main(argv=None):
             summary.update(xi_l_slope=float(np.polyfit(tau[ml], xl[ml], 1)[0]))
         summary.update(xi_w_slope=float(slope), xi_w_intercept=float(icpt),
                        xi_w_slope_manhattan_corrected=float(slope * np.sqrt(6.0 / np.pi)),
-                       v2_phi_mean=float(v2[m].mean()), v2_phi_std=float(v2[m].std()), n_fit=int(m.sum()))
+                       v2_phi_mean=float(v2[m].mean()), v2_phi_std=float(v2[m].std()),
+                       v2_omega_mean=float(vw[m].mean()), v2_omega_std=float(vw[m].std()), n_fit=int(m.sum()))
     print(json.dumps(summary), flush=True)
     return 0
 

@@ -112,7 +112,8 @@ def test_1024_cubed_sampled_step_parity_and_invariants(oracle):
     for key in ("n_wind", "n_wind_xy", "n_wind_xz", "n_wind_yz", "n_near_branch", "n_big_plaq"):
         assert rec[key] == d1[key], (key, rec[key], d1[key])
     assert rec["gauss_max"] == d1["gauss_max"]
-    for key in ("sum_pi2_L", "sum_grad2_L", "sum_L", "gauss_l2", "gauss_div_l2", "gauss_charge_l2", "v2_phi"):
+    for key in ("sum_pi2_L", "sum_grad2_L", "sum_L", "sum_p_L", "sum_rho_L", "gauss_l2", "gauss_div_l2", "gauss_charge_l2",
+                "v2_phi", "v2_omega"):
         assert rec[key] == pytest.approx(d1[key], rel=FUSED_SUM_RTOL), key
     # ... and the fused step moved the sampled sites exactly as the oracle says (same bound as the plain step)
     Po5 = oracle.make_params(5, 5, 5, **MODEL)

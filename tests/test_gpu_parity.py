@@ -364,9 +364,10 @@ def test_parity_config3_512cubed_matter_fused_record(ah, oracle):
         assert abs(rec[key] - od[key]) <= slack, (key, rec[key], od[key], slack)
     assert rec["n_wind"] > 1000
     assert rec["n_big_plaq"] == od["n_big_plaq"]
-    for key in ("sum_pi2_L", "sum_grad2_L", "sum_L"):
+    for key in ("sum_pi2_L", "sum_grad2_L", "sum_L", "sum_p_L", "sum_rho_L"):
         assert rec[key] == pytest.approx(od[key], rel=1e-5), (key, rec[key], od[key])
     assert rec["v2_phi"] == pytest.approx(od["v2_phi"], abs=1e-5)
+    assert rec["v2_omega"] == pytest.approx(od["v2_omega"], abs=1e-5)
     assert rec["xi_l"] == pytest.approx(od["xi_l"], rel=1e-5)
     for key in ("gauss_max", "gauss_l2", "gauss_div_l2", "gauss_charge_l2"):
         assert rec[key] == pytest.approx(od[key], rel=1e-9), (key, rec[key], od[key])
@@ -441,6 +442,7 @@ def test_static_vortex_pair_cooling_on_the_tiled_kernel(ah, oracle):
     assert 0.005 < deficit < 0.02, deficit
     assert d["xi_l"] == pytest.approx(d["xi_w"] * (1 + 0.5 * deficit), rel=2e-3)
     assert d["v2_phi"] < 1e-6
+    assert abs(d["v2_omega"]) < 0.02          # p = -rho/3 on the static critical-coupling string (O(dx^2) on the lattice)
     # static: 300 undamped Minkowski steps move nothing beyond the relaxation residual
     eps = max(np.abs(g[2:4]).max(), np.abs(g[7:10]).max())
     sim.step(300, 1.0, dt)
@@ -499,9 +501,10 @@ def test_sigma_diagnostics_on_snapshot(ah, oracle, model):
     snap = sim.get_fields().astype(np.float64)
     d_gpu = sim.diagnostics(tau, 0.1)
     d_or = oracle.diagnostics(Po, snap, tau, 0.1)
-    for key in ("sum_pi2_L", "sum_grad2_L", "sum_L"):
+    for key in ("sum_pi2_L", "sum_grad2_L", "sum_L", "sum_p_L", "sum_rho_L"):
         assert d_gpu[key] == pytest.approx(d_or[key], rel=1e-5), (key, d_gpu[key], d_or[key])
     assert d_gpu["v2_phi"] == pytest.approx(d_or["v2_phi"], abs=1e-5)
+    assert d_gpu["v2_omega"] == pytest.approx(d_or["v2_omega"], abs=1e-5)      # Eq. 17 right
     # Gauss: evaluated in fp64 from the same stored values on both sides
     for key in ("gauss_max", "gauss_l2", "gauss_div_l2", "gauss_charge_l2"):
         assert d_gpu[key] == pytest.approx(d_or[key], rel=1e-9), (key, d_gpu[key], d_or[key])
@@ -571,7 +574,8 @@ def test_fused_step_diag_tiled_kernel(ah, oracle, shape, model):
     recs = a.step_diag(nsteps, tau0, dt, every)
     assert len(recs) == 3
     ints = ("n_wind", "n_wind_xy", "n_wind_xz", "n_wind_yz", "n_near_branch", "n_big_plaq")
-    sums = ("sum_pi2_L", "sum_grad2_L", "sum_L", "gauss_l2", "gauss_div_l2", "gauss_charge_l2", "v2_phi", "gauss_rel")
+    sums = ("sum_pi2_L", "sum_grad2_L", "sum_L", "sum_p_L", "sum_rho_L", "gauss_l2", "gauss_div_l2", "gauss_charge_l2",
+            "v2_phi", "v2_omega", "gauss_rel")
     Po = oracle.make_params(nx, ny, nz, **model)
     done = 0
     for r in recs:

@@ -52,7 +52,8 @@ def test_slabs_reproduce_the_single_lattice_bit_for_bit(ah, shape, nslabs, overl
     for key in ("n_wind", "n_wind_xy", "n_wind_xz", "n_wind_yz", "n_near_branch", "n_big_plaq"):
         assert d1[key] == d2[key], key
     assert d1["gauss_max"] == d2["gauss_max"]
-    for key in ("sum_pi2_L", "sum_grad2_L", "sum_L", "gauss_l2", "gauss_div_l2", "gauss_charge_l2", "v2_phi", "xi_l", "xi_w"):
+    for key in ("sum_pi2_L", "sum_grad2_L", "sum_L", "sum_p_L", "sum_rho_L", "gauss_l2", "gauss_div_l2", "gauss_charge_l2",
+                "v2_phi", "v2_omega", "xi_l", "xi_w"):
         assert d2[key] == pytest.approx(d1[key], rel=1e-11), key
     one.close()
     grp.close()
@@ -75,7 +76,7 @@ def test_slab_fused_records_equal_single_lattice_records(ah):
         for key in ("n_wind", "n_wind_xy", "n_wind_xz", "n_wind_yz", "n_near_branch", "n_big_plaq"):
             assert a[key] == b[key], key
         assert a["gauss_max"] == b["gauss_max"]
-        for key in ("sum_pi2_L", "sum_grad2_L", "sum_L", "gauss_l2", "gauss_div_l2", "gauss_charge_l2"):
+        for key in ("sum_pi2_L", "sum_grad2_L", "sum_L", "sum_p_L", "sum_rho_L", "gauss_l2", "gauss_div_l2", "gauss_charge_l2"):
             assert b[key] == pytest.approx(a[key], rel=1e-11, abs=1e-300), key
     assert r1[0]["n_wind"] > 0
     assert np.array_equal(one.get_fields(), grp.get_fields())

@@ -157,4 +157,5 @@ def test_slab_partition_and_schedule_host_logic():
     with pytest.raises(ValueError):
         ah.slab_planes(4, 5, 0)
     assert ah.halo_schedule(0, 1) == [("send", 0, 0), ("recv", 3, 0), ("send", 1, 0), ("recv", 2, 0)]
-    assert ah.combine_partials([([1] * 5, [1.0] * 6 + [3.0]), ([2] * 5, [0.5] * 6 + [7.0])]) == ([3] * 5, [1.5] * 6 + [7.0])
+    nf = ah.AH_NDIAG_FLT - 1
+    assert ah.combine_partials([([1] * 5, [1.0] * nf + [3.0]), ([2] * 5, [0.5] * nf + [7.0])]) == ([3] * 5, [1.5] * nf + [7.0])
