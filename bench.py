@@ -54,6 +54,10 @@ def parse():
     ap.add_argument("--sustained-steps", type=int, default=200,
                     help="after the K timed steps, time a further window of this many steps (0 = skip) and report it "
                          "as roofline.sustained: the number the board holds under its power cap")
+    ap.add_argument("--decomp", default="replicas", choices=["replicas", "slabs"],
+                    help="N > 1: independent replicas (default; BASELINE north_star keeps one lattice on one GPU) or ONE "
+                         "lattice of size x size x (N size) cut into z slabs with a per-step exchange of boundary planes "
+                         "over NCCL (SURVEY 8(f)2; untimed on this 1-GPU pool)")
     ap.add_argument("--selftest-launcher", action="store_true",
                     help="CPU-only check of the multi-rank launch path (gloo): no kernels, synthetic per-rank timings")
     return ap.parse_args()
@@ -231,6 +235,8 @@ def run_ours(args):
 
     n, K, W = args.size, args.steps, max(args.warmup, 3)
     params = workload_params(n, total_steps(args))
+    if args.decomp == "slabs":
+        return run_slabs(args, torch, dist, binding, replicas, params, rank, local, world)
     sim = binding.Simulation(params=binding.make_params(n, **params), device=f"cuda:{local}")
     if args.kernel != "auto":
         sim.set_kernel({"site": binding.KERNEL_SITE, "tiled": binding.KERNEL_TILED}[args.kernel])
@@ -359,6 +365,45 @@ def run_ours(args):
     sim.close()
     if world > 1:
         dist.destroy_process_group()
+    return 0
+
+
+def run_slabs(args, torch, dist, binding, replicas, params, rank, local, world):
+    """--decomp slabs: ONE periodic lattice of size x size x (world * size) sites, one z slab per rank, boundary planes
+    exchanged over torch.distributed (NCCL) every step, overlapped with the update of the interior (weak scaling in z)."""
+    n, K, W = args.size, args.steps, max(args.warmup, 3)
+    if world == 1 and not dist.is_initialized():
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        os.environ.setdefault("MASTER_PORT", str(free_port()))
+        dist.init_process_group("gloo", rank=0, world_size=1)
+    P = binding.make_params(n, n, n * world, **params)
+    ds = binding.DistributedSlab(P, dist, device=f"cuda:{local}")
+    ds.slab.init_fields(1)
+    ds.step(W, TAU0, DT)
+    torch.cuda.synchronize()
+    dist.barrier()
+    torch.cuda.synchronize()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    l0 = ds.slab.launch_count()
+    ev0.record(ds.slab.stream)
+    ds.step(K, TAU0 + W * DT, DT)
+    ev1.record(ds.slab.stream)
+    torch.cuda.synchronize()
+    dist.barrier()
+    ms, units = replicas.aggregate(ev0.elapsed_time(ev1), float(n) ** 3 * K, dist if world > 1 else None,
+                                   device="cuda" if dist.get_backend() == "nccl" else "cpu")
+    if rank == 0:
+        value = replicas.throughput(ms, units)
+        print(json.dumps({
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W, "ms_per_step": ms / K,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": {"workload": f"ONE {n}x{n}x{n * world} periodic lattice in {world} z slab(s), radiation era, s=1, "
+                                   "seeded random-phase IC, no diagnostics", "parallelism": f"z slabs x{world}, halo exchange "
+                                   "of 6 planes per direction and step on a communication stream"},
+            "pct_of_8TBs_roofline": 100.0 * value / world * BYTES_PER_SITE / (NOMINAL_HBM_GBS * 1e9),
+            "gpu_launches": int(ds.slab.launch_count() - l0)}), flush=True)
+    ds.slab.close()
+    dist.destroy_process_group()
     return 0
 
 

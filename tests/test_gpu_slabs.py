@@ -123,3 +123,36 @@ def test_slab_api_errors(ah):
     whole = ah.Simulation(params=P)
     assert L.ah_slab_step(whole._ctx, 1.0, 0.1, 0, None) == ah.AH_ESTATE
     whole.close()
+
+
+def test_distributed_slab_single_rank(ah):
+    """DistributedSlab (one slab per rank over torch.distributed) with a world of one rank: the slab is its own
+    neighbour, the exchange degenerates to copies on the communication stream, read-outs go through the all-reduce
+    path.  Must equal the single lattice bit for bit.  (More ranks need more GPUs; the exchange schedule itself is
+    covered over gloo in tests/test_replicas_gloo.py.)"""
+    import os
+    import socket
+    import torch.distributed as dist
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port))
+    dist.init_process_group("gloo", rank=0, world_size=1)
+    try:
+        nx, ny, nz = 128, 9, 14
+        P = ah.make_params(nx, ny, nz, **MODEL)
+        one = ah.Simulation(params=P)
+        ds = ah.DistributedSlab(P, dist)
+        one.init_fields(2)
+        ds.slab.init_fields(2)
+        r1 = one.step_diag(6, 1.0, 0.1, 3)
+        r2 = ds.step(6, 1.0, 0.1, diag_every=3)
+        assert np.array_equal(one.get_fields(), ds.slab.get_fields()[:, 1:-1])
+        assert [a["n_wind"] for a in r1] == [b["n_wind"] for b in r2]
+        assert r2[1]["sum_L"] == pytest.approx(r1[1]["sum_L"], rel=1e-11)
+        d1, d2 = one.diagnostics(1.6, 0.1), ds.diagnostics(1.6, 0.1)
+        assert d1["n_wind"] == d2["n_wind"] and d2["v2_omega"] == pytest.approx(d1["v2_omega"], rel=1e-11)
+        one.close()
+        ds.slab.close()
+    finally:
+        dist.destroy_process_group()
