@@ -267,6 +267,14 @@ tiled_step_kernel(ConstFields<float> in, Fields<float> out, StepCoef<float> k, i
         }
     };
     // running state of the next load (no division in the march): ring slot, plane offset of plane z0 - 1 + n
+    //
+    // Write-after-read on a ring slot: produce() overwrites (async proxy) the slot whose plane the generic-proxy
+    // loads of ALL warps read last in phase 1 of the previous iteration (DIAG: in phase 2 of the iteration before the
+    // CTA barrier it follows).  Every call site sits after the __syncthreads that follows those reads, and a read
+    // value has gone through dependent arithmetic (or a store) before its thread reaches that barrier, so no read of
+    // the old plane can still be in flight when the copy is issued.  A violation would put the next plane's phi, th
+    // under a slower warp's loads and change Pi+, ep+ of its row by O(1): test_one_step_fp32 (256,16,11) and
+    // test_tiled_step_repeats_bit_identically would fail.
     int ld_slot = 0, ld_z = (z0 == 0) ? nz - 1 : z0 - 1;
     size_t ld_plane = (size_t)ld_z * sxy;
     auto produce = [&]() {
@@ -287,7 +295,10 @@ tiled_step_kernel(ConstFields<float> in, Fields<float> out, StepCoef<float> k, i
         }
     };
 
-    // Pi, ep of the warp's own row, plane after plane starting at z0 -> sm.qe[w]
+    // Pi, ep of the warp's own row, plane after plane starting at z0 -> sm.qe[w].
+    // Write-after-read: only the warp itself reads sm.qe[w]; produce_q() is called after the __syncwarp that follows
+    // the last use of the staged values in arithmetic (plain: the final Eq. 7-10 updates; DIAG: the read-out loop), so
+    // the refill cannot land under a lane that has not read yet.
     size_t q_off = (size_t)z0 * sxy + (size_t)(y0 + w < ny ? y0 + w : 0) * nx + x0;
     auto produce_q = [&]() {
         if (elect_one()) {
