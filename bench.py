@@ -49,6 +49,8 @@ def parse():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--diag-every", type=int, default=0, help="fused diagnostics every n steps (0 = none)")
+    ap.add_argument("--diag-sums-only", action="store_true",
+                    help="with --diag-every: ah_step_diag_sums (xi_L, <v^2>, Gauss; no winding), the paper's timed set")
     ap.add_argument("--pre-steps", type=int, default=0,
                     help="untimed steps before the warm-up (starts the timed window at a later epoch tau)")
     ap.add_argument("--sustained-steps", type=int, default=200,
@@ -252,7 +254,7 @@ def run_ours(args):
 
     def advance(nsteps, tau):
         if args.diag_every > 0:
-            return len(sim.step_diag(nsteps, tau, DT, args.diag_every))
+            return len(sim.step_diag(nsteps, tau, DT, args.diag_every, winding=not args.diag_sums_only))
         sim.step(nsteps, tau, DT)
         return 0
 
@@ -348,6 +350,7 @@ def run_ours(args):
             "config": {"workload": f"{n}^3 periodic lattice, dx=0.5, dt=0.1, fp32 SoA ping-pong ({20 * 4 * sites / 1e9:.1f} GB), "
                                    f"lambda=2, e=1, sigma=1, radiation era, s=1, seeded random-phase IC, "
                                    f"{'no diagnostics' if not diag else 'fused diagnostics every %d steps' % args.diag_every}"
+                                   f"{' (sums only: xi_L, <v^2>, Gauss; no winding)' if diag and args.diag_sums_only else ''}"
                                    f"{' (BASELINE configs[3])' if n == 1024 and not diag else ''}"
                                    f"{' (BASELINE configs[4] row)' if diag and args.diag_every == 10 else ''}",
                        "kernel": kernel_name, "parallelism": "replicas only" if world > 1 else "single GPU",

@@ -148,6 +148,16 @@ int ah_diagnostics(ah_ctx *ctx, double tau, double dt, ah_diag *host_out);
 int ah_step_diag(ah_ctx *ctx, int n, double tau, double dt, int every, ah_diag *host_out, int cap,
                  int *n_written);
 
+/*
+ * ah_step_diag_sums — as ah_step_diag, but the records carry the Lagrangian-weighted estimators (xi_L, <v^2>_phi,
+ * <v^2>_omega and their sums) and the Gauss residual only: the set the paper's timed runs evaluate every 5 steps
+ * (PAPER.md:181).  The winding read-out is skipped (on the tiled kernel neither site phases nor link phases are
+ * computed): n_wind* = n_near_branch = n_big_plaq = -1, string_length = xi_w = NaN.  All other fields are bit-identical
+ * to ah_step_diag's, and so are the fields the steps leave.
+ */
+int ah_step_diag_sums(ah_ctx *ctx, int n, double tau, double dt, int every, ah_diag *host_out, int cap,
+                      int *n_written);
+
 /* Per-plaquette winding integers of the current snapshot: host_w3 receives 3 arrays (xy, xz, yz)
  * of nx*ny*nz int8; host_near3 (may be NULL) the near-branch flags as uint8.  Synchronous. */
 int ah_winding_field(ah_ctx *ctx, int8_t *host_w3, uint8_t *host_near3);

@@ -32,7 +32,7 @@ FIELD_NAMES = ("phi_re", "phi_im", "pi_re", "pi_im", "th_x", "th_y", "th_z", "ep
 # every symbol include/*.h declares (checked by tests/test_abi.py)
 EXPORTS = (
     "ah_create_slab", "ah_slab_step", "ah_slab_halo_ptrs", "ah_slab_exchange_done", "ah_slab_diagnostics",
-    "ah_slab_diag_partial", "ah_diag_finish",
+    "ah_slab_diag_partial", "ah_diag_finish", "ah_step_diag_sums",
     "ah_create", "ah_destroy", "ah_init_fields", "ah_set_fields", "ah_get_fields", "ah_current_bufs",
     "ah_step", "ah_step_cooling", "ah_diagnostics", "ah_step_diag", "ah_winding_field", "ah_set_kernel", "ah_get_kernel",
     "ah_launch_count", "ah_tiled_launch_info", "ah_coeffs", "ah_test_trig", "ah_test_trig_fast", "ah_last_error", "ah_version",
@@ -106,6 +106,7 @@ def lib():
     L.ah_step_cooling.argtypes = [vp, ip, dp, dp]
     L.ah_diagnostics.argtypes = [vp, dp, dp, C.POINTER(Diag)]
     L.ah_step_diag.argtypes = [vp, ip, dp, dp, ip, C.POINTER(Diag), ip, C.POINTER(ip)]
+    L.ah_step_diag_sums.argtypes = [vp, ip, dp, dp, ip, C.POINTER(Diag), ip, C.POINTER(ip)]
     L.ah_winding_field.argtypes = [vp, vp, vp]
     L.ah_set_kernel.argtypes = [vp, ip]
     L.ah_get_kernel.argtypes = [vp]
@@ -247,12 +248,14 @@ class Simulation:
             _check(lib().ah_diagnostics(self._ctx, float(tau), float(dt), C.byref(d)))
         return d.asdict()
 
-    def step_diag(self, n: int, tau: float, dt: float, every: int):
+    def step_diag(self, n: int, tau: float, dt: float, every: int, winding: bool = True):
+        """ah_step_diag (winding=True) or ah_step_diag_sums (winding=False: no winding read-out in the records)."""
         cap = max(1, (n + every - 1) // every) if every >= 1 else 1
         recs = (Diag * cap)()
         nw = C.c_int(0)
+        fn = lib().ah_step_diag if winding else lib().ah_step_diag_sums
         with self._dev():
-            _check(lib().ah_step_diag(self._ctx, int(n), float(tau), float(dt), int(every), recs, cap, C.byref(nw)))
+            _check(fn(self._ctx, int(n), float(tau), float(dt), int(every), recs, cap, C.byref(nw)))
         return [recs[i].asdict() for i in range(nw.value)]
 
     def winding_field(self):

@@ -80,6 +80,7 @@ ah::DiagCoef make_diag_coef(const ah_params &P, double tau, double dt)
     // callers check it (ah_diagnostics returns AH_EINVAL); 0 keeps the kernel's sums finite
     k.two_e2_kappa = (w == 1.0) ? 0.0 : 2.0 * P.e0 * P.e0 * q * (1.0 - d) / (1.0 - w);
     k.compact = P.compact;
+    k.winding = 1;
     k.f_idx2 = (float)k.idx2;
     k.f_idx4 = (float)(k.idx2 * k.idx2);
     k.f_quarter_lam_q = (float)k.quarter_lam_q;
@@ -158,7 +159,7 @@ int check_time(const ah_ctx *c, double tau, double dt)
 // diag_slot >= 0 (tiled fp32 kernel only): the fused DIAG instantiation also leaves the read-outs of the entry
 // snapshot of those planes in d_results[diag_slot] (SURVEY 8(a) row D-fuse).
 cudaError_t enqueue_step(ah_ctx *c, const ah_params &P, double tau, double dt, ah::ZRange zr, int diag_slot, int *flag,
-                         int *next_flag)
+                         int *next_flag, bool winding = true)
 {
     cudaError_t e;
     const int nx = P.nx, ny = P.ny, nza = c->nza;
@@ -173,7 +174,8 @@ cudaError_t enqueue_step(ah_ctx *c, const ah_params &P, double tau, double dt, a
     } else if (c->kernel == AH_KERNEL_TILED) {
         const ah::StepCoef<float> k = make_coef<float>(P, tau, dt);
         if (diag_slot >= 0) {
-            const ah::DiagCoef dk = make_diag_coef(P, tau, dt);
+            ah::DiagCoef dk = make_diag_coef(P, tau, dt);
+            dk.winding = winding ? 1 : 0;
             e = ah::launch_tiled_step(cur_fields<float>(c), next_fields<float>(c), k, nx, ny, nza, zr, flag, c->st, &dk,
                                       c->d_partials);
             // a link angle outside the tiled kernel's domain spoils its read-outs as well: the standalone kernel
@@ -207,10 +209,10 @@ cudaError_t enqueue_step(ah_ctx *c, const ah_params &P, double tau, double dt, a
 // One whole step.  Context state (ping-pong parity, flag parity) changes only after EVERY launch of the step was
 // accepted; a failed launch leaves the context on the entry snapshot with both overflow flags cleared.
 // P: the model the step uses (the context's own, or ah_step_cooling's constant-damping copy of it)
-int one_step(ah_ctx *c, const ah_params &P, double tau, double dt, int diag_slot = -1)
+int one_step(ah_ctx *c, const ah_params &P, double tau, double dt, int diag_slot = -1, bool winding = true)
 {
     int *flag = c->d_overflow + c->step_parity, *next_flag = c->d_overflow + (1 - c->step_parity);
-    const cudaError_t e = enqueue_step(c, P, tau, dt, c->zr, diag_slot, flag, next_flag);
+    const cudaError_t e = enqueue_step(c, P, tau, dt, c->zr, diag_slot, flag, next_flag, winding);
     if (e != cudaSuccess) {
         cudaMemsetAsync(c->d_overflow, 0, 2 * sizeof(int), c->st);   // a half-issued step must not leave a stale flag
         return cuda_fail(e, "step kernel launch");
@@ -278,20 +280,26 @@ int enqueue_diag(ah_ctx *c, double tau, double dt, int slot, int8_t *w3, uint8_t
     return AH_OK;
 }
 
-// totals -> the derived numbers of ah_diag (P: the GLOBAL lattice the totals belong to)
-void finish_diag(const ah_params &P, const ah::DiagPartial &r, double tau, ah_diag *out)
+// totals -> the derived numbers of ah_diag (P: the GLOBAL lattice the totals belong to).
+// winding == false: the record carries no winding read-out (counts -1, lengths NaN), whatever the kernel summed.
+void finish_diag(const ah_params &P, const ah::DiagPartial &r, double tau, ah_diag *out, bool winding = true)
 {
     out->tau = tau;
-    out->n_wind_xy = r.i[ah::DS_NW_XY];
-    out->n_wind_xz = r.i[ah::DS_NW_XZ];
-    out->n_wind_yz = r.i[ah::DS_NW_YZ];
-    out->n_wind = out->n_wind_xy + out->n_wind_xz + out->n_wind_yz;
-    out->n_near_branch = r.i[ah::DS_NEAR];
-    out->n_big_plaq = r.i[ah::DS_BIG];
-    out->string_length = P.dx * (double)out->n_wind;   // L_W = dx * n_W (reading #13)
-    const double V = (double)P.nx * P.ny * P.nz * P.dx * P.dx * P.dx;
-    out->xi_w = out->n_wind > 0 ? std::sqrt(V / out->string_length)
-                                : std::numeric_limits<double>::infinity();
+    if (winding) {
+        out->n_wind_xy = r.i[ah::DS_NW_XY];
+        out->n_wind_xz = r.i[ah::DS_NW_XZ];
+        out->n_wind_yz = r.i[ah::DS_NW_YZ];
+        out->n_wind = out->n_wind_xy + out->n_wind_xz + out->n_wind_yz;
+        out->n_near_branch = r.i[ah::DS_NEAR];
+        out->n_big_plaq = r.i[ah::DS_BIG];
+        out->string_length = P.dx * (double)out->n_wind;   // L_W = dx * n_W (reading #13)
+        const double V = (double)P.nx * P.ny * P.nz * P.dx * P.dx * P.dx;
+        out->xi_w = out->n_wind > 0 ? std::sqrt(V / out->string_length)
+                                    : std::numeric_limits<double>::infinity();
+    } else {
+        out->n_wind = out->n_wind_xy = out->n_wind_xz = out->n_wind_yz = out->n_near_branch = out->n_big_plaq = -1;
+        out->string_length = out->xi_w = std::numeric_limits<double>::quiet_NaN();
+    }
     out->sum_pi2_L = r.f[ah::DF_SPI];
     out->sum_grad2_L = r.f[ah::DF_SGR];
     out->sum_L = r.f[ah::DF_SL];
@@ -571,7 +579,21 @@ int ah_diagnostics(ah_ctx *c, double tau, double dt, ah_diag *out)
     return AH_OK;
 }
 
+static int step_diag_impl(ah_ctx *c, int n, double tau, double dt, int every, ah_diag *out, int cap, int *n_written,
+                          bool winding);
+
 int ah_step_diag(ah_ctx *c, int n, double tau, double dt, int every, ah_diag *out, int cap, int *n_written)
+{
+    return step_diag_impl(c, n, tau, dt, every, out, cap, n_written, true);
+}
+
+int ah_step_diag_sums(ah_ctx *c, int n, double tau, double dt, int every, ah_diag *out, int cap, int *n_written)
+{
+    return step_diag_impl(c, n, tau, dt, every, out, cap, n_written, false);
+}
+
+static int step_diag_impl(ah_ctx *c, int n, double tau, double dt, int every, ah_diag *out, int cap, int *n_written,
+                          bool winding)
 {
     if (!c || !out || !n_written) return fail(AH_EINVAL, "ah_step_diag: null pointer");
     *n_written = 0;
@@ -594,7 +616,7 @@ int ah_step_diag(ah_ctx *c, int n, double tau, double dt, int every, ah_diag *ou
             rc = enqueue_diag(c, tj, dt, r, nullptr, nullptr);
             if (rc != AH_OK) return rc;
         }
-        rc = one_step(c, c->P, tj, dt, fused ? r : -1);
+        rc = one_step(c, c->P, tj, dt, fused ? r : -1, winding);
         if (rc != AH_OK) return rc;
         if (diag) ++r;
     }
@@ -602,7 +624,7 @@ int ah_step_diag(ah_ctx *c, int n, double tau, double dt, int every, ah_diag *ou
         AH_CUDA(cudaMemcpyAsync(c->h_results, c->d_results, sizeof(ah::DiagPartial) * (size_t)r,
                                 cudaMemcpyDeviceToHost, c->st));
     AH_CUDA(cudaStreamSynchronize(c->st));
-    for (int i = 0; i < r; ++i) finish_diag(c->P, c->h_results[i], tau + (double)(i * every) * dt, out + i);
+    for (int i = 0; i < r; ++i) finish_diag(c->P, c->h_results[i], tau + (double)(i * every) * dt, out + i, winding);
     *n_written = r;
     return AH_OK;
 }

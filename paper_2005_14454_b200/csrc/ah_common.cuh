@@ -35,6 +35,8 @@ struct DiagCoef {
     double inv_2e2q;    // 1/(2 e0^2 q)
     double two_e2_kappa;// 2 e0^2 kappa, kappa = q (1-delta)/(1-omega)   reading #18
     int compact;
+    int winding;        // 1: all read-outs; 0: no winding read-out D1 (fused DIAG instantiation only; the
+                        // standalone kernel always evaluates everything and the API masks the record)
     // the same scalars rounded once to fp32 on the host, for the fp32 read-out arithmetic
     float f_idx2, f_idx4, f_quarter_lam_q, f_sig2, f_inv_2e2q;
 };

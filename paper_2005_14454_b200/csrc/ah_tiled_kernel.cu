@@ -210,7 +210,10 @@ namespace {
 //     and one ep_x per row.
 // Per-thread partial sums (int32 counts, fp64 sums) live in shared memory between loops, are reduced per CTA
 // into partials[linear CTA index]; diag_final_kernel adds them in a fixed order.
-template <int SPT, int TY, bool COMPACT, bool DIAG>
+// WIND (DIAG only): include the winding read-out D1 (site phases, link phases, |W| and the two plaquette counts);
+// without it the DIAG instantiation evaluates the Lagrangian-weighted sums and the Gauss residual only — the set
+// the paper's timed runs compute every 5 steps — and needs neither the phase ring nor atan2.
+template <int SPT, int TY, bool COMPACT, bool DIAG, bool WIND>
 __global__ void __launch_bounds__((TY + 1) * 32, ((TY + 1) * 32 <= 256) ? 2 : 1)
 tiled_step_kernel(ConstFields<float> in, Fields<float> out, StepCoef<float> k, int nx, int ny, int nz, int z_lo,
                   int z_hi, int zc, int *overflow, DiagCoef dk, DiagPartial *partials)
@@ -344,7 +347,7 @@ tiled_step_kernel(ConstFields<float> in, Fields<float> out, StepCoef<float> k, i
     // DIAG: site phases of this warp's staged row (helper: halo row TY+1, and the column x0+128 of every row) of
     // the plane in ring slot `slot` -> sm.alpha[slot].  Lane l takes columns l, l+32, ... (conflict-free).
     auto stage_alpha = [&](int slot) {
-        if constexpr (DIAG) {
+        if constexpr (DIAG && WIND) {
             const int r = is_main ? w + 1 : TY + 1;
 #pragma unroll
             for (int j = 0; j < SPT; ++j) {
@@ -721,15 +724,17 @@ tiled_step_kernel(ConstFields<float> in, Fields<float> out, StepCoef<float> k, i
                     const float tx_zp = sm.raw[sf][2][r_own][c], ty_zp = sm.raw[sf][3][r_own][c];
                     const float Pxy = plaq_angle_f32(t0x, ty_xp, tx_yp, t0y), Pxz = plaq_angle_f32(t0x, tz_xp, tx_zp, t0z);
                     const float Pyz = plaq_angle_f32(t0y, tz_yp, ty_zp, t0z);
-                    const SiteWinding sw = readout_winding(
-                        sm.alpha[so][w][c], sm.alpha[so][w][c + 1], sm.alpha[so][w + 1][c], sm.alpha[sf][w][c],
-                        sm.alpha[so][w + 1][c + 1], sm.alpha[sf][w][c + 1], sm.alpha[sf][w + 1][c], t0x, t0y, t0z, ty_xp,
-                        tz_xp, tx_yp, tz_yp, tx_zp, ty_zp, Pxy, Pxz, Pyz);
+                    if constexpr (WIND) {
+                        const SiteWinding sw = readout_winding(
+                            sm.alpha[so][w][c], sm.alpha[so][w][c + 1], sm.alpha[so][w + 1][c], sm.alpha[sf][w][c],
+                            sm.alpha[so][w + 1][c + 1], sm.alpha[sf][w][c + 1], sm.alpha[sf][w + 1][c], t0x, t0y, t0z, ty_xp,
+                            tz_xp, tx_yp, tz_yp, tx_zp, ty_zp, Pxy, Pxz, Pyz);
 #pragma unroll
-                    for (int pq = 0; pq < 3; ++pq) {
-                        wnd[pq] += sw.absw[pq];
-                        n_near += sw.nearf[pq];
-                        n_big += sw.big[pq];
+                        for (int pq = 0; pq < 3; ++pq) {
+                            wnd[pq] += sw.absw[pq];
+                            n_near += sw.nearf[pq];
+                            n_big += sw.big[pq];
+                        }
                     }
                     // D2, D3 (Eqs. 17-18, Eq. 5) from the staged phi, Pi, ep and the step's gradient energy
                     const float fr = sm.raw[so][0][r_own][c], fi = sm.raw[so][1][r_own][c];
@@ -821,23 +826,25 @@ static int spt_for(int nx) { return nx % 128 == 0 ? 4 : 2; }
 
 bool tiled_supported(int nx, int ny, int nz) { return nx >= 64 && nx % 64 == 0 && ny >= 1 && nz >= 1; }
 
-template <int SPT, int TY, bool COMPACT, bool DIAG>
+template <int SPT, int TY, bool COMPACT, bool DIAG, bool WIND>
 static cudaError_t setup_one()
 {
-    cudaError_t e = cudaFuncSetAttribute(tiled_step_kernel<SPT, TY, COMPACT, DIAG>,
+    cudaError_t e = cudaFuncSetAttribute(tiled_step_kernel<SPT, TY, COMPACT, DIAG, WIND>,
                                          cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Smem<SPT, TY, DIAG>));
     if (e != cudaSuccess) return e;
-    return cudaFuncSetAttribute(tiled_step_kernel<SPT, TY, COMPACT, DIAG>,
+    return cudaFuncSetAttribute(tiled_step_kernel<SPT, TY, COMPACT, DIAG, WIND>,
                                 cudaFuncAttributePreferredSharedMemoryCarveout, 100);
 }
 
 template <int SPT>
 static cudaError_t setup_spt()
 {
-    cudaError_t e = setup_one<SPT, TILE_Y, true, false>();
-    if (e == cudaSuccess) e = setup_one<SPT, TILE_Y, false, false>();
-    if (e == cudaSuccess) e = setup_one<SPT, TILE_Y_DIAG, true, true>();
-    if (e == cudaSuccess) e = setup_one<SPT, TILE_Y_DIAG, false, true>();
+    cudaError_t e = setup_one<SPT, TILE_Y, true, false, false>();
+    if (e == cudaSuccess) e = setup_one<SPT, TILE_Y, false, false, false>();
+    if (e == cudaSuccess) e = setup_one<SPT, TILE_Y_DIAG, true, true, true>();
+    if (e == cudaSuccess) e = setup_one<SPT, TILE_Y_DIAG, false, true, true>();
+    if (e == cudaSuccess) e = setup_one<SPT, TILE_Y_DIAG, true, true, false>();
+    if (e == cudaSuccess) e = setup_one<SPT, TILE_Y_DIAG, false, true, false>();
     return e;
 }
 
@@ -892,7 +899,7 @@ int tiled_num_blocks(int nx, int ny, int nz, bool diag)
     return (nx / (32 * spt_for(nx))) * ((ny + ty - 1) / ty) * ((nz + zc - 1) / zc);
 }
 
-template <int SPT, int TY, bool COMPACT, bool DIAG>
+template <int SPT, int TY, bool COMPACT, bool DIAG, bool WIND>
 static cudaError_t launch_one(const ConstFields<float> &in, const Fields<float> &out, const StepCoef<float> &k, int nx,
                               int ny, int nz, ZRange zr, int *overflow, cudaStream_t st, const DiagCoef &d,
                               DiagPartial *partials)
@@ -901,7 +908,7 @@ static cudaError_t launch_one(const ConstFields<float> &in, const Fields<float> 
     dim3 grid(nx / (32 * SPT), (ny + TY - 1) / TY, (zr.hi - zr.lo + zc - 1) / zc);
     dim3 block((TY + 1) * 32);
     if (grid.y > 65535u || grid.z > 65535u) return cudaErrorInvalidConfiguration;
-    return launch_pdl(tiled_step_kernel<SPT, TY, COMPACT, DIAG>, grid, block, sizeof(Smem<SPT, TY, DIAG>), st, in, out, k, nx,
+    return launch_pdl(tiled_step_kernel<SPT, TY, COMPACT, DIAG, WIND>, grid, block, sizeof(Smem<SPT, TY, DIAG>), st, in, out, k, nx,
                       ny, nz, zr.lo, zr.hi, zc, overflow, d, partials);
 }
 
@@ -910,11 +917,14 @@ static cudaError_t launch_spt(const ConstFields<float> &in, const Fields<float> 
                               int ny, int nz, ZRange zr, int *overflow, cudaStream_t st, bool diag, const DiagCoef &d,
                               DiagPartial *partials)
 {
-    if (k.compact)
-        return diag ? launch_one<SPT, TILE_Y_DIAG, true, true>(in, out, k, nx, ny, nz, zr, overflow, st, d, partials)
-                    : launch_one<SPT, TILE_Y, true, false>(in, out, k, nx, ny, nz, zr, overflow, st, d, nullptr);
-    return diag ? launch_one<SPT, TILE_Y_DIAG, false, true>(in, out, k, nx, ny, nz, zr, overflow, st, d, partials)
-                : launch_one<SPT, TILE_Y, false, false>(in, out, k, nx, ny, nz, zr, overflow, st, d, nullptr);
+    if (!diag)
+        return k.compact ? launch_one<SPT, TILE_Y, true, false, false>(in, out, k, nx, ny, nz, zr, overflow, st, d, nullptr)
+                         : launch_one<SPT, TILE_Y, false, false, false>(in, out, k, nx, ny, nz, zr, overflow, st, d, nullptr);
+    if (d.winding)
+        return k.compact ? launch_one<SPT, TILE_Y_DIAG, true, true, true>(in, out, k, nx, ny, nz, zr, overflow, st, d, partials)
+                         : launch_one<SPT, TILE_Y_DIAG, false, true, true>(in, out, k, nx, ny, nz, zr, overflow, st, d, partials);
+    return k.compact ? launch_one<SPT, TILE_Y_DIAG, true, true, false>(in, out, k, nx, ny, nz, zr, overflow, st, d, partials)
+                     : launch_one<SPT, TILE_Y_DIAG, false, true, false>(in, out, k, nx, ny, nz, zr, overflow, st, d, partials);
 }
 
 // partials == nullptr: plain step.  Otherwise the DIAG instantiation, which also writes one DiagPartial per

@@ -638,6 +638,34 @@ def test_one_step_mixed_precision(ah, oracle, case, shape):
     sim.close()
 
 
+@pytest.mark.parametrize("shape", [(128, 20, 9), (64, 7, 6), (20, 12, 7)])
+def test_step_diag_sums_equals_step_diag_without_the_winding(ah, shape):
+    """ah_step_diag_sums (the read-outs the paper's timed runs evaluate): every field of its records
+    except the winding ones is bit-identical to ah_step_diag's, the winding fields say "not computed", and the steps
+    leave the same fields — on the tiled kernel (both row widths) and on the site kernel."""
+    nx, ny, nz = shape
+    a = ah.Simulation(params=ah.make_params(nx, ny, nz, p=1.0, s=1.0, tau_ref=4.0))
+    b = ah.Simulation(params=ah.make_params(nx, ny, nz, p=1.0, s=1.0, tau_ref=4.0))
+    f0 = inputs.random_state(nx, ny, nz, seed=33, th_amp=0.3)
+    a.set_fields(f0)
+    b.set_fields(f0)
+    ra = a.step_diag(9, 1.5, 0.1, 4)
+    rb = b.step_diag(9, 1.5, 0.1, 4, winding=False)
+    assert len(ra) == len(rb) == 3
+    wind = ("n_wind", "n_wind_xy", "n_wind_xz", "n_wind_yz", "n_near_branch", "n_big_plaq")
+    for x, y in zip(ra, rb):
+        for key, val in x.items():
+            if key in wind:
+                assert y[key] == -1 and val >= 0, key
+            elif key in ("string_length", "xi_w"):
+                assert np.isnan(y[key]), key
+            else:
+                assert y[key] == val, (key, y[key], val)
+    assert np.array_equal(a.get_fields(), b.get_fields())
+    a.close()
+    b.close()
+
+
 def test_diagnostics_deterministic(ah):
     sim = ah.Simulation(nx=48, p=1.0, s=0.0)
     sim.init_fields(8)
