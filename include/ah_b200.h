@@ -209,6 +209,57 @@ int ah_slab_diag_partial(ah_ctx *ctx, int64_t host_counts[AH_NDIAG_INT], double 
 int ah_diag_finish(const ah_params *global_params, const int64_t host_counts[AH_NDIAG_INT],
                    const double host_sums[AH_NDIAG_FLT], double tau, ah_diag *host_out);
 
+/*
+ * ah_readout_noalloc — the read-outs D1-D3 of one whole-lattice snapshot (what ah_diagnostics computes: winding
+ * counts, Eq. 16 right; Lagrangian-weighted sums, Eqs. 17-18; Gauss residual,
+ * Eq. 5) WITHOUT a context and without allocating anything, on the device or on the host.
+ *
+ * Who needs it.  Every other read-out call goes through an ah_ctx, and ah_create obtains the context's scratch with
+ * cudaMalloc / cudaMallocHost.  Some callers cannot do that at the moment they want a read-out:
+ *   - a host program that handed (nearly) all of the GPU's memory to its own pool up front (a 1024^3 run already
+ *     holds 86 GB of fields; a framework's caching allocator typically owns the rest), so a driver allocation
+ *     may fail, or may succeed only after the pool is trimmed;
+ *   - a monitoring or steering loop that must not stall the GPU: cudaMalloc and cudaFree synchronise the whole
+ *     device, so a read-out that allocates would drain every stream of the process each time it is asked for;
+ *   - code that runs inside somebody else's no-allocation region (a plugin or callback contract that forbids
+ *     changes to the memory map, a fixed-footprint service that is audited for a constant memory use).
+ * Such callers own the field arrays already (they are the inputs) and can set 112 bytes aside for the result; the
+ * only other memory the read-out needs is the per-block partial sums, and for this call those live in a fixed array
+ * inside the library image.
+ *
+ *   params     : the model and the extents of the lattice (host pointer); fp64 = 0 or 2 reads float arrays, 1 double.
+ *   dev_fields : AH_NFIELDS DEVICE arrays of nx*ny*nz elements in the field order above (e.g. what ah_current_bufs
+ *                returned, or the caller's own buffers); read only.
+ *   tau, dt    : as for ah_diagnostics (fields at tau, momenta at tau - dt/2).
+ *   dev_totals : DEVICE buffer of AH_NOALLOC_TOTALS_BYTES, 8-byte aligned, caller-owned: receives int64
+ *                counts[AH_NDIAG_INT] followed by double sums[AH_NDIAG_FLT], the raw totals that ah_slab_diag_partial
+ *                also returns.  Copy them to the host when convenient and pass them to ah_diag_finish (host
+ *                arithmetic only) for xi_W, xi_L, <v^2>, the Gauss norms.
+ *   cuda_stream: the two kernels are enqueued on it; the call returns without synchronising.
+ *
+ * Limit.  The fixed array holds AH_NOALLOC_MAX_PARTIALS partial sums, one per block of 64 x 4 x 8 sites:
+ * ceil(nx/64) * ceil(ny/4) * ceil(nz/8) must not exceed it, so 512^3 is the largest cube.  Larger lattices get
+ * AH_EINVAL with a message naming the limit; nothing is launched.  The array costs 7 MiB of device memory on every GPU
+ * on which the library's code is loaded, from then until the process ends, whether or not this call is ever made.
+ *
+ * First call.  The first call on each device asks the CUDA runtime for the array's device address
+ * (cudaGetSymbolAddress, once per device, with that device current) and keeps it; later calls only launch.  Make that
+ * first call at start-up, with the device you will use current and before any stream capture begins.
+ *
+ * Sharing.  There is ONE array per device, shared by every call from every thread, and it keeps whatever the last call
+ * left in it.  Nothing in it needs clearing (each call overwrites every entry it later reads), but two calls whose
+ * kernels can run at the same time on one GPU — different streams with no ordering between them — race on it and both
+ * results are then garbage.  Keep the calls of one device on one stream, or order them with events.
+ *
+ * Results are bit-identical to ah_diagnostics on the same snapshot (same kernels, same summation order).
+ * Errors: AH_EINVAL (null or misaligned pointer, bad params, dt <= 0, tau <= 0 with p != 0, omega = 1, lattice beyond
+ * the limit), AH_ECUDA (no device, address look-up or launch failed).
+ */
+#define AH_NOALLOC_MAX_PARTIALS 65536
+#define AH_NOALLOC_TOTALS_BYTES (8 * (AH_NDIAG_INT + AH_NDIAG_FLT))
+int ah_readout_noalloc(const ah_params *params, const void *const dev_fields[AH_NFIELDS], double tau, double dt,
+                       void *dev_totals, void *cuda_stream);
+
 /* Host-side coefficients as the kernels receive them (for tests): a, q = a^{2s}, delta, omega. */
 int ah_coeffs(const ah_params *params, double tau, double dt, double *a, double *q, double *delta,
               double *omega);

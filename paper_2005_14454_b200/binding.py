@@ -32,7 +32,7 @@ FIELD_NAMES = ("phi_re", "phi_im", "pi_re", "pi_im", "th_x", "th_y", "th_z", "ep
 # every symbol include/*.h declares (checked by tests/test_abi.py)
 EXPORTS = (
     "ah_create_slab", "ah_slab_step", "ah_slab_halo_ptrs", "ah_slab_exchange_done", "ah_slab_diagnostics",
-    "ah_slab_diag_partial", "ah_diag_finish", "ah_step_diag_sums",
+    "ah_slab_diag_partial", "ah_diag_finish", "ah_step_diag_sums", "ah_readout_noalloc",
     "ah_create", "ah_destroy", "ah_init_fields", "ah_set_fields", "ah_get_fields", "ah_current_bufs",
     "ah_step", "ah_step_cooling", "ah_diagnostics", "ah_step_diag", "ah_winding_field", "ah_set_kernel", "ah_get_kernel",
     "ah_launch_count", "ah_tiled_launch_info", "ah_coeffs", "ah_test_trig", "ah_test_trig_fast", "ah_last_error", "ah_version",
@@ -97,6 +97,7 @@ def lib():
     L.ah_slab_diagnostics.argtypes = [vp, dp, dp]
     L.ah_slab_diag_partial.argtypes = [vp, C.POINTER(C.c_int64), C.POINTER(dp)]
     L.ah_diag_finish.argtypes = [C.POINTER(Params), C.POINTER(C.c_int64), C.POINTER(dp), dp, C.POINTER(Diag)]
+    L.ah_readout_noalloc.argtypes = [C.POINTER(Params), C.POINTER(vp), dp, dp, vp, vp]
     L.ah_destroy.argtypes = [vp]
     L.ah_init_fields.argtypes = [vp, C.c_uint64]
     L.ah_set_fields.argtypes = [vp, vp]
@@ -289,6 +290,36 @@ def diag_finish(P: Params, counts, sums, tau: float) -> dict:
     d = Diag()
     _check(lib().ah_diag_finish(C.byref(P), ci, cf, float(tau), C.byref(d)))
     return d.asdict()
+
+
+NOALLOC_MAX_PARTIALS = 65536                 # AH_NOALLOC_MAX_PARTIALS: blocks of 64 x 4 x 8 sites (512^3 at most)
+NOALLOC_TOTALS_WORDS = AH_NDIAG_INT + AH_NDIAG_FLT   # dev_totals: that many 8-byte words
+
+
+def readout_noalloc(P: Params, dev_fields, tau: float, dt: float, dev_totals, stream=None):
+    """ah_readout_noalloc: read-outs of the snapshot in the 10 device tensors dev_fields, for callers that may not
+    allocate (see include/ah_b200.h): no context, no cudaMalloc; the partial sums use the library's fixed device array
+    (shared by all calls on a device: keep them on one stream).  dev_totals is the caller's own device tensor of
+    NOALLOC_TOTALS_WORDS int64; it receives the raw totals asynchronously on `stream` (default: torch's current one).
+    Nothing is allocated here either: turn the totals into a record later with noalloc_totals_to_diag."""
+    import torch
+
+    if len(dev_fields) != AH_NFIELDS:
+        raise ValueError(f"need {AH_NFIELDS} field tensors")
+    if dev_totals.dtype != torch.int64 or dev_totals.numel() < NOALLOC_TOTALS_WORDS or not dev_totals.is_cuda:
+        raise ValueError(f"dev_totals must be a CUDA int64 tensor of {NOALLOC_TOTALS_WORDS} elements")
+    st = stream if stream is not None else torch.cuda.current_stream(dev_totals.device)
+    ptrs = (C.c_void_p * AH_NFIELDS)(*[t.data_ptr() for t in dev_fields])
+    with torch.cuda.device(dev_totals.device):
+        _check(lib().ah_readout_noalloc(C.byref(P), ptrs, float(tau), float(dt), C.c_void_p(dev_totals.data_ptr()),
+                                        C.c_void_p(st.cuda_stream)))
+
+
+def noalloc_totals_to_diag(P: Params, host_totals, tau: float) -> dict:
+    """The 14 words ah_readout_noalloc left in dev_totals, copied to the host (numpy int64), -> the ah_diag record
+    (ah_diag_finish).  Words 0..4 are the int64 counts, words 5..13 hold the bit patterns of the double sums."""
+    a = np.ascontiguousarray(host_totals, dtype=np.int64)
+    return diag_finish(P, a[:AH_NDIAG_INT], a[AH_NDIAG_INT:NOALLOC_TOTALS_WORDS].view(np.float64), tau)
 
 
 def slab_planes(nz: int, nslabs: int, r: int):

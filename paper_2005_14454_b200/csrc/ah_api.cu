@@ -772,6 +772,63 @@ int ah_diag_finish(const ah_params *global_params, const int64_t counts[AH_NDIAG
     return AH_OK;
 }
 
+// ------------------------------------------------------------------------------------------------ no allocation
+
+// Read-outs D1-D3 for callers that may not allocate (see ah_b200.h).  Everything is checked before the first CUDA call;
+// no cudaMalloc / cudaFree / cudaMallocHost / event or stream creation happens here or below (the per-block partials
+// live in the fixed device array of ah_diag_kernel.cu, the totals go to the caller's dev_totals).
+static_assert(sizeof(ah::DiagPartial) == AH_NOALLOC_TOTALS_BYTES && ah::DS_NINT == AH_NDIAG_INT &&
+                  ah::DS_NFLT == AH_NDIAG_FLT,
+              "dev_totals layout of ah_b200.h: int64 counts, then double sums");
+
+int ah_readout_noalloc(const ah_params *P, const void *const dev_fields[AH_NFIELDS], double tau, double dt,
+                       void *dev_totals, void *cuda_stream)
+{
+    if (!P || !dev_fields || !dev_totals) return fail(AH_EINVAL, "ah_readout_noalloc: null pointer");
+    int rc = check_params(P, "ah_readout_noalloc");
+    if (rc != AH_OK) return rc;
+    const size_t elem = is_fp64(*P) ? sizeof(double) : sizeof(float);
+    for (int a = 0; a < AH_NFIELDS; ++a) {
+        if (!dev_fields[a]) return fail(AH_EINVAL, "ah_readout_noalloc: dev_fields[%d] is null", a);
+        if (((uintptr_t)dev_fields[a]) & (elem - 1))
+            return fail(AH_EINVAL, "ah_readout_noalloc: dev_fields[%d] is not aligned to its element size", a);
+    }
+    if (((uintptr_t)dev_totals) & 7u) return fail(AH_EINVAL, "ah_readout_noalloc: dev_totals is not 8-byte aligned");
+    if (!(dt > 0.0) || !std::isfinite(dt) || !std::isfinite(tau))
+        return fail(AH_EINVAL, "ah_readout_noalloc: dt must be positive and finite (dt=%g, tau=%g)", dt, tau);
+    if (P->p != 0.0 && !(tau > 0.0))
+        return fail(AH_EINVAL, "ah_readout_noalloc: tau must be > 0 in an expanding background (tau=%g, p=%g)", tau, P->p);
+    {
+        double a, q, d, w;
+        coeffs(*P, tau, dt, a, q, d, w);
+        if (w == 1.0)
+            return fail(AH_EINVAL, "ah_readout_noalloc: omega = (1-s) delta = 1 at tau=%g, dt=%g: no Gauss coefficient",
+                        tau, dt);
+    }
+    const long long need = (long long)((P->nx + 63) / 64) * ((P->ny + 3) / 4) * ((P->nz + 7) / 8);
+    if (need > (long long)ah::diag_noalloc_capacity())
+        return fail(AH_EINVAL,
+                    "ah_readout_noalloc: a %d x %d x %d lattice needs %lld partial sums (one per 64 x 4 x 8 sites), the "
+                    "library's fixed scratch array holds %d (AH_NOALLOC_MAX_PARTIALS; 512^3 is the largest cube): use "
+                    "ah_diagnostics on a context for larger lattices",
+                    P->nx, P->ny, P->nz, need, ah::diag_noalloc_capacity());
+    const ah::DiagCoef k = make_diag_coef(*P, tau, dt);
+    cudaError_t e;
+    if (is_fp64(*P)) {
+        ah::ConstFields<double> f;
+        for (int a = 0; a < AH_NFIELDS; ++a) f.f[a] = (const double *)dev_fields[a];
+        e = ah::launch_diag_noalloc<double>(f, k, P->nx, P->ny, P->nz, (ah::DiagPartial *)dev_totals,
+                                            (cudaStream_t)cuda_stream);
+    } else {
+        ah::ConstFields<float> f;
+        for (int a = 0; a < AH_NFIELDS; ++a) f.f[a] = (const float *)dev_fields[a];
+        e = ah::launch_diag_noalloc<float>(f, k, P->nx, P->ny, P->nz, (ah::DiagPartial *)dev_totals,
+                                           (cudaStream_t)cuda_stream);
+    }
+    if (e != cudaSuccess) return cuda_fail(e, "ah_readout_noalloc: scratch look-up or kernel launch");
+    return AH_OK;
+}
+
 // ------------------------------------------------------------------------------------------------ test hooks
 
 int ah_test_trig(const float *dev_x, float *dev_sin, float *dev_cos, float *dev_plaq_sin, size_t n,

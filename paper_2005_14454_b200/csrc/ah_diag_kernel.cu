@@ -10,6 +10,8 @@
 // numbers, is evaluated in fp64 from the stored values), accumulated in fp64, reduced per block
 // with warp shuffles, and summed over blocks in a fixed order by a second one-block kernel, so
 // results are bit-reproducible run to run.
+#include <atomic>
+
 #include "ah_kernels.h"
 #include "ah_diag_site.cuh"
 
@@ -274,6 +276,71 @@ template cudaError_t launch_diag<double>(const ConstFields<double> &, const Diag
                                          DiagPartial *, DiagPartial *, int8_t *, uint8_t *, cudaStream_t);
 template cudaError_t launch_diag_partials<float>(const ConstFields<float> &, const DiagCoef &, int, int, int, ZRange,
                                                  DiagPartial *, int8_t *, uint8_t *, const int *, cudaStream_t);
+
+// ------------------------------------------------------------------------- read-outs with no allocation
+//
+// ah_readout_noalloc (include/ah_b200.h): the two read-out kernels above, with the per-block partials in a fixed
+// array that is part of the loaded library image instead of in memory a context obtained from cudaMalloc.  It exists
+// for callers that must not allocate device memory when they want a read-out (see the header for who they are).
+//
+//   * Size: AH_NOALLOC_MAX_PARTIALS DiagPartial of 112 bytes = 7 MiB, resident on every GPU that loads the library
+//     until the process exits.  One partial per block of 64 x 4 x 8 sites, so the largest lattice is 512^3
+//     (or any other shape with ceil(nx/64) * ceil(ny/4) * ceil(nz/8) <= 65536).
+//   * g_noalloc_partials as written in HOST code is only a handle for the runtime, not an address a kernel can use;
+//     the device address is looked up once per device with cudaGetSymbolAddress (noalloc_scratch below) and that
+//     pointer is what the kernels get.
+//   * Nothing in the array has to be zero on entry: the first kernel writes partial vb for EVERY block vb < nvb
+//     (thread 0 of a block stores its partial whether or not the block holds active sites) and the second kernel reads
+//     exactly those nvb entries, so what an earlier, larger call left behind is never read and nothing is cleared.
+//   * All calls on a device share the array: calls whose kernels can be in flight at the same time race on it.
+
+namespace {
+
+constexpr int NOALLOC_MAX_PARTIALS = 65536;
+static __device__ __align__(256) DiagPartial g_noalloc_partials[NOALLOC_MAX_PARTIALS];
+
+constexpr int NOALLOC_MAX_DEVICES = 64;
+std::atomic<DiagPartial *> g_noalloc_ptr[NOALLOC_MAX_DEVICES];   // zero-initialised: not looked up yet
+
+// Device address of g_noalloc_partials on the CURRENT device.  The first call per device asks the runtime (which may
+// load the module on that device then); later calls read the cached pointer.  Two threads that both find the slot
+// empty both ask and store the same value.
+cudaError_t noalloc_scratch(DiagPartial **out)
+{
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= NOALLOC_MAX_DEVICES) return cudaErrorInvalidDevice;
+    DiagPartial *p = g_noalloc_ptr[dev].load(std::memory_order_acquire);
+    if (p == nullptr) {
+        e = cudaGetSymbolAddress((void **)&p, g_noalloc_partials);
+        if (e != cudaSuccess) return e;
+        if (p == nullptr) return cudaErrorInvalidSymbol;
+        g_noalloc_ptr[dev].store(p, std::memory_order_release);
+    }
+    *out = p;
+    return cudaSuccess;
+}
+
+}  // namespace
+
+int diag_noalloc_capacity() { return NOALLOC_MAX_PARTIALS; }
+
+template <typename real>
+cudaError_t launch_diag_noalloc(const ConstFields<real> &in, const DiagCoef &k, int nx, int ny, int nz,
+                                DiagPartial *result, cudaStream_t st)
+{
+    if (diag_num_blocks(nx, ny, nz) > NOALLOC_MAX_PARTIALS) return cudaErrorInvalidValue;   // callers check first
+    DiagPartial *scratch = nullptr;
+    cudaError_t e = noalloc_scratch(&scratch);
+    if (e != cudaSuccess) return e;
+    return launch_diag<real>(in, k, nx, ny, nz, ZRange{0, nz}, scratch, result, nullptr, nullptr, st);
+}
+
+template cudaError_t launch_diag_noalloc<float>(const ConstFields<float> &, const DiagCoef &, int, int, int,
+                                                DiagPartial *, cudaStream_t);
+template cudaError_t launch_diag_noalloc<double>(const ConstFields<double> &, const DiagCoef &, int, int, int,
+                                                 DiagPartial *, cudaStream_t);
 
 // ------------------------------------------------------------------------- trig test hook
 

@@ -60,6 +60,14 @@ cudaError_t launch_diag_partials(const ConstFields<real> &in, const DiagCoef &k,
 cudaError_t launch_diag_final(const DiagPartial *partials, int n, DiagPartial *result, cudaStream_t st, int n_alt = 0,
                               const int *use_alt = nullptr);
 
+// read-outs of a whole lattice with the partials in the library's own fixed device array (no allocation anywhere):
+// at most diag_noalloc_capacity() blocks, i.e. diag_num_blocks(nx, ny, nz) <= that; result as in launch_diag.  The
+// first call on a device looks the array's address up (cudaGetSymbolAddress).
+int diag_noalloc_capacity();
+template <typename real>
+cudaError_t launch_diag_noalloc(const ConstFields<real> &in, const DiagCoef &k, int nx, int ny, int nz,
+                                DiagPartial *result, cudaStream_t st);
+
 // tests only: evaluate the fp32 trig helpers on device arrays
 cudaError_t launch_test_trig(const float *x, float *s, float *c, float *ps, size_t n, cudaStream_t st);
 cudaError_t launch_test_trig_fast(const float *x, float *s, float *c, float *ss, size_t n, cudaStream_t st);
