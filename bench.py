@@ -12,6 +12,14 @@ rank evolves its own replica of the same lattice (a different seed), value = all
 divided by the slowest rank's device time, scaling "weak".  Started without a torchrun environment,
 `--gpus N` (N > 1) re-executes itself under `python -m torch.distributed.run` with N ranks on 127.0.0.1.
 
+Order of the device-timed windows (all CUDA events on the launching stream, max over ranks):
+  W warm-up steps -> one K-step window straight after the warm-up (`roofline.burst`: the board has not reached
+  its power cap yet) -> one S-step window (`roofline.sustained`, S = 200: BASELINE configs[3]'s "steady-state
+  throughput timed over 200 steps") -> R = 3 repetitions of the K-step window with the board in that steady state.
+  The top-level `value` / `ms_per_step` / `roofline` are the MEDIAN repetition ("3 repetitions, report
+  median and best"); `repetitions` lists all three and the best.  `clocks` spans the sustained window and the
+  repetitions (continuous load), so it holds enough samples to mean something.
+
 Prints ONE JSON line on rank 0.  `--impl reference` times the fp64 CPU oracle (oracle/) on the host
 cores on a bounded sample of the same workload.
 """
@@ -35,6 +43,7 @@ UNIT = "site-updates/s"
 BYTES_PER_SITE = 80.0          # 10 fp32 read + 10 fp32 written
 DX, DT, TAU0 = 0.5, 0.1, 1.0
 NOMINAL_HBM_GBS = 8000.0       # the metric's own denominator (8 TB/s)
+REPS = 3                       # repetitions of the K-step timed window ("report median and best")
 FALLBACK_HBM_GBS = 6650.0      # B200_PROFILING.md fallback
 
 
@@ -60,15 +69,19 @@ def parse():
                     help="N > 1: independent replicas (default; BASELINE north_star keeps one lattice on one GPU) or ONE "
                          "lattice of size x size x (N size) cut into z slabs with a per-step exchange of boundary planes "
                          "over NCCL (SURVEY 8(f)2; untimed on this 1-GPU pool)")
+    ap.add_argument("--oracle-leg", default="", help=argparse.SUPPRESS)   # "n,steps": one oracle timing (cpu_baseline's child)
     ap.add_argument("--selftest-launcher", action="store_true",
                     help="CPU-only check of the multi-rank launch path (gloo): no kernels, synthetic per-rank timings")
     return ap.parse_args()
 
 
-def workload_params(n, total_steps):
-    # configs[3]: radiation era (p=1), s=1; a(tau) normalised to 1 at the end of the run (reading #6)
-    return dict(dx=DX, lambda0=2.0, e0=1.0, sigma=1.0, s=1.0, p=1.0,
-                tau_ref=TAU0 + DT * total_steps, alpha=2.0, compact=1)
+TAU_REF = TAU0 + DT * (20 + 200)   # a(tau) = 1 after its 20 warm-up + 200 timed steps (reading #6)
+
+
+def workload_params(n):
+    # configs[3]: radiation era (p=1), s=1.  tau_ref is a constant of the workload: it does not move with --steps,
+    # --warmup, --pre-steps or --sustained-steps, so every invocation times the same physical configuration.
+    return dict(dx=DX, lambda0=2.0, e0=1.0, sigma=1.0, s=1.0, p=1.0, tau_ref=TAU_REF, alpha=2.0, compact=1)
 
 
 def measured_peak():
@@ -166,16 +179,64 @@ def oracle_rate(params, n_sample, steps, seed=1):
     return n_sample ** 3 * steps / el, el, o.num_threads()
 
 
+def cpu_model():
+    try:
+        for ln in Path("/proc/cpuinfo").read_text().splitlines():
+            if ln.lower().startswith("model name"):
+                return ln.split(":", 1)[1].strip()
+    except OSError:
+        pass
+    return "unknown"
+
+
+def oracle_leg_single_thread(n_sample, steps):
+    """The same oracle timing in a child process whose OpenMP runtime is limited to ONE thread (the oracle has no
+    thread-count call of its own and is not given one for this: OMP_NUM_THREADS must be set before it loads)."""
+    env = dict(os.environ, OMP_NUM_THREADS="1")
+    res = subprocess.run([sys.executable, str(Path(__file__).resolve()), "--oracle-leg", f"{n_sample},{steps}"], env=env,
+                         capture_output=True, text=True, timeout=600)
+    if res.returncode != 0:
+        return {"error": (res.stderr or res.stdout)[-300:]}
+    return json.loads(res.stdout.strip().splitlines()[-1])
+
+
+def run_oracle_leg(spec):
+    n_sample, steps = (int(v) for v in spec.split(","))
+    rate, el, threads = oracle_rate(workload_params(n_sample), n_sample, steps)
+    print(json.dumps({"lattice": f"{n_sample}^3", "steps": steps, "threads": threads, "value": rate, "unit": UNIT,
+                      "seconds": el}), flush=True)
+    return 0
+
+
 def cpu_baseline(params):
-    # ~10-30 s of CPU work: calibrate on 64^3, then run 256^3 (or 128^3 on a slow host) for a few steps
-    rate64, _, threads = oracle_rate(params, 64, 2)
-    n_s = 256 if rate64 > 1.5e6 else 128
-    steps = max(1, min(12, int(20.0 * rate64 * 3 / n_s ** 3)))   # larger lattices run ~3x the 64^3 rate
-    rate, el, threads = oracle_rate(params, n_s, steps)
+    """SURVEY 8(d) "oracle timing beside it": the fp64 oracle, as it stands, on 64^3 x 160 steps and 256^3 x 10 steps,
+    with OpenMP on all host cores (in this process) and single-threaded (child process); step counts of the slower
+    legs are cut so that the whole baseline stays within ~30 s of CPU work, and each leg says what it ran."""
+    legs = []
+
+    def leg(n_s, steps, rate, el, threads):
+        legs.append({"lattice": f"{n_s}^3", "steps": steps, "threads": threads, "value": rate, "unit": UNIT, "seconds": el})
+
+    cal, _, _ = oracle_rate(params, 64, 2)                         # calibration: sizes the legs below
+    steps64 = max(1, min(160, int(6.0 * cal / 64 ** 3)))           # 160 steps (BASELINE configs[0]) on any recent host
+    rate64, el, threads = oracle_rate(params, 64, steps64)
+    leg(64, steps64, rate64, el, threads)
+    steps256 = max(1, min(10, int(8.0 * rate64 * 3 / 256 ** 3)))   # larger lattices run ~3x the 64^3 rate
+    rate, el256, threads = oracle_rate(params, 256, steps256)
+    leg(256, steps256, rate, el256, threads)
+    # single thread: assume at best perfect scaling to size the legs (~10 s and ~6 s)
+    one = max(rate / max(threads, 1), 1.0)
+    s64 = max(1, min(160, int(10.0 * one / 64 ** 3)))
+    s256 = max(1, min(10, int(6.0 * one / 256 ** 3)))
+    for n_s, st in ((64, s64), (256, s256)):
+        r = oracle_leg_single_thread(n_s, st)
+        legs.append(r if "error" in r else {k: r[k] for k in ("lattice", "steps", "threads", "value", "unit", "seconds")})
     return {"value": rate, "unit": UNIT, "cores": threads, "kind": "oracle",
-            "sample": f"{n_s}^3 sub-lattice of the same workload (same parameters, seeded random-phase IC), "
-                      f"{steps} leapfrog steps, fp64, gcc -O2 -fopenmp, {el:.1f} s",
-            "host_cpus": os.cpu_count()}
+            "sample": f"256^3 sub-lattice of the same workload (same parameters, seeded random-phase IC), "
+                      f"{steps256} leapfrog steps, fp64, {threads} OpenMP threads, {el256:.1f} s; the other legs "
+                      f"(64^3 up to 160 steps, single-threaded runs) are under 'legs'",
+            "legs": legs, "host_cpus": os.cpu_count(), "cpu_model": cpu_model(),
+            "compiler": "gcc -O2 -std=c99 -fopenmp -ffp-contract=off (oracle/ah_oracle.py build())"}
 
 
 def run_reference(args):
@@ -183,7 +244,7 @@ def run_reference(args):
     if rank != 0:
         return 0
     n = args.size
-    params = workload_params(n, args.steps + args.warmup)
+    params = workload_params(n)
     from oracle import ah_oracle as o
     rate64, _, threads = oracle_rate(params, 64, 2)
     budget_s = 150.0
@@ -216,10 +277,6 @@ def run_reference(args):
 
 # ------------------------------------------------------------------------------- CUDA arm
 
-def total_steps(args):
-    return args.pre_steps + max(args.warmup, 3) + args.steps + args.sustained_steps
-
-
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -236,7 +293,7 @@ def run_ours(args):
     build.build()
 
     n, K, W = args.size, args.steps, max(args.warmup, 3)
-    params = workload_params(n, total_steps(args))
+    params = workload_params(n)
     if args.decomp == "slabs":
         return run_slabs(args, torch, dist, binding, replicas, params, rank, local, world)
     sim = binding.Simulation(params=binding.make_params(n, **params), device=f"cuda:{local}")
@@ -258,11 +315,11 @@ def run_ours(args):
         sim.step(nsteps, tau, DT)
         return 0
 
-    def timed_window(nsteps, tau):
+    def timed_window(nsteps, tau, sample_clocks=True):
         """(max-over-ranks ms, whole-job units, launches, clocks) of nsteps steps from tau, device-timed."""
         barrier()
-        sampler = ClockSampler(local)
-        if rank == 0:
+        sampler = ClockSampler(local) if (sample_clocks and rank == 0) else None
+        if sampler:
             sampler.start()
         l0 = sim.launch_count()
         ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
@@ -272,9 +329,13 @@ def run_ours(args):
         barrier()
         ms_local = ev0.elapsed_time(ev1)
         launches = sim.launch_count() - l0
-        clocks = sampler.stop() if rank == 0 else None
+        clocks = sampler.stop() if sampler else None
         ms, units = replicas.aggregate(ms_local, sites * nsteps, dist if world > 1 else None, device="cuda")
         return ms, units, launches, clocks
+
+    def window_record(nsteps, ms_w, units_w, clocks_w):
+        return {"steps": nsteps, "ms_per_step": ms_w / nsteps, "value": replicas.throughput(ms_w, units_w), "unit": UNIT,
+                "clocks": clocks_w}
 
     # ---- device-resident throughput
     sim.init_fields(replicas.replica_seed(1, rank))
@@ -284,18 +345,37 @@ def run_ours(args):
         tau += args.pre_steps * DT
     advance(W, tau)
     tau += W * DT
-    tau_timed = tau
-    ms, units, launches, clocks = timed_window(K, tau)
-    tau += K * DT
-    value = replicas.throughput(ms, units)
 
-    # ---- the same measurement over a longer window: what the board sustains under its power cap
+    # (1) K steps straight after the warm-up: the board is still below its power cap
+    ms_b, units_b, _, clocks_b = timed_window(K, tau)
+    tau += K * DT
+    burst = window_record(K, ms_b, units_b, clocks_b)
+
+    # (2) the longer window (BASELINE configs[3]: "steady-state throughput timed over 200 steps"), which also brings
+    # the board to the clocks it holds under its power cap; the clock sampler of the top-level record starts here
+    span_sampler = ClockSampler(local) if rank == 0 else None
+    if span_sampler:
+        span_sampler.start()
     sustained = None
     if args.sustained_steps > 0:
         ms_s, units_s, _, clocks_s = timed_window(args.sustained_steps, tau)
         tau += args.sustained_steps * DT
-        sustained = {"steps": args.sustained_steps, "ms_per_step": ms_s / args.sustained_steps,
-                     "value": replicas.throughput(ms_s, units_s), "unit": UNIT, "clocks": clocks_s}
+        sustained = window_record(args.sustained_steps, ms_s, units_s, clocks_s)
+
+    # (3) the K timed steps, REPS times, in that steady state; the median repetition is the line's value
+    tau_timed = tau
+    reps = []
+    for _ in range(REPS):
+        ms_r, units_r, launches_r, _ = timed_window(K, tau, sample_clocks=False)
+        tau += K * DT
+        reps.append((ms_r, units_r, launches_r))
+    clocks = span_sampler.stop() if span_sampler else None
+    ms, units, launches = sorted(reps)[len(reps) // 2]
+    value = replicas.throughput(ms, units)
+    repetitions = {"n": REPS, "steps_each": K, "ms_per_step": [r[0] / K for r in reps],
+                   "values": [replicas.throughput(r[0], r[1]) for r in reps],
+                   "median_value": value, "best_value": max(replicas.throughput(r[0], r[1]) for r in reps),
+                   "what": "back-to-back K-step windows after the sustained window; the line's value is the median"}
 
     # ---- end to end through the C ABI with HOST buffers: upload, K steps, download
     e2e = None
@@ -334,15 +414,17 @@ def run_ours(args):
                     "traffic": traffic, "traffic_source": traffic_src, "peak_source": peak_src, "kernel": kernel_name,
                     "algorithmic_bytes_per_launch": BYTES_PER_SITE * sites,
                     "frac_of_nominal_8TBs": achieved / NOMINAL_HBM_GBS,
-                    "timing": "CUDA events on the launching stream around the K timed steps; avg = elapsed/K "
+                    "timing": "CUDA events on the launching stream around the K timed steps of the median repetition "
+                              "(the board already at the clocks it sustains: see the module docstring); avg = elapsed/K "
                               "(each step = 1 tiled_step_kernel launch + 1 conditional-redo launch that exits "
                               "at once, ~2 us; see profiles/ launch list)"
                               + (f" (every {args.diag_every}th step is the DIAG instantiation + 2 small launches; "
                                  "the average is over all steps)" if diag else "")}
-        if sustained is not None:
-            ach_s = BYTES_PER_SITE * sites * world / (sustained["ms_per_step"] * 1e-3) / 1e9 / world
-            sustained.update(achieved=ach_s, frac=ach_s / peak, frac_of_nominal_8TBs=ach_s / NOMINAL_HBM_GBS)
-            roofline["sustained"] = sustained
+        for name, rec in (("sustained", sustained), ("burst", burst)):
+            if rec is not None:
+                ach = BYTES_PER_SITE * sites / (rec["ms_per_step"] * 1e-3) / 1e9
+                rec.update(achieved=ach, frac=ach / peak, frac_of_nominal_8TBs=ach / NOMINAL_HBM_GBS)
+                roofline[name] = rec
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
             "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -354,11 +436,13 @@ def run_ours(args):
                                    f"{' (BASELINE configs[3])' if n == 1024 and not diag else ''}"
                                    f"{' (BASELINE configs[4] row)' if diag and args.diag_every == 10 else ''}",
                        "kernel": kernel_name, "parallelism": "replicas only" if world > 1 else "single GPU",
-                       "tau_at_timed_window": tau_timed,
+                       "tau_at_timed_window": tau_timed, "tau_ref": TAU_REF,
+                       "windows": f"warm-up {W} -> burst {K} -> sustained {args.sustained_steps} -> {REPS} x {K} timed "
+                                  "(value = median repetition)",
                        "l2": "working set (80 B/site x N^3) exceeds the 126 MB L2 for N >= 128; no flush needed"
                              if n >= 128 else "working set fits in L2 (small-lattice case)"},
             "pct_of_8TBs_roofline": 100.0 * value / world * BYTES_PER_SITE / (NOMINAL_HBM_GBS * 1e9),
-            "roofline": roofline, "gpu_launches": int(launches), "clocks": clocks,
+            "roofline": roofline, "gpu_launches": int(launches), "clocks": clocks, "repetitions": repetitions,
         }
         if e2e is not None:
             line["e2e"] = e2e
@@ -388,16 +472,32 @@ def run_slabs(args, torch, dist, binding, replicas, params, rank, local, world):
     torch.cuda.synchronize()
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     l0 = ds.slab.launch_count()
+    sampler = ClockSampler(local) if rank == 0 else None
+    if sampler:
+        sampler.start()
     ev0.record(ds.slab.stream)
     ds.step(K, TAU0 + W * DT, DT)
     ev1.record(ds.slab.stream)
     torch.cuda.synchronize()
     dist.barrier()
+    clocks = sampler.stop() if sampler else None
     ms, units = replicas.aggregate(ev0.elapsed_time(ev1), float(n) ** 3 * K, dist if world > 1 else None,
                                    device="cuda" if dist.get_backend() == "nccl" else "cpu")
     if rank == 0:
         value = replicas.throughput(ms, units)
+        peak, peak_src = measured_peak()
+        # per GPU: one slab of n^3 sites per step = 3 step-kernel launches (two boundary planes, then the interior)
+        achieved = BYTES_PER_SITE * float(n) ** 3 / (ms / K * 1e-3) / 1e9
+        roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                    "traffic": None, "peak_source": peak_src, "kernel": "tiled_step_kernel (per slab: 2 boundary launches "
+                    "+ 1 interior launch per step)", "algorithmic_bytes_per_launch": BYTES_PER_SITE * float(n) ** 3,
+                    "frac_of_nominal_8TBs": achieved / NOMINAL_HBM_GBS,
+                    "timing": "CUDA events on the slab's compute stream around the K timed steps, max over ranks; "
+                              "per-GPU bytes = 80 B x the slab's own sites per step"}
         print(json.dumps({
+            "roofline": roofline, "clocks": clocks, "e2e": None, "cpu_baseline": None,
+            "note": "z-slab decomposition (SURVEY 8(f)2), outside BASELINE's single-GPU north_star: no host-buffer (e2e) "
+                    "leg and no oracle leg are run for it; the replica line (default --decomp) carries both",
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W, "ms_per_step": ms / K,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
             "config": {"workload": f"ONE {n}x{n}x{n * world} periodic lattice in {world} z slab(s), radiation era, s=1, "
@@ -446,6 +546,8 @@ def run_selftest_launcher(args):
 
 def main():
     args = parse()
+    if args.oracle_leg:
+        return run_oracle_leg(args.oracle_leg)
     if args.gpus < 1:
         raise SystemExit("--gpus must be >= 1")
     in_torchrun = "WORLD_SIZE" in os.environ and "RANK" in os.environ
