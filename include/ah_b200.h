@@ -165,8 +165,14 @@ int ah_winding_field(ah_ctx *ctx, int8_t *host_w3, uint8_t *host_near3);
 /*
  * ---- z slabs: one periodic lattice cut along z over several GPUs (the paper's domain decomposition, PAPER.md:122-142,
  * in its natural single-node form: 1-D slabs, one exchange of boundary planes per step, overlapped with the update of
- * the interior).  BASELINE's north_star keeps the measured build on ONE GPU; these calls are the correct-by-
- * construction multi-GPU path (tests cut a lattice into slabs on one GPU and require bit-identical fields).
+ * the interior).  BASELINE's north_star keeps the measured build on ONE GPU.  What has been executed: a lattice cut
+ * into slab contexts on ONE GPU (device-to-device copies stand in for the exchange), bit-identical to the single
+ * lattice.  What has NOT: the exchange between ranks over NCCL on more than one GPU (no multi-GPU node on this pool;
+ * tests/test_gpu_slabs.py holds a two-rank test that is skipped below two GPUs).
+ * Bit identity with the single lattice holds while every link angle stays inside the tiled kernel's domain
+ * (|th| < 2^16 rad): outside it the step is redone with the libm-based site kernel by the slab that READS the angle
+ * (its own planes, its ghost planes, the planes next to its boundary planes), not by the whole lattice, so the other
+ * slabs keep the tiled kernel's bits; every slab's result stays within the one-step tolerance either way.
  *
  * A slab context owns nz_own consecutive planes z_first .. z_first+nz_own-1 of the global lattice params->nz and
  * stores nz_own + 2 planes per array: plane 0 is the ghost copy of global plane z_first-1, planes 1 .. nz_own the

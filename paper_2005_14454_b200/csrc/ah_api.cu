@@ -683,11 +683,22 @@ int ah_slab_step(ah_ctx *c, double tau, double dt, int want_diag, void *comm_str
             if (rc != AH_OK) return rc;
         }
     }
-    if (want_diag && tiled) {
+    const bool split = !(want_diag && tiled) && own.hi - own.lo > 2;
+    if (tiled) {
+        // the planes the launches below read without owning them: the ghost planes and, when the boundary planes go
+        // first, their inner neighbours (ah_site_kernel.cu: th_range_check_kernel)
+        const int planes[4] = {own.lo - 1, own.hi, own.lo + 1, own.hi - 2};
+        e = ah::launch_th_range_check(flag, cur_fields<float>(c), c->P.nx, c->P.ny, planes, split ? 4 : 2,
+                                      ah::tiled_th_limit(), c->st);
+        if (e == cudaSuccess) c->launches += 1;
+    }
+    if (e != cudaSuccess) {
+        // nothing of the step has been enqueued yet
+    } else if (want_diag && tiled) {
         // fused read-outs: one launch over all own planes (no boundary / interior split on diagnostic steps)
         e = enqueue_step(c, c->P, tau, dt, own, 0, flag, next_flag);
         if (e == cudaSuccess) e = cudaEventRecord(c->ev_boundary, c->st);
-    } else if (own.hi - own.lo <= 2) {
+    } else if (!split) {
         e = enqueue_step(c, c->P, tau, dt, own, -1, flag, next_flag);
         if (e == cudaSuccess) e = cudaEventRecord(c->ev_boundary, c->st);
     } else {

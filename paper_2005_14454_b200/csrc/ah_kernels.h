@@ -38,6 +38,11 @@ int tiled_chunk(int nx, int ny, int nz, bool diag = false);        // z planes p
 cudaError_t launch_site_redo(const int *flag, int *clear, const ConstFields<float> &in, const Fields<float> &out,
                              const StepCoef<float> &k, int nx, int ny, int nz, ZRange zr, cudaStream_t st);
 cudaError_t tiled_setup();  // one-time function attributes (shared-memory carve-out)
+float tiled_th_limit();     // the kernel's domain: every |th| below this (2^16 rad)
+// z slabs (ah_site_kernel.cu): raise *flag when a link angle of one of the np <= 4 listed planes is outside the tiled
+// kernel's domain (planes a slab launch reads without owning them)
+cudaError_t launch_th_range_check(int *flag, const ConstFields<float> &in, int nx, int ny, const int *planes, int np,
+                                  float limit, cudaStream_t st);
 
 // diagnostics (ah_diag_kernel.cu)
 //   partials: device array of at least diag_num_blocks(...) DiagPartial

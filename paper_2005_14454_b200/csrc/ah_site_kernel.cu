@@ -165,6 +165,38 @@ cudaError_t launch_site_redo(const int *flag, int *clear, const ConstFields<floa
     return launch_pdl(site_redo_kernel, dim3(148 * 4), dim3(256), 0, st, flag, clear, in, out, k, nx, ny, nz, zr.lo, zr.hi);
 }
 
+// z slabs: a tiled launch checks the link angles of the planes it OWNS against its polynomial domain, and on a whole
+// lattice every plane is owned by some CTA of the same launch.  A slab launch also reads planes it does not own: the
+// two ghost planes (another context's), and, when the boundary planes are launched ahead of the interior, the plane
+// next to each boundary plane.  This kernel raises the same flag for those planes BEFORE the step's launches, so that
+// the conditional redo of every launch that reads them sees it.
+__global__ void __launch_bounds__(256)
+th_range_check_kernel(int *flag, const float *tx, const float *ty, const float *tz, size_t plane, int z0, int z1, int z2,
+                      int z3, int np, float limit)
+{
+    const int zs[4] = {z0, z1, z2, z3};
+    bool bad = false;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < plane * (size_t)np; i += (size_t)gridDim.x * blockDim.x) {
+        const size_t at = (size_t)zs[i / plane] * plane + i % plane;
+        bad |= !(fmaxf(fabsf(tx[at]), fmaxf(fabsf(ty[at]), fabsf(tz[at]))) < limit);
+    }
+    if (bad) *flag = 1;
+}
+
+cudaError_t launch_th_range_check(int *flag, const ConstFields<float> &in, int nx, int ny, const int *planes, int np,
+                                  float limit, cudaStream_t st)
+{
+    if (np < 1 || np > 4) return cudaErrorInvalidValue;
+    int z[4] = {planes[0], planes[0], planes[0], planes[0]};
+    for (int a = 0; a < np; ++a) z[a] = planes[a];
+    const size_t plane = (size_t)nx * ny;
+    const size_t want = (plane * (size_t)np + 255) / 256;
+    const unsigned grid = (unsigned)(want < 148 * 8 ? want : 148 * 8);
+    th_range_check_kernel<<<grid, 256, 0, st>>>(flag, in.f[TH_X], in.f[TH_Y], in.f[TH_Z], plane, z[0], z[1], z[2], z[3], np,
+                                                limit);
+    return cudaGetLastError();
+}
+
 template <typename real>
 cudaError_t launch_site_step(const ConstFields<real> &in, const Fields<real> &out,
                              const StepCoef<real> &k, int nx, int ny, int nz, ZRange zr, cudaStream_t st)

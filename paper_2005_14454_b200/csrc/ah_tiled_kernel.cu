@@ -890,6 +890,8 @@ static int chunk_for(int nx, int ny, int nz, int ty)
 
 int tiled_chunk(int nx, int ny, int nz, bool diag) { return chunk_for(nx, ny, nz, diag ? TILE_Y_DIAG : TILE_Y); }
 
+float tiled_th_limit() { return AH_TILED_TH_LIMIT; }
+
 // nz: number of planes the launch updates
 int tiled_num_blocks(int nx, int ny, int nz, bool diag)
 {

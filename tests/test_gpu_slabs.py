@@ -156,3 +156,64 @@ def test_distributed_slab_single_rank(ah):
         ds.slab.close()
     finally:
         dist.destroy_process_group()
+
+
+@pytest.mark.parametrize("z_big", [12, 1, 23])
+def test_slab_link_angles_beyond_the_tiled_domain_on_planes_a_launch_reads_but_does_not_own(ah, oracle, z_big):
+    """The tiled kernel checks |th| < 2^16 on the planes a launch owns.  A slab launch also reads its two ghost planes
+    (z_big = 12 and 23 are slab 0's upper and lower ghosts here) and, with the boundary planes launched first, the plane
+    next to each boundary plane (z_big = 1 is read by slab 0's separately launched plane 0): an angle out of range there
+    must send every launch of that slab through the libm redo, exactly as it does on a whole lattice.  So slab 0's
+    planes carry the bits of the site kernel, the other slab stays accurate, and the flag does not leak into the next,
+    in-range steps (there the slabs must again equal the single tiled lattice bit for bit)."""
+    nx, ny, nz = 128, 9, 24
+    model = dict(p=1.0, s=0.0)
+    P = ah.make_params(nx, ny, nz, **model)
+    f0 = inputs.random_state(nx, ny, nz, seed=22, th_amp=0.5)
+    f0[4, z_big, 4, 77] = 3.0e5        # th_x beyond 2^18: the polynomial pair is useless there
+    f0[6, z_big, 0, 0] = -7.0e4        # th_z just beyond 2^16
+    site = ah.Simulation(params=P)
+    site.set_kernel(ah.KERNEL_SITE)
+    site.set_fields(f0)
+    site.step(1, 2.0, 0.1)
+    want = site.get_fields()
+    grp = ah.SlabGroup(P, 2)           # slab 0: planes 0..11 (ghosts 23, 12); slab 1: planes 12..23 (ghosts 11, 0)
+    assert all(s.get_kernel() == ah.KERNEL_TILED for s in grp.slabs)
+    grp.set_fields(f0)
+    grp.step(1, 2.0, 0.1)
+    got = grp.get_fields()
+    assert np.array_equal(got[:, 0:12], want[:, 0:12])
+    ref = oracle.step(oracle.make_params(nx, ny, nz, **model), f0.copy(), 1, 2.0, 0.1)
+    for sl, tol in ((slice(0, 2), 1e-5), (slice(4, 7), 1e-6)):        # as in the whole-lattice redo test
+        assert np.abs(got[sl] - ref[sl]).max() <= tol * np.abs(ref[sl]).max()
+    # in-range steps afterwards: both slabs on the fast path again, flags cleared
+    f1 = inputs.random_state(nx, ny, nz, seed=23, th_amp=0.5)
+    one = ah.Simulation(params=P)
+    one.set_fields(f1)
+    one.step(3, 2.0, 0.1)
+    grp.set_fields(f1)
+    grp.step(3, 2.0, 0.1)
+    assert np.array_equal(grp.get_fields(), one.get_fields())
+    for sim in (site, one, grp):
+        sim.close()
+
+
+def test_distributed_slab_two_ranks_over_nccl(ah):
+    """The one leg of the z-slab path that a single GPU cannot run: two ranks, two GPUs, the boundary planes through
+    torch.distributed's NCCL point-to-point calls on the communication stream.  Skipped below two GPUs, which is every
+    box this project has been measured on: until a multi-GPU node runs it, that leg is unexecuted code."""
+    import subprocess
+    import sys
+    import socket
+    import torch
+    from pathlib import Path
+    if torch.cuda.device_count() < 2:
+        pytest.skip("needs 2 GPUs (the NCCL exchange between ranks has never run on this 1-GPU pool)")
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    worker = Path(__file__).resolve().parent / "slab_nccl_worker.py"
+    res = subprocess.run([sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node=2",
+                          "--master-addr", "127.0.0.1", "--master-port", str(port), str(worker)],
+                         capture_output=True, text=True, timeout=600)
+    assert res.returncode == 0 and "SLAB_NCCL_OK" in res.stdout, res.stdout[-2000:] + res.stderr[-2000:]
