@@ -84,6 +84,11 @@ typedef struct {
     double sum_p_L, sum_rho_L; /* sum_x p_x L_x, sum_x rho_x L_x: isotropic pressure and energy density of the five
                     pieces of L_x, weighted with L_x (reading #17)                               */
     double v2_omega; /* equation-of-state estimator (1 + 3 sum p L / sum rho L) / 2 (Eq. 17 right)  */
+    double xi_w_corr; /* xi_w above is the RAW estimator: string_length counts every pierced plaquette as one lattice
+                    spacing (a Manhattan length), which over-counts a smooth string; the values the paper prints for
+                    xi_W (Table 1) carry the usual correction L -> (pi/6) L of that over-count
+                    (reading #13).  xi_w_corr = sqrt(V / ((pi/6) string_length)) = xi_w sqrt(6/pi) is the
+                    number to compare with the paper; +inf when n_wind == 0, NaN without the winding read-out      */
 } ah_diag;
 
 /*

@@ -21,8 +21,10 @@
  * splitmix known answers; <v^2>_omega (Eq. 17 right; the paper leaves its
  * weight, rho and p undefined: DESIGN.md reading #17) by the same uniform-state
  * closed forms, by p = -rho/3 on the relaxed (critical-coupling) string pair,
- * by p = rho/3 for pure gauge radiation, and softly by Table 1.  Parity-unpinned items (stated in DESIGN.md): the
- * normalisation a(tau_ref) = 1 and the tau grid (the paper fixes neither).
+ * by p = rho/3 for pure gauge radiation.  Those pins fix rho and p for ANY weight.
+ * Parity unpinned (stated in DESIGN.md): the normalisation a(tau_ref) = 1 and the tau grid (the paper fixes neither:
+ * readings #6, #7), and the WEIGHT W_x = L_x of <v^2>_omega (reading #17): no CPU-side pin discriminates it; the only
+ * check that sees it is the GPU-side regression against the paper's printed Table 1 (1024^3 rows, 3 printed sigma).
  *
  * Conventions:
  *   site x = (x,y,z), linear index x + nx*(y + ny*z), periodic in all three;

@@ -67,6 +67,7 @@ class Diag(C.Structure):
         ("gauss_div_l2", C.c_double), ("gauss_charge_l2", C.c_double),
         ("xi_l", C.c_double),
         ("sum_p_L", C.c_double), ("sum_rho_L", C.c_double), ("v2_omega", C.c_double),
+        ("xi_w_corr", C.c_double),
     ]
 
     def asdict(self):

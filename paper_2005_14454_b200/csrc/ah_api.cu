@@ -296,9 +296,11 @@ void finish_diag(const ah_params &P, const ah::DiagPartial &r, double tau, ah_di
         const double V = (double)P.nx * P.ny * P.nz * P.dx * P.dx * P.dx;
         out->xi_w = out->n_wind > 0 ? std::sqrt(V / out->string_length)
                                     : std::numeric_limits<double>::infinity();
+        // the paper's xi_W: Manhattan length reduced by pi/6 (reading #13)
+        out->xi_w_corr = out->xi_w * std::sqrt(6.0 / 3.14159265358979323846);
     } else {
         out->n_wind = out->n_wind_xy = out->n_wind_xz = out->n_wind_yz = out->n_near_branch = out->n_big_plaq = -1;
-        out->string_length = out->xi_w = std::numeric_limits<double>::quiet_NaN();
+        out->string_length = out->xi_w = out->xi_w_corr = std::numeric_limits<double>::quiet_NaN();
     }
     out->sum_pi2_L = r.f[ah::DF_SPI];
     out->sum_grad2_L = r.f[ah::DF_SGR];

@@ -67,12 +67,13 @@ def main(argv=None):
         slope, icpt = np.polyfit(tau[m], xi[m], 1)
         # xi_w uses the raw plaquette count L_W = dx * n_W (reading #13).  Counting plaquettes
         # over-estimates the length of a smooth string by the Manhattan factor 6/pi (Hindmarsh et al. 2017, the
-        # paper's reference for this estimator), i.e. xi by sqrt(pi/6); the corrected slope is printed beside it.
+        # paper's reference for this estimator), i.e. xi by sqrt(pi/6); the library returns the corrected value as
+        # xi_w_corr, whose slope is printed beside the raw one.
         ml = m & np.isfinite(xl)
         if ml.sum() >= 3:
             summary.update(xi_l_slope=float(np.polyfit(tau[ml], xl[ml], 1)[0]))
         summary.update(xi_w_slope=float(slope), xi_w_intercept=float(icpt),
-                       xi_w_slope_manhattan_corrected=float(slope * np.sqrt(6.0 / np.pi)),
+                       xi_w_slope_manhattan_corrected=float(np.polyfit(tau[m], np.array([r["xi_w_corr"] for r in recs])[m], 1)[0]),
                        v2_phi_mean=float(v2[m].mean()), v2_phi_std=float(v2[m].std()),
                        v2_omega_mean=float(vw[m].mean()), v2_omega_std=float(vw[m].std()), n_fit=int(m.sum()))
     print(json.dumps(summary), flush=True)

@@ -745,32 +745,58 @@ def _table1():
     return rows
 
 
-@pytest.mark.parametrize("era", ["radiation", "matter"])
-def test_network_estimators_against_table1(ah, era):
-    """End to end on the CUDA path: a 512^3, s = 0 run to half the light-crossing time (1270 steps) with
-    all read-outs every 10 steps, against the values the paper PRINTS for its 1024^3 runs (tests/golden/table1.txt;
-    Table 1).  One seed at half the box size against a 20-run mean: the velocity estimators (seed
-    scatter ~0.01) must land within 0.035 of the printed values, the slopes of the mean string separation (seed
-    scatter ~0.03, three seeds give 0.24 ... 0.31) within 0.08.  This guards readings #13 (Manhattan factor of xi_W),
-    #15/#16 (L_x, mu) and #17 (<v^2>_omega) of DESIGN.md: a wrong term in L_x, rho or p moves <v^2> by > 0.1."""
-    ref = _table1()[era]
-    n, dt, tau0, steps, every = 512, 0.1, 1.0, 1270, 10
-    sim = ah.Simulation(params=ah.make_params(n, s=0.0, p=ref["p"], tau_ref=tau0 + steps * dt))
+def table1_run(ah, n, era_p, steps, every, fit_from, seed=1):
+    """One s = 0 run of n^3 sites from tau = 1 with all read-outs every `every` steps: the slopes of xi_L and of the
+    library's corrected xi_W (xi_w_corr, reading #13; no factor is applied in the tests) and the mean velocity
+    estimators over the records with tau >= fit_from, plus the worst relative Gauss residual."""
+    dt, tau0 = 0.1, 1.0
+    sim = ah.Simulation(params=ah.make_params(n, s=0.0, p=era_p, tau_ref=tau0 + steps * dt))
     assert sim.get_kernel() == ah.KERNEL_TILED
-    sim.init_fields(1)
+    sim.init_fields(seed)
     recs = sim.step_diag(steps, tau0, dt, every)
     sim.close()
     tau = np.array([r["tau"] for r in recs])
-    m = tau >= 80.0                                       # the paper's fit range for 512^3 boxes: [80, 128]
-    xi_l = np.polyfit(tau[m], np.array([r["xi_l"] for r in recs])[m], 1)[0]
-    xi_w = np.polyfit(tau[m], np.array([r["xi_w"] for r in recs])[m], 1)[0] * np.sqrt(6.0 / np.pi)   # reading #13
-    v2_phi = float(np.mean(np.array([r["v2_phi"] for r in recs])[m]))
-    v2_omega = float(np.mean(np.array([r["v2_omega"] for r in recs])[m]))
-    print(era, dict(xi_l_dot=xi_l, xi_w_dot=xi_w, v2_phi=v2_phi, v2_omega=v2_omega), "paper:", ref)
-    assert abs(v2_phi - ref["v2_phi"][0]) <= 0.035
-    assert abs(v2_omega - ref["v2_omega"][0]) <= 0.035
-    assert v2_omega > v2_phi                               # as in every row of Table 1
-    assert abs(xi_l - ref["xi_l"][0]) <= 0.08
-    assert abs(xi_w - ref["xi_w"][0]) <= 0.08
-    assert abs(xi_l - xi_w) <= 0.04                         # "fully consistent" estimators
-    assert max(r["gauss_rel"] for r in recs) < 1e-4         # Gauss's law at fp32 round-off throughout (s = 0)
+    m = tau >= fit_from
+    col = lambda key: np.array([r[key] for r in recs])[m]
+    return dict(size=n, seed=seed, steps=steps, every=every, fit_range=[float(tau[m][0]), float(tau[-1])],
+                xi_l_dot=float(np.polyfit(tau[m], col("xi_l"), 1)[0]), xi_w_dot=float(np.polyfit(tau[m], col("xi_w_corr"), 1)[0]),
+                v2_phi=float(col("v2_phi").mean()), v2_omega=float(col("v2_omega").mean()),
+                gauss_rel_max=float(max(r["gauss_rel"] for r in recs)))
+
+
+def record_table1(got):
+    """Printed, and written to gpurun_out/ when that directory exists (copied to profiles/ by hand)."""
+    import json
+    from pathlib import Path
+    print(json.dumps(got))
+    out = Path(__file__).resolve().parent.parent / "gpurun_out"
+    if out.is_dir():
+        (out / f"table1_{got['size']}_{got['era']}.json").write_text(json.dumps(got, indent=1) + "\n")
+
+
+@pytest.mark.parametrize("era", ["radiation", "matter"])
+def test_network_estimators_against_table1(ah, era):
+    """End to end on the CUDA path, quick version: a 512^3, s = 0 run to half the light-crossing time (1270 steps,
+    PAPER.md:63), read-outs every 10 steps, fit range [80, 128].
+
+    Which printed row?  Table 1 has a 512^3 row (PAPER.md:153 / :160), but it is the EARLIER single-GPU code's
+    (Correia & Martins 2020b, twelve runs), and it sits 0.03-0.04 above every row of this paper's own code in <v^2>
+    (0.31 against 0.272 / 0.283 / 0.282 for 1024^3 ... 4096^3).  This build lands on this paper's own rows (the 1024^3
+    run is compared like for like, within 3 printed sigma, in tests/test_gpu_fullsize.py) and NOT on the 2020b row: at
+    512^3 it gives <v^2>_phi = 0.257 / 0.200 (radiation / matter) against 0.31 / 0.25 +- 0.01 printed, i.e. 5 sigma
+    low, which this repository cannot resolve (the 2020b set-up is not in PAPER.md).  So this test keeps the bands of
+    an unlike-box comparison with this paper's 1024^3 rows (one seed at half the box size: 0.035 on the velocities,
+    0.08 on the slopes), bounds the distance to the 2020b row only loosely (0.07 / 0.09), and records both distances
+    (profiles/r03_table1.md)."""
+    rows = _table1()
+    ref, ref512 = rows[era], rows[era + "_512"]
+    got = table1_run(ah, 512, ref["p"], 1270, 10, 80.0)
+    got.update(era=era, paper_1024=ref, paper_512_2020b=ref512)
+    record_table1(got)
+    for key, band, band512 in (("v2_phi", 0.035, 0.07), ("v2_omega", 0.035, 0.07), ("xi_l", 0.08, 0.09), ("xi_w", 0.08, 0.09)):
+        mine = got[key if key.startswith("v2") else key + "_dot"]
+        assert abs(mine - ref[key][0]) <= band, (key, mine, ref[key])
+        assert abs(mine - ref512[key][0]) <= band512, (key, mine, ref512[key])
+    assert got["v2_omega"] > got["v2_phi"]                  # as in every row of Table 1
+    assert abs(got["xi_l_dot"] - got["xi_w_dot"]) <= 0.04   # "fully consistent" estimators (PAPER.md:173)
+    assert got["gauss_rel_max"] < 1e-4                      # Gauss's law at fp32 round-off throughout (s = 0)

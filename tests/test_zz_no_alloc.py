@@ -24,7 +24,7 @@ import pytest
 from paper_2005_14454_b200 import inputs
 
 INTS = ("n_wind", "n_wind_xy", "n_wind_xz", "n_wind_yz", "n_near_branch", "n_big_plaq")
-FLOATS = ("string_length", "xi_w", "sum_pi2_L", "sum_grad2_L", "sum_L", "v2_phi", "gauss_max", "gauss_l2", "gauss_rel",
+FLOATS = ("string_length", "xi_w", "xi_w_corr", "sum_pi2_L", "sum_grad2_L", "sum_L", "v2_phi", "gauss_max", "gauss_l2", "gauss_rel",
           "gauss_div_l2", "gauss_charge_l2", "xi_l", "sum_p_L", "sum_rho_L", "v2_omega")
 
 
