@@ -77,8 +77,11 @@ struct DiagPartial {
 // Link variables need cos/sin of an unbounded angle th (Eq. 10 never wraps it); plaquette
 // forces need sin of a (normally small) angle Phi.  fp32 path: round-to-nearest multiple of
 // pi/2 (resp. pi) by the add-magic-constant trick, two-term Cody-Waite reduction with FMA
-// (pi/2 = C1 + C2 to 48 bits, enough for |x| < 2^15), then odd/even polynomials fitted by
-// csrc/fit_trig_coeffs.py (relative error of the polynomials 7.5e-9 / 2.3e-10 / 1.1e-8, i.e.
+// (pi/2 = C1 + C2 to 48 bits, enough for |x| < 2^15), then odd/even polynomials whose coefficients
+// are weighted least-squares (near-minimax) fits on Chebyshev nodes of the reduced interval, made
+// once with numpy in fp64 and rounded to fp32; the fitting script is not part of the repository,
+// the coefficients below are bounded by tests/test_gpu_parity.py::test_trig_against_fp64 and
+// ::test_tiled_kernel_trig_against_fp64 (relative error of the polynomials 7.5e-9 / 2.3e-10 / 1.1e-8, i.e.
 // below half an fp32 ulp).  Measured against fp64 in tests/test_gpu_parity.py::test_trig.
 // Arguments beyond 2^15 take the libm path.  fp64 path: libm.
 

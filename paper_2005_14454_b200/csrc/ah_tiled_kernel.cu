@@ -4,8 +4,12 @@
 // once and written once (80 B per site).  DESIGN.md "Kernels / tiled step" has the derivation.
 //
 // Decomposition
-//   * a thread owns 4 consecutive x sites (128-bit accesses), a warp one 128-site row segment, a CTA a
-//     tile of 128 x TY sites; the CTA marches through a chunk of z planes;
+//   * a thread owns SPT consecutive x sites, a warp one row segment of 32 SPT sites, a CTA a tile of
+//     32 SPT x TY sites; the CTA marches through a chunk of z planes.  SPT = 4 (128-bit accesses, 128-site
+//     rows) when nx % 128 == 0, else SPT = 2 (64-bit accesses, 64-site rows; needs nx % 64 == 0).  TY = 6
+//     rows for the plain step, 5 for the DIAG instantiations (their read-out ring needs the shared memory);
+//     the arithmetic of a site does not depend on the tile it falls in (slabs and the two tilings agree
+//     bit for bit).  Numbers below are for SPT = 4;
 //   * the OLD phi, th planes (the only fields with a stencil) are staged in shared memory with their
 //     halo rows y0-1, y0+TY and halo columns x0-4..x0-1, x0+128..x0+131 by 1-D bulk TMA copies
 //     (cp.async.bulk, one per field row, issued by one elected lane of the warp that owns the row) into
