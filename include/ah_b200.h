@@ -216,6 +216,12 @@ int ah_slab_diagnostics(ah_ctx *ctx, double tau, double dt);
  * adding counts and sums[0..7] and taking the maximum of sums[8] (an all-reduce of 14 numbers), then ah_diag_finish. */
 int ah_slab_diag_partial(ah_ctx *ctx, int64_t host_counts[AH_NDIAG_INT], double host_sums[AH_NDIAG_FLT]);
 
+/* Totals of a whole lattice from the raw partial sums of its n_parts slabs (host arithmetic only): part r's counts are
+ * host_counts[r*AH_NDIAG_INT ..], its sums host_sums[r*AH_NDIAG_FLT ..]; counts and sums[0..7] add in the order
+ * given (fixed order: reproducible), sums[8] (max |G|) takes the maximum.  AH_EINVAL for null pointers or n_parts < 1. */
+int ah_diag_combine(int n_parts, const int64_t *host_counts, const double *host_sums,
+                    int64_t host_counts_out[AH_NDIAG_INT], double host_sums_out[AH_NDIAG_FLT]);
+
 /* Totals of a whole lattice -> the ah_diag record; host arithmetic only: xi_W, xi_L, <v^2>_phi, Gauss norms. */
 int ah_diag_finish(const ah_params *global_params, const int64_t host_counts[AH_NDIAG_INT],
                    const double host_sums[AH_NDIAG_FLT], double tau, ah_diag *host_out);

@@ -32,7 +32,7 @@ FIELD_NAMES = ("phi_re", "phi_im", "pi_re", "pi_im", "th_x", "th_y", "th_z", "ep
 # every symbol include/*.h declares (checked by tests/test_abi.py)
 EXPORTS = (
     "ah_create_slab", "ah_slab_step", "ah_slab_halo_ptrs", "ah_slab_exchange_done", "ah_slab_diagnostics",
-    "ah_slab_diag_partial", "ah_diag_finish", "ah_step_diag_sums", "ah_readout_noalloc",
+    "ah_slab_diag_partial", "ah_diag_finish", "ah_diag_combine", "ah_step_diag_sums", "ah_readout_noalloc",
     "ah_create", "ah_destroy", "ah_init_fields", "ah_set_fields", "ah_get_fields", "ah_current_bufs",
     "ah_step", "ah_step_cooling", "ah_diagnostics", "ah_step_diag", "ah_winding_field", "ah_set_kernel", "ah_get_kernel",
     "ah_launch_count", "ah_tiled_launch_info", "ah_coeffs", "ah_test_trig", "ah_test_trig_fast", "ah_last_error", "ah_version",
@@ -98,6 +98,7 @@ def lib():
     L.ah_slab_diagnostics.argtypes = [vp, dp, dp]
     L.ah_slab_diag_partial.argtypes = [vp, C.POINTER(C.c_int64), C.POINTER(dp)]
     L.ah_diag_finish.argtypes = [C.POINTER(Params), C.POINTER(C.c_int64), C.POINTER(dp), dp, C.POINTER(Diag)]
+    L.ah_diag_combine.argtypes = [ip, C.POINTER(C.c_int64), C.POINTER(dp), C.POINTER(C.c_int64), C.POINTER(dp)]
     L.ah_readout_noalloc.argtypes = [C.POINTER(Params), C.POINTER(vp), dp, dp, vp, vp]
     L.ah_destroy.argtypes = [vp]
     L.ah_init_fields.argtypes = [vp, C.c_uint64]
@@ -442,10 +443,13 @@ class SlabSimulation:
 
 
 def combine_partials(parts):
-    """Totals of per-slab (counts, sums): counts and all sums but the last add, the last (max |G|) takes the maximum."""
-    counts = [sum(p[0][a] for p in parts) for a in range(AH_NDIAG_INT)]
-    sums = [sum(p[1][a] for p in parts) for a in range(AH_NDIAG_FLT - 1)] + [max(p[1][AH_NDIAG_FLT - 1] for p in parts)]
-    return counts, sums
+    """ah_diag_combine: totals of per-slab (counts, sums) — marshalling only, the adding is done behind the C ABI."""
+    n = len(parts)
+    ci = (C.c_int64 * (AH_NDIAG_INT * n))(*[int(v) for p in parts for v in p[0]])
+    cf = (C.c_double * (AH_NDIAG_FLT * n))(*[float(v) for p in parts for v in p[1]])
+    co, so = (C.c_int64 * AH_NDIAG_INT)(), (C.c_double * AH_NDIAG_FLT)()
+    _check(lib().ah_diag_combine(n, ci, cf, co, so))
+    return list(co), list(so)
 
 
 class SlabGroup:

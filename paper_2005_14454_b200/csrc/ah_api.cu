@@ -774,6 +774,23 @@ int ah_slab_diag_partial(ah_ctx *c, int64_t counts[AH_NDIAG_INT], double sums[AH
     return AH_OK;
 }
 
+int ah_diag_combine(int n_parts, const int64_t *counts, const double *sums, int64_t counts_out[AH_NDIAG_INT],
+                    double sums_out[AH_NDIAG_FLT])
+{
+    if (!counts || !sums || !counts_out || !sums_out) return fail(AH_EINVAL, "ah_diag_combine: null pointer");
+    if (n_parts < 1) return fail(AH_EINVAL, "ah_diag_combine: n_parts must be >= 1 (got %d)", n_parts);
+    for (int a = 0; a < AH_NDIAG_INT; ++a) counts_out[a] = 0;
+    for (int a = 0; a < AH_NDIAG_FLT; ++a) sums_out[a] = 0.0;
+    for (int r = 0; r < n_parts; ++r) {
+        for (int a = 0; a < AH_NDIAG_INT; ++a) counts_out[a] += counts[r * AH_NDIAG_INT + a];
+        for (int a = 0; a < AH_NDIAG_FLT; ++a) {
+            const double v = sums[r * AH_NDIAG_FLT + a];
+            sums_out[a] = (a == ah::DF_GMAX) ? std::fmax(sums_out[a], v) : sums_out[a] + v;
+        }
+    }
+    return AH_OK;
+}
+
 int ah_diag_finish(const ah_params *global_params, const int64_t counts[AH_NDIAG_INT], const double sums[AH_NDIAG_FLT],
                    double tau, ah_diag *out)
 {
