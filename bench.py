@@ -69,6 +69,8 @@ def parse():
                     help="N > 1: independent replicas (default; BASELINE north_star keeps one lattice on one GPU) or ONE "
                          "lattice of size x size x (N size) cut into z slabs with a per-step exchange of boundary planes "
                          "over NCCL (SURVEY 8(f)2; untimed on this 1-GPU pool)")
+    ap.add_argument("--seed", type=int, default=1,
+                    help="seed of the random-phase initial condition (SURVEY 8(d): seeds 1-3 for run-to-run variance)")
     ap.add_argument("--oracle-leg", default="", help=argparse.SUPPRESS)   # "n,steps": one oracle timing (cpu_baseline's child)
     ap.add_argument("--selftest-launcher", action="store_true",
                     help="CPU-only check of the multi-rank launch path (gloo): no kernels, synthetic per-rank timings")
@@ -338,7 +340,7 @@ def run_ours(args):
                 "clocks": clocks_w}
 
     # ---- device-resident throughput
-    sim.init_fields(replicas.replica_seed(1, rank))
+    sim.init_fields(replicas.replica_seed(args.seed, rank))
     tau = TAU0
     if args.pre_steps > 0:
         sim.step(args.pre_steps, tau, DT)
@@ -436,7 +438,7 @@ def run_ours(args):
                                    f"{' (BASELINE configs[3])' if n == 1024 and not diag else ''}"
                                    f"{' (BASELINE configs[4] row)' if diag and args.diag_every == 10 else ''}",
                        "kernel": kernel_name, "parallelism": "replicas only" if world > 1 else "single GPU",
-                       "tau_at_timed_window": tau_timed, "tau_ref": TAU_REF,
+                       "tau_at_timed_window": tau_timed, "tau_ref": TAU_REF, "seed": args.seed,
                        "windows": f"warm-up {W} -> burst {K} -> sustained {args.sustained_steps} -> {REPS} x {K} timed "
                                   "(value = median repetition)",
                        "l2": "working set (80 B/site x N^3) exceeds the 126 MB L2 for N >= 128; no flush needed"

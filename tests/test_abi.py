@@ -147,3 +147,20 @@ def test_product_does_not_import_oracle():
     for path in (ROOT / "paper_2005_14454_b200").rglob("*"):
         if path.suffix in (".py", ".cu", ".cuh", ".h"):
             assert not bad.search(path.read_text()), f"{path} refers to the oracle"
+
+
+def test_diag_combine_adds_counts_and_sums_and_takes_the_maximum(ahlib):
+    """ah_diag_combine (host arithmetic of the z-slab read-outs): counts and the first eight sums add in the order
+    given, the last sum (max |G|) takes the maximum; bad arguments are refused."""
+    parts = [([1, 2, 3, 4, 5], [1.0, 2.0, 3.0, 4.0, 5.0, 6.0, 7.0, 8.0, 0.5]),
+             ([10, 20, 30, 40, 50], [0.5] * 8 + [0.9]),
+             ([2 ** 40, 0, 0, 0, 1], [1e-20] * 8 + [0.7])]
+    counts, sums = ahlib.combine_partials(parts)
+    assert counts == [11 + 2 ** 40, 22, 33, 44, 56]
+    assert sums[:8] == [(a + 0.5) + 1e-20 for a in (1.0, 2.0, 3.0, 4.0, 5.0, 6.0, 7.0, 8.0)]
+    assert sums[8] == 0.9
+    assert ahlib.combine_partials(parts[:1]) == (parts[0][0], parts[0][1])
+    L = ahlib.lib()
+    ci, cf = (C.c_int64 * 5)(), (C.c_double * 9)()
+    assert L.ah_diag_combine(0, ci, cf, ci, cf) == ahlib.AH_EINVAL
+    assert L.ah_diag_combine(1, None, cf, ci, cf) == ahlib.AH_EINVAL
