@@ -157,7 +157,7 @@ int ah_step_diag(ah_ctx *ctx, int n, double tau, double dt, int every, ah_diag *
  * ah_step_diag_sums — as ah_step_diag, but the records carry the Lagrangian-weighted estimators (xi_L, <v^2>_phi,
  * <v^2>_omega and their sums) and the Gauss residual only: the set the paper's timed runs evaluate every 5 steps
  * (PAPER.md:181).  The winding read-out is skipped (on the tiled kernel neither site phases nor link phases are
- * computed): n_wind* = n_near_branch = n_big_plaq = -1, string_length = xi_w = NaN.  All other fields are bit-identical
+ * computed): n_wind* = n_near_branch = n_big_plaq = -1, string_length = xi_w = xi_w_corr = NaN.  All other fields are bit-identical
  * to ah_step_diag's, and so are the fields the steps leave.
  */
 int ah_step_diag_sums(ah_ctx *ctx, int n, double tau, double dt, int every, ah_diag *host_out, int cap,
