@@ -199,7 +199,8 @@ int ah_create_slab(ah_ctx **out, const ah_params *global_params, int nz_own, int
                    int nbufs, size_t bytes_each, void *cuda_stream);
 
 /* One step of the slab's own planes.  want_diag != 0: also the read-outs D1-D3 of the ENTRY snapshot of the own
- * planes (fused on the tiled kernel), left on the device for ah_slab_diag_partial. */
+ * planes (fused on the tiled kernel, boundary planes first there too, so the exchange overlaps the interior on read-out
+ * steps as well), left on the device for ah_slab_diag_partial. */
 int ah_slab_step(ah_ctx *ctx, double tau, double dt, int want_diag, void *comm_stream);
 
 /* Device pointers of the boundary / ghost planes of the CURRENT state, per exchanged field (AH_NHALO of them, order

@@ -226,7 +226,9 @@ int ensure_diag_scratch(ah_ctx *c, int records)
 {
     const int own = c->zr.hi - c->zr.lo;
     int nb = ah::diag_num_blocks(c->P.nx, c->P.ny, own);
-    const int nbt = ah::tiled_num_blocks(c->P.nx, c->P.ny, own, true);
+    int nbt = ah::tiled_num_blocks(c->P.nx, c->P.ny, own, true);
+    if (c->slab && own > 2)   // boundary planes and interior read out by three launches (ah_slab_step)
+        nbt = 2 * ah::tiled_num_blocks(c->P.nx, c->P.ny, 1, true) + ah::tiled_num_blocks(c->P.nx, c->P.ny, own - 2, true);
     if (nbt > nb) nb = nbt;
     if (c->n_partials < nb) {
         if (c->d_partials) cudaFree(c->d_partials);
@@ -685,7 +687,7 @@ int ah_slab_step(ah_ctx *c, double tau, double dt, int want_diag, void *comm_str
             if (rc != AH_OK) return rc;
         }
     }
-    const bool split = !(want_diag && tiled) && own.hi - own.lo > 2;
+    const bool split = own.hi - own.lo > 2;
     if (tiled) {
         // the planes the launches below read without owning them: the ghost planes and, when the boundary planes go
         // first, their inner neighbours (ah_site_kernel.cu: th_range_check_kernel)
@@ -696,8 +698,38 @@ int ah_slab_step(ah_ctx *c, double tau, double dt, int want_diag, void *comm_str
     }
     if (e != cudaSuccess) {
         // nothing of the step has been enqueued yet
+    } else if (want_diag && tiled && split) {
+        // fused read-outs with the paper's order kept: the two boundary planes go through the DIAG
+        // instantiation first, each leaving its per-CTA partials behind the previous launch's, then the exchange may
+        // start; the interior follows, and ONE fixed-order total covers the partials of all three launches.  A link
+        // angle outside the tiled domain (flag, cumulative over the launches) makes the standalone kernel re-evaluate
+        // the whole own range into the same array, which the total then reads instead.
+        const int nx = c->P.nx, ny = c->P.ny, nza = c->nza;
+        const ah::StepCoef<float> k = make_coef<float>(c->P, tau, dt);
+        const ah::DiagCoef dk = make_diag_coef(c->P, tau, dt);
+        const ah::ConstFields<float> in = cur_fields<float>(c);
+        const ah::Fields<float> out = next_fields<float>(c);
+        const ah::ZRange parts[3] = {{own.lo, own.lo + 1}, {own.hi - 1, own.hi}, {own.lo + 1, own.hi - 1}};
+        int at = 0;
+        for (int r = 0; r < 3 && e == cudaSuccess; ++r) {
+            e = ah::launch_tiled_step(in, out, k, nx, ny, nza, parts[r], flag, c->st, &dk, c->d_partials + at);
+            if (e != cudaSuccess) break;
+            c->launches += 1;
+            at += ah::tiled_num_blocks(nx, ny, parts[r].hi - parts[r].lo, true);
+            if (r == 2) {
+                e = ah::launch_diag_partials<float>(in, dk, nx, ny, nza, own, c->d_partials, nullptr, nullptr, flag, c->st);
+                if (e == cudaSuccess)
+                    e = ah::launch_diag_final(c->d_partials, at, c->d_results, c->st,
+                                              ah::diag_num_blocks(nx, ny, own.hi - own.lo), flag);
+                if (e != cudaSuccess) break;
+                c->launches += 2;
+            }
+            e = ah::launch_site_redo(flag, next_flag, in, out, k, nx, ny, nza, parts[r], c->st);
+            if (e == cudaSuccess) c->launches += 1;
+            if (e == cudaSuccess && r == 1) e = cudaEventRecord(c->ev_boundary, c->st);
+        }
     } else if (want_diag && tiled) {
-        // fused read-outs: one launch over all own planes (no boundary / interior split on diagnostic steps)
+        // at most two own planes: one fused launch
         e = enqueue_step(c, c->P, tau, dt, own, 0, flag, next_flag);
         if (e == cudaSuccess) e = cudaEventRecord(c->ev_boundary, c->st);
     } else if (!split) {

@@ -217,3 +217,40 @@ def test_distributed_slab_two_ranks_over_nccl(ah):
                           "--master-addr", "127.0.0.1", "--master-port", str(port), str(worker)],
                          capture_output=True, text=True, timeout=600)
     assert res.returncode == 0 and "SLAB_NCCL_OK" in res.stdout, res.stdout[-2000:] + res.stderr[-2000:]
+
+
+@pytest.mark.parametrize("z_big", [12, 1])
+def test_slab_fused_record_with_a_link_angle_beyond_the_tiled_domain(ah, z_big):
+    """A read-out step of a slab goes through three DIAG launches (boundary planes first, then the interior) and one
+    total over their partials.  With a link angle out of range on a plane the slab reads, the flag makes the standalone
+    kernel re-evaluate that slab's own planes instead; the other slab keeps its fused partials.  Either way the record
+    of the entry snapshot (identical fields on both sides) must equal the single lattice's: integers exactly, sums to
+    the order of summation.  One step later the fields are bit-identical only if BOTH slabs were redone with the site
+    kernel, as the whole single lattice is (z_big = 12 lies on a plane both slabs read); with z_big = 1 slab 1 stays
+    on the tiled kernel (include/ah_b200.h: scope of bit identity), its fields differ from the site kernel's in the last
+    fp32 bit, and the second record agrees to fp32 round-off instead."""
+    nx, ny, nz = 128, 9, 24
+    P = ah.make_params(nx, ny, nz, p=1.0, s=0.0)
+    f0 = inputs.random_state(nx, ny, nz, seed=24, th_amp=0.5)
+    f0[4, z_big, 4, 77] = 3.0e5
+    one = ah.Simulation(params=P)
+    grp = ah.SlabGroup(P, 2)
+    one.set_fields(f0)
+    grp.set_fields(f0)
+    r1 = one.step_diag(2, 2.0, 0.1, 1)
+    r2 = grp.step(2, 2.0, 0.1, diag_every=1)
+    assert len(r1) == len(r2) == 2
+    ints = ("n_wind", "n_wind_xy", "n_wind_xz", "n_wind_yz", "n_near_branch", "n_big_plaq")
+    sums = ("sum_pi2_L", "sum_grad2_L", "sum_L", "sum_p_L", "sum_rho_L", "gauss_l2", "gauss_div_l2", "gauss_charge_l2")
+    for j, (a, b) in enumerate(zip(r1, r2)):
+        exact = j == 0 or z_big == 12
+        for key in ints:
+            assert abs(a[key] - b[key]) <= (0 if exact else a["n_near_branch"] + b["n_near_branch"]), key
+        if exact:
+            assert a["gauss_max"] == b["gauss_max"]
+        for key in sums:
+            assert b[key] == pytest.approx(a[key], rel=1e-11 if exact else 1e-6, abs=1e-300), key
+    same = np.array_equal(one.get_fields(), grp.get_fields())
+    assert same == (z_big == 12)
+    one.close()
+    grp.close()
